@@ -1,0 +1,208 @@
+/*
+ * bls_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, fp64 CPU statement of what the hot path computes: the box-least-squares (BLS)
+ * search of PAPER.md section 2.2.2 (L133-147): "phase the light curves at all possible periods and
+ * search for a transit-like signal" (L135); per trial period the curve is phased and "a range of
+ * durations and phases" is tested (L145).  The paper prints no formula; the statistic is the one
+ * BASELINE.json `north_star` fixes, SR = s^2/(r(1-r)), depth = s/(r(1-r)), which is the weighted
+ * least-squares fit of a two-level (in-box / out-of-box) signal (derivation: DESIGN.md "The
+ * statistic"; checked by brute force in tests/test_oracle_pins.py).  Steps O1..O5 are SURVEY.md
+ * section 8(c) / DESIGN.md "Readings".
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * build, load or call this file.  It shares no code, header, table or constant with the CUDA
+ * library under paper_1112_1701_b200/csrc/ and is never linked into it.
+ *
+ * Written so it can be checked against the definition by eye: no blocking, no prefix-sum tricks,
+ * no SIMD, no reordering.  Every box is summed directly (running sum over its bins, in bin order).
+ * Build: gcc -O2 -ffp-contract=off -shared -fPIC (no FMA contraction: the phase rule O4 is a
+ * sequence of individually rounded IEEE operations).
+ *
+ * Pins (tests/test_oracle_pins.py, tests/test_oracle_bins.py, tests/test_oracle_peaks.py):
+ *   oracle_prepare      - weighted-mean identities, weight-scaling invariance          (pinned)
+ *   oracle_widths       - table of DESIGN.md reading R9                               (pinned)
+ *   oracle_bin          - exact rational arithmetic (fractions.Fraction) + edge cases (pinned)
+ *   oracle_spectrum     - brute force over boxes from the least-squares definition,
+ *                         brute force over all point subsets (N<=12), noiseless injected box
+ *                         with closed-form depth and SR, invariants                   (pinned)
+ *   oracle_sr_at        - same brute force, box/complement symmetry                   (pinned)
+ *   oracle_peaks        - hand-written spectra with answers written out               (pinned)
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+
+/* O1 + O2 (reading R4, R5): w_i = sigma_i^-2 / sum_j sigma_j^-2 ; mu = sum w_i m_i ; x_i = m_i - mu.
+ * Sums run in index order.  Returns 0, or a per-curve data fault:
+ *   1 = fewer than 2 points, 2 = non-finite t/mag/sigma, 3 = sigma <= 0. */
+int oracle_prepare(int64_t n, const float *t, const float *mag, const float *sigma,
+                   double *w, double *x)
+{
+    if (n < 2) return 1;
+    for (int64_t i = 0; i < n; ++i) {
+        if (!isfinite((double)t[i]) || !isfinite((double)mag[i]) || !isfinite((double)sigma[i]))
+            return 2;
+        if (!(sigma[i] > 0.0f)) return 3;
+    }
+    double sw = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        double s = (double)sigma[i];
+        sw += 1.0 / (s * s);
+    }
+    if (!isfinite(sw) || !(sw > 0.0)) return 2;
+    double mu = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        double s = (double)sigma[i];
+        w[i] = (1.0 / (s * s)) / sw;
+        mu += w[i] * (double)mag[i];
+    }
+    for (int64_t i = 0; i < n; ++i) x[i] = (double)mag[i] - mu;
+    return 0;
+}
+
+/* O3 (reading R9): trial widths in whole bins, rounded outward from [q_min, q_max]:
+ *   kmin = max(1, floor(q_min*nb + 1e-9)),  kmax = min(nb-1, ceil(q_max*nb - 1e-9)). */
+void oracle_widths(int nb, double q_min, double q_max, int *kmin, int *kmax)
+{
+    int lo = (int)floor(q_min * (double)nb + 1e-9);
+    int hi = (int)ceil(q_max * (double)nb - 1e-9);
+    if (lo < 1) lo = 1;
+    if (hi > nb - 1) hi = nb - 1;
+    if (hi < lo) hi = lo;
+    *kmin = lo;
+    *kmax = hi;
+}
+
+/* O4 phase rule (reading R8): three individually rounded fp64 operations, no fused multiply-add.
+ *   p = RN(f*t) ; phi = p - floor(p) (exact) ; b = trunc(RN(phi*nb)) ; b = nb-1 if b >= nb. */
+int oracle_bin(double f, double t, int nb)
+{
+    volatile double p = f * t;              /* volatile: one rounding, never contracted */
+    double phi = p - floor(p);
+    volatile double xb = phi * (double)nb;
+    int b = (int)xb;
+    if (b >= nb) b = nb - 1;
+    return b;
+}
+
+/* O4 fold ("phases the light curve at that period", L145): W[b] += w_i, Y[b] += w_i x_i. */
+static void fold(int64_t n, const float *t, const double *w, const double *x, double f, int nb,
+                 double *W, double *Y)
+{
+    for (int b = 0; b < nb; ++b) { W[b] = 0.0; Y[b] = 0.0; }
+    for (int64_t i = 0; i < n; ++i) {
+        int b = oracle_bin(f, (double)t[i], nb);
+        W[b] += w[i];
+        Y[b] += w[i] * x[i];
+    }
+}
+
+/* O4 box search ("tests a range of durations and phases", L145).  Every start bin a in [0,nb) and
+ * every width k in [kmin,kmax]; bins are cyclic (reading R11); each box is a direct running sum in
+ * bin order; a box is valid iff r(1-r) > 0 (R10); ties go to the smallest k, then the smallest a
+ * (R12).  An all-invalid frequency reports SR = 0, a = 0, k = kmin, depth = 0. */
+static void search(int nb, int kmin, int kmax, const double *W, const double *Y,
+                   double *sr, int *best_a, int *best_k, double *depth)
+{
+    double bv = 0.0, bd = 0.0;
+    int ba = 0, bk = kmin;
+    for (int a = 0; a < nb; ++a) {
+        double r = 0.0, s = 0.0;
+        for (int k = 1; k <= kmax; ++k) {
+            int j = (a + k - 1) % nb;
+            r += W[j];
+            s += Y[j];
+            if (k < kmin) continue;
+            double den = r * (1.0 - r);
+            double v = (den > 0.0) ? (s * s) / den : 0.0;
+            if (v > bv || (v == bv && v > 0.0 && (k < bk || (k == bk && a < ba)))) {
+                bv = v; ba = a; bk = k; bd = s / den;
+            }
+        }
+    }
+    *sr = bv; *best_a = ba; *best_k = bk; *depth = bd;
+}
+
+/* O1..O4 for one curve over a frequency list.  Outputs have nf entries each.
+ * Returns the status of oracle_prepare; on a data fault the outputs are zero-filled. */
+int oracle_spectrum(int64_t n, const float *t, const float *mag, const float *sigma,
+                    int64_t nf, const double *freqs, int nb, int kmin, int kmax,
+                    double *sr, int32_t *best_a, int32_t *best_k, double *depth)
+{
+    double *w = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    double *x = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    double *W = (double *)malloc(sizeof(double) * (size_t)nb);
+    double *Y = (double *)malloc(sizeof(double) * (size_t)nb);
+    int st = oracle_prepare(n, t, mag, sigma, w, x);
+    for (int64_t q = 0; q < nf; ++q) {
+        if (st != 0) { sr[q] = 0.0; best_a[q] = 0; best_k[q] = kmin; depth[q] = 0.0; continue; }
+        fold(n, t, w, x, freqs[q], nb, W, Y);
+        int a, k;
+        search(nb, kmin, kmax, W, Y, &sr[q], &a, &k, &depth[q]);
+        best_a[q] = a; best_k[q] = k;
+    }
+    free(w); free(x); free(W); free(Y);
+    return st;
+}
+
+/* O4 for a single box (a, k) at one frequency: used by the comparator to score the box the CUDA
+ * path chose.  Returns SR (0 for an invalid box); *depth = s/(r(1-r)) or 0. */
+double oracle_sr_at(int64_t n, const float *t, const float *mag, const float *sigma,
+                    double f, int nb, int a, int k, double *depth)
+{
+    double *w = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    double *x = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    double *W = (double *)malloc(sizeof(double) * (size_t)nb);
+    double *Y = (double *)malloc(sizeof(double) * (size_t)nb);
+    double v = 0.0, d = 0.0;
+    if (oracle_prepare(n, t, mag, sigma, w, x) == 0) {
+        fold(n, t, w, x, f, nb, W, Y);
+        double r = 0.0, s = 0.0;
+        for (int kk = 1; kk <= k; ++kk) {
+            int j = (a + kk - 1) % nb;
+            r += W[j];
+            s += Y[j];
+        }
+        double den = r * (1.0 - r);
+        if (den > 0.0) { v = (s * s) / den; d = s / den; }
+    }
+    if (depth) *depth = d;
+    free(w); free(x); free(W); free(Y);
+    return v;
+}
+
+/* Folded bins at one frequency (for the tests that pin the fold itself). */
+int oracle_fold_bins(int64_t n, const float *t, const float *mag, const float *sigma,
+                     double f, int nb, double *W, double *Y)
+{
+    double *w = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    double *x = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    int st = oracle_prepare(n, t, mag, sigma, w, x);
+    if (st == 0) fold(n, t, w, x, f, nb, W, Y);
+    free(w); free(x);
+    return st;
+}
+
+/* O5 (reading R14): index q is a peak iff SR[q] > 0 and (q == 0 or SR[q] > SR[q-1]) and
+ * (q == nf-1 or SR[q] >= SR[q+1]); peaks are ranked by (SR descending, index ascending); the first
+ * kpk are written to idx[], padded with -1.  Returns the number of peaks written. */
+int oracle_peaks(int64_t nf, const double *sr, int kpk, int64_t *idx)
+{
+    int found = 0;
+    for (int j = 0; j < kpk; ++j) idx[j] = -1;
+    for (int64_t q = 0; q < nf; ++q) {
+        if (!(sr[q] > 0.0)) continue;
+        if (q > 0 && !(sr[q] > sr[q - 1])) continue;
+        if (q < nf - 1 && !(sr[q] >= sr[q + 1])) continue;
+        /* insert into the ranked list: strictly larger SR goes first; equal SR keeps index order */
+        int pos = found < kpk ? found : kpk;
+        while (pos > 0 && sr[q] > sr[idx[pos - 1]]) --pos;
+        if (pos >= kpk) continue;
+        int last = found < kpk ? found : kpk - 1;
+        for (int j = last; j > pos; --j) idx[j] = idx[j - 1];
+        idx[pos] = q;
+        if (found < kpk) ++found;
+    }
+    return found;
+}
