@@ -1,0 +1,171 @@
+/*
+ * bls.h -- C ABI of the B200-native box-least-squares (BLS) periodogram library.
+ *
+ * What it computes (section 2.2.2): for every light curve of a batch, "phase the
+ * light curves at all possible periods and search for a transit-like signal" (L135); at each trial
+ * period the curve is phased and "a range of durations and phases" is tested (L145).  The paper
+ * names the algorithm (BLS, Kovacs et al. 2002) and prints no formula; the statistic, binning and
+ * outputs are the ones BASELINE.json `north_star` fixes and DESIGN.md "Readings" R1-R17 spell out:
+ *
+ *   per curve      w_i = sigma_i^-2 / sum_j sigma_j^-2 ,  x_i = mag_i - sum_j w_j mag_j
+ *   per frequency  fold:  b_i = floor(nb * frac(f * t_i)) ;  W[b] += w_i ;  Y[b] += w_i x_i
+ *                  for every start bin a in [0,nb) and width k in [kmin,kmax] (cyclic):
+ *                      r = sum_{j<k} W[(a+j) mod nb] ,  s = sum_{j<k} Y[(a+j) mod nb]
+ *                      SR(a,k) = s^2 / (r (1-r))        (0 if r(1-r) <= 0)
+ *                  report max_{a,k} SR, its (a,k) and depth = s / (r(1-r))  (> 0 = dimming)
+ *   per curve      top-k local maxima of the SR spectrum (bls_topk).
+ *
+ * SR here is the SQUARE of the quantity Kovacs et al. call SR (reading R1); ordering is identical.
+ *
+ * Conventions
+ *   - Every function returns BLS_OK (0) or a negative bls_status.  None throws, aborts or prints.
+ *   - "DEVICE" pointers are CUDA device pointers on the plan's device; "HOST" pointers are ordinary
+ *     host memory.  The caller owns every batch / output buffer and keeps it alive until the stream
+ *     has drained.  The plan owns its copy of the frequency grid and all scratch.
+ *   - bls_run / bls_topk only enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL =
+ *     the legacy default stream).  They synchronise the stream only when plan scratch must grow.
+ *   - Structural faults (NULL, bad sizes, CUDA failure) return an error before anything is
+ *     launched.  Per-curve DATA faults (fewer than 2 points, non-finite values, sigma <= 0) are
+ *     found on the device and reported in status[c]; that curve's spectrum is zero-filled and its
+ *     peak list is empty (freq_index = -1), the rest of the batch is unaffected.
+ *   - A plan is used by one host thread at a time.  Distinct plans are independent.
+ *   - There is no CPU fallback: without a CUDA device bls_plan_create fails with BLS_ERR_CUDA.
+ */
+#ifndef BLS_B200_H
+#define BLS_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    BLS_OK = 0,
+    BLS_ERR_NULL = -1,        /* a required pointer is NULL                                        */
+    BLS_ERR_CONFIG = -2,      /* bad bls_config (sizes, q range, bin count, frequency grid)        */
+    BLS_ERR_BATCH = -3,       /* bad bls_batch (negative count, NULL arrays)                       */
+    BLS_ERR_ARG = -4,         /* bad call argument (k out of range, topk before run)               */
+    BLS_ERR_CUDA = -5,        /* a CUDA call failed (no device, out of memory, launch failure)     */
+    BLS_ERR_UNSUPPORTED = -6  /* shape the kernels cannot hold (curve too long for shared memory)  */
+} bls_status;
+
+/* per-curve data status written to bls_outputs.status / readable after bls_run */
+#define BLS_CURVE_OK 0
+#define BLS_CURVE_TOO_FEW 1      /* fewer than 2 points                    */
+#define BLS_CURVE_NONFINITE 2    /* NaN/Inf in t, mag or sigma             */
+#define BLS_CURVE_BAD_SIGMA 3    /* some sigma <= 0                        */
+
+typedef struct bls_plan bls_plan; /* opaque */
+
+/* Trial grid and capacities (BASELINE.json north_star: "frequency grid, bin count, duration
+ * fraction range").  Copied by bls_plan_create; the caller may free `freqs` afterwards. */
+typedef struct {
+    int32_t struct_size;   /* = sizeof(bls_config)                                                  */
+    int32_t device;        /* CUDA device ordinal                                                   */
+    int64_t n_freq;        /* nf >= 1                                                               */
+    const double *freqs;   /* HOST, nf trial frequencies in cycles/day, finite, > 0; NULL = uniform */
+    double f0, df;         /* used iff freqs == NULL: f_k = f0 + k*df evaluated in fp64 (R13)       */
+    int32_t n_bins;        /* nb, 4 <= nb <= 2048                                                   */
+    double q_min, q_max;   /* 0 < q_min <= q_max <= 0.5; widths kmin..kmax bins by reading R9:
+                              kmin = max(1, floor(q_min*nb + 1e-9)), kmax = min(nb-1, ceil(q_max*nb - 1e-9)) */
+    int32_t max_top_k;     /* 1..32: upper bound for bls_topk's k                                   */
+    int64_t scratch_bytes; /* budget for the plan-owned spectrum scratch; 0 = default (2 GiB)       */
+    uint32_t flags;        /* BLS_FLAG_*                                                            */
+} bls_config;
+
+#define BLS_FLAG_NONE 0u
+#define BLS_FLAG_CANONICAL_PHASE 1u /* compute every bin index with the slow 3-rounding fp64 rule
+                                       (R8) instead of the guarded fast path; results identical   */
+
+/* Ragged CSR batch of light curves (per star a list of HJD times, calibrated
+ * magnitudes and errors).  Curve c owns points [offsets[c], offsets[c+1]). */
+typedef struct {
+    int64_t n_curves;
+    const int64_t *offsets;  /* HOST, [n_curves+1], offsets[0] = 0, non-decreasing                 */
+    const float *t;          /* DEVICE, days relative to the curve's own origin; need not be sorted */
+    const float *mag;        /* DEVICE, magnitudes (larger = fainter)                              */
+    const float *sigma;      /* DEVICE, 1-sigma errors, > 0                                        */
+    const double *t_origin;  /* HOST, [n_curves] HJD of t = 0 for each curve, or NULL (= 0); only
+                                used to report bls_peak.epoch                                      */
+} bls_batch;
+
+/* Optional full-spectrum outputs; any pointer may be NULL = "do not write".  All DEVICE,
+ * caller-allocated, row-major [n_curves][nf]. */
+typedef struct {
+    float *sr;             /* per-frequency max over boxes of s^2/(r(1-r))                          */
+    uint16_t *best_start;  /* start bin a in [0,nb) of that box                                     */
+    uint16_t *best_width;  /* its width k in [kmin,kmax] bins                                       */
+    float *depth;          /* signed s/(r(1-r)) of that box; > 0 = dimming in magnitudes (R2)       */
+    int32_t *status;       /* [n_curves] BLS_CURVE_*                                                */
+} bls_outputs;
+
+/* One peak of a curve's SR spectrum (reading R14: local maximum, ranked by SR descending then
+ * index ascending).  freq_index = -1 pads lists shorter than k. */
+typedef struct {
+    int32_t freq_index;
+    float sr;
+    float depth;
+    uint16_t start_bin;
+    uint16_t width_bins;
+    double freq;   /* cycles/day                                                                    */
+    double epoch;  /* t_origin[c] + ((start_bin + width_bins/2.0)/nb)/freq : mid-box time of the
+                      first box after the origin                                                    */
+} bls_peak;
+
+/* what to ask bls_plan_query for */
+#define BLS_QUERY_KMIN 1
+#define BLS_QUERY_KMAX 2
+#define BLS_QUERY_NBINS 3
+#define BLS_QUERY_NFREQ 4
+#define BLS_QUERY_SCRATCH_BYTES 5   /* device bytes currently owned by the plan                    */
+#define BLS_QUERY_LAST_LAUNCHES 6   /* kernels launched by the last bls_run + bls_topk            */
+#define BLS_QUERY_LAST_CANONICAL 7  /* point-folds of the last bls_run that took the canonical
+                                       fp64 bin rule because the fast phase fell in its guard band
+                                       (synchronises the stream of that run)                       */
+#define BLS_QUERY_TILE_FREQS 8      /* frequencies per CTA work item in the search kernel          */
+#define BLS_QUERY_SEARCH_CTAS 9     /* CTAs of the last search launch                              */
+
+/* Validate cfg, copy the grid to the device, derive kmin/kmax and launch geometry.  *out_plan is
+ * set only on success. */
+int bls_plan_create(const bls_config *cfg, bls_plan **out_plan);
+
+/* Search every curve of `batch` at every frequency of the plan: prep (weights, mean removal) ->
+ * fold + box search per (curve, frequency) -> per-curve peak candidates kept in the plan for
+ * bls_topk.  `out` may be NULL (peaks only).  Enqueues on cuda_stream. */
+int bls_run(bls_plan *plan, const bls_batch *batch, const bls_outputs *out, void *cuda_stream);
+
+/* Write the k best peaks of every curve of the last bls_run to peaks (DEVICE, [n_curves*k]).
+ * 1 <= k <= max_top_k.  Enqueues on cuda_stream (must be the stream of that bls_run, or one
+ * ordered after it). */
+int bls_topk(bls_plan *plan, int32_t k, bls_peak *peaks, void *cuda_stream);
+
+/* Convenience for callers whose data lives in HOST memory: copies the batch to the device, runs
+ * bls_run + bls_topk, copies peaks (HOST, [n_curves*k]) and status (HOST, [n_curves], may be NULL)
+ * back, and synchronises.  host_batch uses HOST pointers for t / mag / sigma as well. */
+int bls_search_host(bls_plan *plan, const bls_batch *host_batch, int32_t k, bls_peak *peaks,
+                    int32_t *status);
+
+/* Diagnostic: bins[i] = the phase bin the fold kernel assigns to time t[i] (days) at frequency f[i]
+ * (cycles/day) with nb bins -- the same device function the search kernel uses (guarded fast phase,
+ * canonical fp64 rule inside the guard band; flags = BLS_FLAG_CANONICAL_PHASE forces the latter).
+ * f, t, bins: DEVICE arrays of n entries; *n_canonical (HOST, may be NULL) receives how many pairs
+ * took the canonical rule.  Synchronises.  Valid for |f t| < 2^18 cycles. */
+int bls_debug_fold_bins(int32_t device, const double *f, const double *t, int64_t n, int32_t n_bins,
+                        uint32_t flags, int32_t *bins, int64_t *n_canonical);
+
+/* NULL is a no-op. */
+int bls_plan_destroy(bls_plan *plan);
+
+int bls_plan_query(const bls_plan *plan, int32_t what, int64_t *value);
+
+/* Static string for a bls_status (never NULL). */
+const char *bls_strerror(int status);
+
+/* Last CUDA error string seen by this plan (static storage owned by the plan; "" if none). */
+const char *bls_plan_last_cuda_error(const bls_plan *plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BLS_B200_H */

@@ -58,6 +58,8 @@ def lib():
                                        _f64p, _f64p]
         L.oracle_peaks.restype = C.c_int
         L.oracle_peaks.argtypes = [C.c_int64, _f64p, C.c_int, _i64p]
+        L.oracle_bins_many.restype = None
+        L.oracle_bins_many.argtypes = [C.c_int64, _f64p, _f64p, C.c_int, _i32p]
         _lib = L
     return _lib
 
@@ -81,6 +83,13 @@ def widths(nb: int, q_min: float, q_max: float) -> Tuple[int, int]:
 
 def bin_index(f: float, t: float, nb: int) -> int:
     return lib().oracle_bin(float(f), float(t), int(nb))
+
+
+def bins_many(f, t, nb: int) -> np.ndarray:
+    f = np.ascontiguousarray(f, dtype=np.float64); t = np.ascontiguousarray(t, dtype=np.float64)
+    out = np.zeros(f.size, dtype=np.int32)
+    lib().oracle_bins_many(f.size, f, t, int(nb), out)
+    return out
 
 
 def fold_bins(t, mag, sigma, f: float, nb: int):

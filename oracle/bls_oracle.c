@@ -206,3 +206,9 @@ int oracle_peaks(int64_t nf, const double *sr, int kpk, int64_t *idx)
     }
     return found;
 }
+
+/* oracle_bin over arrays (for the bin-index parity test on very many (f, t) pairs). */
+void oracle_bins_many(int64_t n, const double *f, const double *t, int nb, int32_t *bins)
+{
+    for (int64_t i = 0; i < n; ++i) bins[i] = oracle_bin(f[i], t[i], nb);
+}

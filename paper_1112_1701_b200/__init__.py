@@ -1,0 +1,15 @@
+"""B200-native box-least-squares periodogram (arxiv 1112.1701, section 2.2.2): Python binding of the
+C-ABI library libbls_b200.so.  The CUDA kernels are the product; this package only marshals
+arguments.  Importing it never builds or falls back to anything on the CPU."""
+from .binding import (  # noqa: F401
+    BLS_FLAG_CANONICAL_PHASE,
+    BLS_FLAG_NONE,
+    BlsError,
+    EXPORTS,
+    LIB_PATH,
+    PEAK_DTYPE,
+    Plan,
+    debug_fold_bins,
+    lib,
+)
+from . import binding  # noqa: F401

@@ -1,0 +1,415 @@
+// C ABI of libbls_b200.so (include/bls.h): plan lifetime, validation, scratch ownership, launch
+// geometry and chunking.  Every arithmetic step of the path runs in the kernels of bls_prep.cu,
+// bls_search.cu and bls_peaks.cu; this file only validates, allocates and enqueues.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "bls_internal.cuh"
+
+using namespace bls;
+
+struct bls_plan {
+    int device = 0;
+    int sm_count = 0;
+    int max_smem_optin = 0;
+    int64_t nf = 0;
+    int nb = 0, kmin = 0, kmax = 0, max_top_k = 0;
+    uint32_t flags = 0;
+    double fmax = 0.0;
+    int64_t scratch_budget = 0;
+
+    double *d_freqs = nullptr;
+
+    // grow-on-demand buffers
+    PointRec *d_pts = nullptr;      int64_t cap_pts = 0;
+    CurveMeta *d_meta = nullptr;    int64_t cap_curves = 0;
+    int64_t *d_offsets = nullptr;
+    double *d_origin = nullptr;
+    PeakCand *d_cand = nullptr;
+    float *d_sr = nullptr;          int64_t cap_chunk = 0;   // curves per chunk the scratch can hold
+    uint32_t *d_ak = nullptr;
+    float *d_depth = nullptr;
+    unsigned long long *d_canon = nullptr;
+    // staging for bls_search_host
+    float *d_ht = nullptr, *d_hmag = nullptr, *d_hsig = nullptr;  int64_t cap_host_pts = 0;
+    bls_peak *d_hpeaks = nullptr;   int64_t cap_host_peaks = 0;
+    int32_t *d_hstatus = nullptr;   int64_t cap_host_status = 0;
+
+    int64_t last_n_curves = -1;
+    bool last_has_origin = false;
+    int64_t last_launches = 0;
+    int64_t last_search_ctas = 0;
+    int last_tiles_per_item = 0;
+    cudaStream_t last_stream = nullptr;
+    int64_t bytes_owned = 0;
+    char cuda_err[256] = {0};
+};
+
+namespace {
+
+int fail_cuda(bls_plan *p, cudaError_t e, const char *where)
+{
+    if (p) snprintf(p->cuda_err, sizeof(p->cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    cudaGetLastError();  // clear the sticky-less error state
+    return BLS_ERR_CUDA;
+}
+
+#define BLS_CUDA(p, call)                                         \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return fail_cuda((p), e__, #call); \
+    } while (0)
+
+template <typename T>
+int grow(bls_plan *p, T *&ptr, int64_t &cap, int64_t need, bool sync_first, cudaStream_t st)
+{
+    if (need <= cap && ptr) return BLS_OK;
+    if (need < 1) need = 1;
+    if (ptr) {
+        if (sync_first) BLS_CUDA(p, cudaStreamSynchronize(st));
+        BLS_CUDA(p, cudaFree(ptr));
+        p->bytes_owned -= cap * (int64_t)sizeof(T);
+        ptr = nullptr; cap = 0;
+    }
+    BLS_CUDA(p, cudaMalloc(&ptr, (size_t)need * sizeof(T)));
+    cap = need;
+    p->bytes_owned += need * (int64_t)sizeof(T);
+    return BLS_OK;
+}
+
+template <typename T>
+void release(T *&ptr)
+{
+    if (ptr) cudaFree(ptr);
+    ptr = nullptr;
+}
+
+void widths_from_q(int nb, double qmin, double qmax, int *kmin, int *kmax)
+{
+    int lo = (int)floor(qmin * (double)nb + 1e-9);
+    int hi = (int)ceil(qmax * (double)nb - 1e-9);
+    if (lo < 1) lo = 1;
+    if (hi > nb - 1) hi = nb - 1;
+    if (hi < lo) hi = lo;
+    *kmin = lo; *kmax = hi;
+}
+
+}  // namespace
+
+extern "C" {
+#pragma GCC visibility push(default)
+
+const char *bls_strerror(int status)
+{
+    switch (status) {
+        case BLS_OK: return "ok";
+        case BLS_ERR_NULL: return "required pointer is NULL";
+        case BLS_ERR_CONFIG: return "invalid bls_config";
+        case BLS_ERR_BATCH: return "invalid bls_batch";
+        case BLS_ERR_ARG: return "invalid argument";
+        case BLS_ERR_CUDA: return "CUDA failure (see bls_plan_last_cuda_error)";
+        case BLS_ERR_UNSUPPORTED: return "shape not supported by the kernels";
+        default: return "unknown status";
+    }
+}
+
+const char *bls_plan_last_cuda_error(const bls_plan *plan) { return plan ? plan->cuda_err : ""; }
+
+int bls_plan_create(const bls_config *cfg, bls_plan **out_plan)
+{
+    if (!cfg || !out_plan) return BLS_ERR_NULL;
+    if (cfg->struct_size != (int32_t)sizeof(bls_config)) return BLS_ERR_CONFIG;
+    if (cfg->n_freq < 1 || cfg->n_freq > 2147483647LL) return BLS_ERR_CONFIG;
+    if (cfg->n_bins < 4 || cfg->n_bins > 2048) return BLS_ERR_CONFIG;
+    if (!(cfg->q_min > 0.0) || !(cfg->q_max >= cfg->q_min) || !(cfg->q_max <= 0.5)) return BLS_ERR_CONFIG;
+    if (cfg->max_top_k < 1 || cfg->max_top_k > 32) return BLS_ERR_CONFIG;
+    if (cfg->scratch_bytes < 0) return BLS_ERR_CONFIG;
+
+    std::vector<double> grid((size_t)cfg->n_freq);
+    double fmax = 0.0;
+    for (int64_t k = 0; k < cfg->n_freq; ++k) {
+        double f = cfg->freqs ? cfg->freqs[k] : cfg->f0 + (double)k * cfg->df;
+        if (!isfinite(f) || !(f > 0.0)) return BLS_ERR_CONFIG;
+        grid[(size_t)k] = f;
+        if (f > fmax) fmax = f;
+    }
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || cfg->device < 0 || cfg->device >= ndev) {
+        cudaGetLastError();
+        return BLS_ERR_CUDA;   // no CPU fallback
+    }
+    bls_plan *p = new (std::nothrow) bls_plan();
+    if (!p) return BLS_ERR_CUDA;
+    p->device = cfg->device;
+    p->nf = cfg->n_freq;
+    p->nb = cfg->n_bins;
+    p->max_top_k = cfg->max_top_k;
+    p->flags = cfg->flags;
+    p->fmax = fmax;
+    p->scratch_budget = cfg->scratch_bytes > 0 ? cfg->scratch_bytes : (int64_t)2 << 30;
+    widths_from_q(p->nb, cfg->q_min, cfg->q_max, &p->kmin, &p->kmax);
+
+    cudaError_t e = cudaSetDevice(p->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device);
+    if (e == cudaSuccess) e = search_configure(p->max_smem_optin);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_freqs, (size_t)p->nf * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemcpy(p->d_freqs, grid.data(), (size_t)p->nf * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_canon, sizeof(unsigned long long));
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        release(p->d_freqs); release(p->d_canon);
+        delete p;
+        return BLS_ERR_CUDA;
+    }
+    p->bytes_owned = p->nf * (int64_t)sizeof(double) + 8;
+    if (search_smem_bytes(p->nb, 0) > (size_t)p->max_smem_optin) {   // the bins alone must fit
+        release(p->d_freqs); release(p->d_canon);
+        delete p;
+        return BLS_ERR_UNSUPPORTED;
+    }
+    *out_plan = p;
+    return BLS_OK;
+}
+
+int bls_plan_destroy(bls_plan *p)
+{
+    if (!p) return BLS_OK;
+    cudaSetDevice(p->device);
+    release(p->d_freqs); release(p->d_pts); release(p->d_meta); release(p->d_offsets);
+    release(p->d_origin); release(p->d_cand); release(p->d_sr); release(p->d_ak); release(p->d_depth);
+    release(p->d_canon); release(p->d_ht); release(p->d_hmag); release(p->d_hsig);
+    release(p->d_hpeaks); release(p->d_hstatus);
+    delete p;
+    return BLS_OK;
+}
+
+int bls_plan_query(const bls_plan *p, int32_t what, int64_t *value)
+{
+    if (!p || !value) return BLS_ERR_NULL;
+    switch (what) {
+        case BLS_QUERY_KMIN: *value = p->kmin; break;
+        case BLS_QUERY_KMAX: *value = p->kmax; break;
+        case BLS_QUERY_NBINS: *value = p->nb; break;
+        case BLS_QUERY_NFREQ: *value = p->nf; break;
+        case BLS_QUERY_SCRATCH_BYTES: *value = p->bytes_owned; break;
+        case BLS_QUERY_LAST_LAUNCHES: *value = p->last_launches; break;
+        case BLS_QUERY_TILE_FREQS: *value = (int64_t)p->last_tiles_per_item * kTileFreqs; break;
+        case BLS_QUERY_SEARCH_CTAS: *value = p->last_search_ctas; break;
+        case BLS_QUERY_LAST_CANONICAL: {
+            if (p->last_n_curves < 0) return BLS_ERR_ARG;
+            unsigned long long v = 0;
+            if (cudaSetDevice(p->device) != cudaSuccess) return BLS_ERR_CUDA;
+            if (cudaStreamSynchronize(p->last_stream) != cudaSuccess) return BLS_ERR_CUDA;
+            if (cudaMemcpy(&v, p->d_canon, sizeof(v), cudaMemcpyDeviceToHost) != cudaSuccess) return BLS_ERR_CUDA;
+            *value = (int64_t)v;
+            break;
+        }
+        default: return BLS_ERR_ARG;
+    }
+    return BLS_OK;
+}
+
+int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_stream)
+{
+    if (!p || !b) return BLS_ERR_NULL;
+    if (b->n_curves < 0) return BLS_ERR_BATCH;
+    if (!b->offsets) return BLS_ERR_NULL;
+    const int64_t nc = b->n_curves;
+    if (b->offsets[0] != 0) return BLS_ERR_BATCH;
+    int64_t max_n = 0;
+    for (int64_t c = 0; c < nc; ++c) {
+        const int64_t n = b->offsets[c + 1] - b->offsets[c];
+        if (n < 0 || n > 2147483647LL / 64) return BLS_ERR_BATCH;
+        if (n > max_n) max_n = n;
+    }
+    const int64_t npts = b->offsets[nc];
+    if (npts > 0 && (!b->t || !b->mag || !b->sigma)) return BLS_ERR_NULL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    BLS_CUDA(p, cudaSetDevice(p->device));
+    p->last_n_curves = -1;
+    p->last_launches = 0;
+    p->last_stream = st;
+    if (nc == 0) { p->last_n_curves = 0; return BLS_OK; }
+
+    // ---- scratch (grows on demand; growing synchronises the stream) -----------------------------
+    int rc;
+    {
+        if (nc > p->cap_curves || !p->d_meta) {
+            if (p->d_meta) BLS_CUDA(p, cudaStreamSynchronize(st));
+            release(p->d_meta); release(p->d_offsets); release(p->d_origin); release(p->d_cand);
+            p->bytes_owned -= p->cap_curves * (int64_t)(sizeof(CurveMeta) + 16 + sizeof(PeakCand) * p->max_top_k);
+            p->cap_curves = 0;
+            BLS_CUDA(p, cudaMalloc(&p->d_meta, (size_t)nc * sizeof(CurveMeta)));
+            BLS_CUDA(p, cudaMalloc(&p->d_offsets, (size_t)(nc + 1) * sizeof(int64_t)));
+            BLS_CUDA(p, cudaMalloc(&p->d_origin, (size_t)nc * sizeof(double)));
+            BLS_CUDA(p, cudaMalloc(&p->d_cand, (size_t)nc * p->max_top_k * sizeof(PeakCand)));
+            p->cap_curves = nc;
+            p->bytes_owned += nc * (int64_t)(sizeof(CurveMeta) + 16 + sizeof(PeakCand) * p->max_top_k);
+        }
+    }
+    if ((rc = grow(p, p->d_pts, p->cap_pts, npts, true, st)) != BLS_OK) return rc;
+
+    const int64_t per_curve = p->nf * 12;                       // sr + ak + depth
+    int64_t chunk = p->scratch_budget / per_curve;
+    if (chunk < 1) chunk = 1;
+    if (chunk > nc) chunk = nc;
+    if (chunk > p->cap_chunk || !p->d_sr) {
+        if (p->d_sr) BLS_CUDA(p, cudaStreamSynchronize(st));
+        release(p->d_sr); release(p->d_ak); release(p->d_depth);
+        p->bytes_owned -= p->cap_chunk * per_curve;
+        p->cap_chunk = 0;
+        BLS_CUDA(p, cudaMalloc(&p->d_sr, (size_t)(chunk * p->nf) * sizeof(float)));
+        BLS_CUDA(p, cudaMalloc(&p->d_ak, (size_t)(chunk * p->nf) * sizeof(uint32_t)));
+        BLS_CUDA(p, cudaMalloc(&p->d_depth, (size_t)(chunk * p->nf) * sizeof(float)));
+        p->cap_chunk = chunk;
+        p->bytes_owned += chunk * per_curve;
+    }
+
+    // ---- metadata to the device (stream ordered; the caller keeps offsets alive until then) ------
+    BLS_CUDA(p, cudaMemcpyAsync(p->d_offsets, b->offsets, (size_t)(nc + 1) * sizeof(int64_t),
+                                cudaMemcpyHostToDevice, st));
+    p->last_has_origin = b->t_origin != nullptr;
+    if (b->t_origin)
+        BLS_CUDA(p, cudaMemcpyAsync(p->d_origin, b->t_origin, (size_t)nc * sizeof(double),
+                                    cudaMemcpyHostToDevice, st));
+    BLS_CUDA(p, cudaMemsetAsync(p->d_canon, 0, sizeof(unsigned long long), st));
+
+    // ---- a0 prep -------------------------------------------------------------------------------
+    BLS_CUDA(p, launch_prep(b->t, b->mag, b->sigma, p->d_offsets, nc, p->fmax, p->d_pts, p->d_meta,
+                            out ? out->status : nullptr, st));
+    p->last_launches += 1;
+
+    // ---- launch geometry of the search ---------------------------------------------------------
+    const int ntiles = (int)((p->nf + kTileFreqs - 1) / kTileFreqs);
+    size_t smem = search_smem_bytes(p->nb, max_n);
+    int pts_in_smem = 1;
+    if (smem > (size_t)p->max_smem_optin) {        // curve too long to stage: read it through L1/L2
+        pts_in_smem = 0;
+        smem = search_smem_bytes(p->nb, 0);
+    }
+    int ctas_per_sm = (int)((size_t)(228 * 1024) / (smem + 1024));
+    if (ctas_per_sm < 1) ctas_per_sm = 1;
+    if (ctas_per_sm > 2048 / kSearchThreads) ctas_per_sm = 2048 / kSearchThreads;
+    const int64_t target_ctas = (int64_t)p->sm_count * ctas_per_sm * 12;   // >= 12 waves hides the tail
+    int64_t items = (target_ctas + chunk - 1) / chunk;
+    if (items < 1) items = 1;
+    if (items > ntiles) items = ntiles;
+    int tiles_per_item = (int)((ntiles + items - 1) / items);
+    items = (ntiles + tiles_per_item - 1) / tiles_per_item;
+    p->last_tiles_per_item = tiles_per_item;
+
+    SearchArgs a;
+    a.pts = p->d_pts; a.offsets = p->d_offsets; a.meta = p->d_meta; a.freqs = p->d_freqs;
+    a.nf = (int)p->nf; a.nb = p->nb; a.kmin = p->kmin; a.kmax = p->kmax;
+    a.tiles_per_item = tiles_per_item; a.items_per_curve = (int)items;
+    a.pts_in_smem = pts_in_smem;
+    a.force_canonical = (p->flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0;
+    a.sr = p->d_sr; a.ak = p->d_ak; a.depth = p->d_depth;
+    a.u_sr = out ? out->sr : nullptr;
+    a.u_start = out ? out->best_start : nullptr;
+    a.u_width = out ? out->best_width : nullptr;
+    a.u_depth = out ? out->depth : nullptr;
+    a.canon_count = p->d_canon;
+
+    // ---- per chunk of curves: search -> peak candidates ------------------------------------------
+    p->last_search_ctas = 0;
+    for (int64_t base = 0; base < nc; base += chunk) {
+        const int64_t cc = (nc - base < chunk) ? nc - base : chunk;
+        a.curve_base = base;
+        BLS_CUDA(p, launch_search(a, cc, smem, st));
+        BLS_CUDA(p, launch_peaks(p->d_sr, p->d_ak, p->d_depth, p->d_meta, base, cc, (int)p->nf,
+                                 p->max_top_k, p->d_cand, st));
+        p->last_launches += 2;
+        p->last_search_ctas += cc * items;
+    }
+    p->last_n_curves = nc;
+    return BLS_OK;
+}
+
+int bls_debug_fold_bins(int32_t device, const double *f, const double *t, int64_t n, int32_t n_bins,
+                        uint32_t flags, int32_t *bins, int64_t *n_canonical)
+{
+    if (!f || !t || !bins) return BLS_ERR_NULL;
+    if (n < 0 || n_bins < 4 || n_bins > 2048) return BLS_ERR_ARG;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    unsigned long long *d_cnt = nullptr, h_cnt = 0;
+    if (cudaMalloc(&d_cnt, sizeof(h_cnt)) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    cudaError_t e = cudaMemset(d_cnt, 0, sizeof(h_cnt));
+    if (e == cudaSuccess) e = launch_debug_bins(f, t, n, n_bins, (flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0, bins, d_cnt, nullptr);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(&h_cnt, d_cnt, sizeof(h_cnt), cudaMemcpyDeviceToHost);
+    cudaFree(d_cnt);
+    if (e != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    if (n_canonical) *n_canonical = (int64_t)h_cnt;
+    return BLS_OK;
+}
+
+int bls_topk(bls_plan *p, int32_t k, bls_peak *peaks, void *cuda_stream)
+{
+    if (!p || !peaks) return BLS_ERR_NULL;
+    if (p->last_n_curves < 0) return BLS_ERR_ARG;
+    if (k < 1 || k > p->max_top_k) return BLS_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    BLS_CUDA(p, cudaSetDevice(p->device));
+    BLS_CUDA(p, launch_format_peaks(p->d_cand, p->max_top_k, k, p->last_n_curves, p->nb, p->d_freqs,
+                                    p->last_has_origin ? p->d_origin : nullptr, peaks, st));
+    p->last_launches += 1;
+    return BLS_OK;
+}
+
+int bls_search_host(bls_plan *p, const bls_batch *hb, int32_t k, bls_peak *peaks, int32_t *status)
+{
+    if (!p || !hb || !peaks) return BLS_ERR_NULL;
+    if (hb->n_curves < 0 || !hb->offsets) return BLS_ERR_BATCH;
+    if (k < 1 || k > p->max_top_k) return BLS_ERR_ARG;
+    const int64_t nc = hb->n_curves;
+    const int64_t npts = hb->offsets[nc];
+    if (npts < 0) return BLS_ERR_BATCH;
+    if (npts > 0 && (!hb->t || !hb->mag || !hb->sigma)) return BLS_ERR_NULL;
+    BLS_CUDA(p, cudaSetDevice(p->device));
+    cudaStream_t st = nullptr;
+    int rc;
+    if (npts > p->cap_host_pts || !p->d_ht) {
+        release(p->d_ht); release(p->d_hmag); release(p->d_hsig);
+        p->bytes_owned -= p->cap_host_pts * 12;
+        p->cap_host_pts = 0;
+        const int64_t need = npts > 0 ? npts : 1;
+        BLS_CUDA(p, cudaMalloc(&p->d_ht, (size_t)need * 4));
+        BLS_CUDA(p, cudaMalloc(&p->d_hmag, (size_t)need * 4));
+        BLS_CUDA(p, cudaMalloc(&p->d_hsig, (size_t)need * 4));
+        p->cap_host_pts = need;
+        p->bytes_owned += need * 12;
+    }
+    if ((rc = grow(p, p->d_hpeaks, p->cap_host_peaks, nc * k, false, st)) != BLS_OK) return rc;
+    if ((rc = grow(p, p->d_hstatus, p->cap_host_status, nc, false, st)) != BLS_OK) return rc;
+    if (npts > 0) {
+        BLS_CUDA(p, cudaMemcpyAsync(p->d_ht, hb->t, (size_t)npts * 4, cudaMemcpyHostToDevice, st));
+        BLS_CUDA(p, cudaMemcpyAsync(p->d_hmag, hb->mag, (size_t)npts * 4, cudaMemcpyHostToDevice, st));
+        BLS_CUDA(p, cudaMemcpyAsync(p->d_hsig, hb->sigma, (size_t)npts * 4, cudaMemcpyHostToDevice, st));
+    }
+    bls_batch db = *hb;
+    db.t = p->d_ht; db.mag = p->d_hmag; db.sigma = p->d_hsig;
+    bls_outputs out;
+    memset(&out, 0, sizeof(out));
+    out.status = p->d_hstatus;
+    if ((rc = bls_run(p, &db, &out, st)) != BLS_OK) return rc;
+    if (nc > 0) {
+        if ((rc = bls_topk(p, k, p->d_hpeaks, st)) != BLS_OK) return rc;
+        BLS_CUDA(p, cudaMemcpyAsync(peaks, p->d_hpeaks, (size_t)(nc * k) * sizeof(bls_peak),
+                                    cudaMemcpyDeviceToHost, st));
+        if (status)
+            BLS_CUDA(p, cudaMemcpyAsync(status, p->d_hstatus, (size_t)nc * sizeof(int32_t),
+                                        cudaMemcpyDeviceToHost, st));
+    }
+    BLS_CUDA(p, cudaStreamSynchronize(st));
+    return BLS_OK;
+}
+
+#pragma GCC visibility pop
+}  // extern "C"

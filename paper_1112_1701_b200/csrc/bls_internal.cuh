@@ -1,0 +1,104 @@
+// Internal declarations shared by the translation units of libbls_b200.so (sm_100a only).
+// Nothing here is visible through the C ABI (include/bls.h) and nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/bls.h"
+
+namespace bls {
+
+// One prepared point, 16 bytes so that one LDS.128 broadcast feeds a whole warp (DESIGN.md
+// "Data layout").  t is widened to fp64 once here instead of once per point-fold.
+struct __align__(16) PointRec {
+    double t;      // days relative to the curve's origin (exactly the caller's fp32 value)
+    uint32_t qw;   // rint(w_i * SW)            fixed-point weight
+    int32_t qy;    // rint(w_i * x_i * SY)      fixed-point weighted residual
+};
+
+// Per-curve constants written by the prep kernel.
+struct CurveMeta {
+    float cw;          // 1/SW : bin integer -> weight fraction r
+    float cy;          // 1/SY : bin integer -> weighted residual s (0 for a constant curve)
+    int32_t status;    // BLS_CURVE_*
+    int32_t force_canonical;  // 1: |f t| may reach 2^19 cycles, the fast phase is not valid
+    double tabs_max;   // max |t|
+    double wx2;        // sum_i w_i x_i^2  (upper bound of SR)
+};
+
+// Peak candidate kept in the plan between bls_run and bls_topk.
+struct PeakCand {
+    int32_t freq_index;   // -1 = none
+    float sr;
+    float depth;
+    uint32_t ak;          // start | width << 16
+};
+
+constexpr int kTileFreqs = 32;        // frequencies per tile = lanes of a warp
+constexpr int kSearchThreads = 256;   // 8 warps per CTA
+constexpr int kPrepThreads = 256;
+constexpr int kPeakThreads = 256;
+constexpr int kStartsPerThread = 4;   // register tile of the box search (A)
+
+struct SearchArgs {
+    const PointRec *pts;        // [n_points] prepared points of the whole batch
+    const int64_t *offsets;     // device copy of the CSR offsets
+    const CurveMeta *meta;      // [n_curves]
+    const double *freqs;        // [nf]
+    int nf, nb, kmin, kmax;
+    int tiles_per_item, items_per_curve;
+    int64_t curve_base;         // first curve of this chunk
+    int pts_in_smem;            // 1: stage the curve in shared memory, 0: read it through L1
+    int force_canonical;        // BLS_FLAG_CANONICAL_PHASE
+    float *sr;                  // chunk scratch, [chunk_curves][nf]
+    uint32_t *ak;
+    float *depth;
+    float *u_sr;                // optional user outputs, [n_curves][nf] (whole batch), or NULL
+    uint16_t *u_start;
+    uint16_t *u_width;
+    float *u_depth;
+    unsigned long long *canon_count;
+};
+
+constexpr double kPhaseMagic = 1572864.0;   // 1.5 * 2^20: ulp = 2^-32, valid for |f t| < 2^19
+
+#ifdef __CUDACC__
+// Reading R8, the canonical rule: three individually rounded fp64 operations, no FMA.
+__device__ __noinline__ int canonical_bin(double f, double t, int nb);
+
+// Fast phase.  y = RN(f t + 1.5*2^20) has ulp 2^-32, so its low
+// mantissa word is frac(f t) in units of 2^-32 cycle (error <= 2^-33 cycle, one rounding).
+// ph * nb as a 64-bit product = (bin, position inside the bin in units of 2^-32 bin).  If the
+// position is within G = nb + 8 units of a bin edge the canonical rule decides instead; outside
+// the guard band both rules provably give floor(nb frac(f t)) (needs |f t| < 2^18).
+__device__ __forceinline__ int fold_bin(double f, double t, int nb, uint32_t G, bool force_canon,
+                                        unsigned int &n_canon)
+{
+    const double y = fma(f, t, kPhaseMagic);
+    const uint32_t ph = (uint32_t)__double2loint(y);
+    const unsigned long long pr = (unsigned long long)ph * (uint32_t)nb + (unsigned long long)G;
+    int bin = (int)(pr >> 32);
+    const uint32_t lo = (uint32_t)pr;                  // position * 2^32 + G
+    if (force_canon || lo < 2u * G) {
+        bin = canonical_bin(f, t, nb);
+        ++n_canon;
+    }
+    return bin;
+}
+#endif
+
+size_t search_smem_bytes(int nb, int64_t n_points_in_smem);
+cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int nb, int force_canon,
+                              int32_t *bins, unsigned long long *n_canon, cudaStream_t st);
+cudaError_t search_configure(int max_smem_optin);
+cudaError_t launch_prep(const float *t, const float *mag, const float *sigma, const int64_t *offsets,
+                        int64_t n_curves, double fmax, PointRec *pts, CurveMeta *meta, int32_t *u_status,
+                        cudaStream_t st);
+cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem, cudaStream_t st);
+cudaError_t launch_peaks(const float *sr, const uint32_t *ak, const float *depth, const CurveMeta *meta,
+                         int64_t curve_base, int64_t chunk_curves, int nf, int max_k, PeakCand *cand,
+                         cudaStream_t st);
+cudaError_t launch_format_peaks(const PeakCand *cand, int max_k, int k, int64_t n_curves, int nb,
+                                const double *freqs, const double *t_origin, bls_peak *out, cudaStream_t st);
+
+}  // namespace bls

@@ -1,0 +1,124 @@
+// a5 Output (reading R14): per-curve top-k peaks of the SR spectrum.
+// A sample q is a peak iff SR[q] > 0 and (q == 0 or SR[q] > SR[q-1]) and (q == nf-1 or
+// SR[q] >= SR[q+1]); peaks are ranked by SR descending, then index ascending.  One CTA per curve
+// selects max_k peaks in max_k rounds; each round is a block-wide argmax over the candidates that
+// rank strictly after the previous pick.  The spectrum row is nf*4 bytes (<= 2 MB) and stays in
+// L1/L2 across rounds, so HBM sees it once.
+#include "bls_internal.cuh"
+
+namespace bls {
+
+// rank key: larger = better.  SR > 0, so its bit pattern orders like its value.
+__device__ __forceinline__ unsigned long long rank_key(float sr, int q)
+{
+    return ((unsigned long long)__float_as_uint(sr) << 32) | (unsigned long long)(0xffffffffu - (uint32_t)q);
+}
+
+__global__ void __launch_bounds__(kPeakThreads)
+peaks_kernel(const float *__restrict__ sr, const uint32_t *__restrict__ ak, const float *__restrict__ depth,
+             const CurveMeta *__restrict__ meta, int64_t curve_base, int nf, int max_k,
+             PeakCand *__restrict__ cand)
+{
+    __shared__ unsigned long long sh[kPeakThreads / 32];
+    __shared__ unsigned long long s_prev;
+    const int64_t cl = blockIdx.x;
+    const int64_t c = curve_base + cl;
+    const float *row = sr + cl * (int64_t)nf;
+    PeakCand *out = cand + c * (int64_t)max_k;
+    const bool ok = meta[c].status == BLS_CURVE_OK;
+
+    unsigned long long prev = ~0ull;           // everything ranks after "infinity"
+    for (int round = 0; round < max_k; ++round) {
+        unsigned long long best = 0ull;        // 0 = no candidate (SR > 0 makes every real key > 0)
+        if (ok) {
+            for (int q = threadIdx.x; q < nf; q += kPeakThreads) {
+                const float v = row[q];
+                if (!(v > 0.f)) continue;
+                if (q > 0 && !(v > row[q - 1])) continue;
+                if (q < nf - 1 && !(v >= row[q + 1])) continue;
+                const unsigned long long key = rank_key(v, q);
+                if (key < prev && key > best) best = key;
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            unsigned long long other = __shfl_xor_sync(0xffffffffu, best, o);
+            best = other > best ? other : best;
+        }
+        if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = best;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned long long b = 0ull;
+#pragma unroll
+            for (int w = 0; w < kPeakThreads / 32; ++w) b = sh[w] > b ? sh[w] : b;
+            s_prev = b;
+            PeakCand pc;
+            if (b == 0ull) { pc.freq_index = -1; pc.sr = 0.f; pc.depth = 0.f; pc.ak = 0u; }
+            else {
+                const int q = (int)(0xffffffffu - (uint32_t)(b & 0xffffffffull));
+                pc.freq_index = q;
+                pc.sr = row[q];
+                pc.depth = depth[cl * (int64_t)nf + q];
+                pc.ak = ak[cl * (int64_t)nf + q];
+            }
+            out[round] = pc;
+        }
+        __syncthreads();
+        prev = s_prev;
+        if (prev == 0ull) {                    // list exhausted: pad the rest
+            for (int r2 = round + 1 + threadIdx.x; r2 < max_k; r2 += kPeakThreads) {
+                PeakCand pc; pc.freq_index = -1; pc.sr = 0.f; pc.depth = 0.f; pc.ak = 0u;
+                out[r2] = pc;
+            }
+            break;
+        }
+    }
+}
+
+__global__ void format_peaks_kernel(const PeakCand *__restrict__ cand, int max_k, int k, int64_t n_curves,
+                                    int nb, const double *__restrict__ freqs,
+                                    const double *__restrict__ t_origin, bls_peak *__restrict__ out)
+{
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_curves * (int64_t)k) return;
+    const int64_t c = i / k;
+    const int j = (int)(i % k);
+    const PeakCand pc = cand[c * (int64_t)max_k + j];
+    bls_peak p;
+    p.freq_index = pc.freq_index;
+    p.sr = pc.sr;
+    p.depth = pc.depth;
+    p.start_bin = (uint16_t)(pc.ak & 0xffffu);
+    p.width_bins = (uint16_t)(pc.ak >> 16);
+    if (pc.freq_index >= 0) {
+        p.freq = freqs[pc.freq_index];
+        const double mid = ((double)p.start_bin + 0.5 * (double)p.width_bins) / (double)nb;
+        p.epoch = (t_origin ? t_origin[c] : 0.0) + mid / p.freq;
+    } else {
+        p.freq = 0.0;
+        p.epoch = 0.0;
+    }
+    out[i] = p;
+}
+
+cudaError_t launch_peaks(const float *sr, const uint32_t *ak, const float *depth, const CurveMeta *meta,
+                         int64_t curve_base, int64_t chunk_curves, int nf, int max_k, PeakCand *cand,
+                         cudaStream_t st)
+{
+    if (chunk_curves <= 0) return cudaSuccess;
+    peaks_kernel<<<(unsigned)chunk_curves, kPeakThreads, 0, st>>>(sr, ak, depth, meta, curve_base, nf, max_k, cand);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_format_peaks(const PeakCand *cand, int max_k, int k, int64_t n_curves, int nb,
+                                const double *freqs, const double *t_origin, bls_peak *out, cudaStream_t st)
+{
+    const int64_t total = n_curves * (int64_t)k;
+    if (total <= 0) return cudaSuccess;
+    const int threads = 256;
+    const int64_t blocks = (total + threads - 1) / threads;
+    format_peaks_kernel<<<(unsigned)blocks, threads, 0, st>>>(cand, max_k, k, n_curves, nb, freqs, t_origin, out);
+    return cudaGetLastError();
+}
+
+}  // namespace bls

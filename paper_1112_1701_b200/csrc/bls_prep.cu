@@ -1,0 +1,145 @@
+// a0 Prep: once per curve,
+//   w_i = sigma_i^-2 / sum_j sigma_j^-2,  mu = sum_i w_i m_i,  x_i = m_i - mu      (readings R4, R5)
+// all sums in fp64, then the fixed-point records the search kernel folds:
+//   qw_i = rint(w_i * SW),        SW = 2^32 - 2N - 2            (sum_i qw_i < 2^32 for any subset)
+//   qy_i = rint(w_i x_i * SY),    SY = (2^31 - N - 2) / (0.5 sqrt(sum_i w_i x_i^2) (1 + 1e-12))
+// SY is safe for ANY subset of points: the least-squares residual of a two-level fit is >= 0, so
+// s^2 <= r(1-r) sum w x^2 <= sum w x^2 / 4.
+// One CTA per curve, fixed 256-thread strided accumulation + fixed tree => bitwise reproducible.
+#include "bls_internal.cuh"
+
+namespace bls {
+
+__device__ __forceinline__ double block_sum(double v, double *sh) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) sh[warp] = v;
+    __syncthreads();
+    double tot = 0.0;
+#pragma unroll
+    for (int w = 0; w < kPrepThreads / 32; ++w) tot += sh[w];
+    return tot;
+}
+
+__device__ __forceinline__ double block_max(double v, double *sh) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) sh[warp] = v;
+    __syncthreads();
+    double tot = 0.0;
+#pragma unroll
+    for (int w = 0; w < kPrepThreads / 32; ++w) tot = fmax(tot, sh[w]);
+    return tot;
+}
+
+__global__ void __launch_bounds__(kPrepThreads)
+prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const float *__restrict__ sigma,
+            const int64_t *__restrict__ offsets, double fmax_grid, PointRec *__restrict__ pts,
+            CurveMeta *__restrict__ meta, int32_t *__restrict__ u_status)
+{
+    __shared__ double sh[kPrepThreads / 32];
+    __shared__ int s_flags;
+    const int64_t c = blockIdx.x;
+    const int64_t beg = offsets[c], end = offsets[c + 1];
+    const int64_t n = end - beg;
+    if (threadIdx.x == 0) s_flags = 0;
+    __syncthreads();
+
+    // pass 1: validity, sum of inverse variances, max |t|
+    double acc = 0.0, tmax = 0.0;
+    int flags = 0;
+    for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
+        float ti = t[i], mi = mag[i], si = sigma[i];
+        if (!isfinite(ti) || !isfinite(mi) || !isfinite(si)) flags |= 1;
+        else if (!(si > 0.0f)) flags |= 2;
+        else {
+            double s = (double)si;
+            acc += 1.0 / (s * s);
+            tmax = fmax(tmax, fabs((double)ti));
+        }
+    }
+    if (flags) atomicOr(&s_flags, flags);
+    double sw = block_sum(acc, sh);
+    tmax = block_max(tmax, sh);
+    __syncthreads();
+    int status = BLS_CURVE_OK;
+    if (n < 2) status = BLS_CURVE_TOO_FEW;
+    else if (s_flags & 1) status = BLS_CURVE_NONFINITE;
+    else if (s_flags & 2) status = BLS_CURVE_BAD_SIGMA;
+    else if (!isfinite(sw) || !(sw > 0.0)) status = BLS_CURVE_NONFINITE;
+
+    if (status != BLS_CURVE_OK) {
+        for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
+            PointRec r; r.t = 0.0; r.qw = 0u; r.qy = 0;
+            pts[i] = r;
+        }
+        if (threadIdx.x == 0) {
+            CurveMeta m; m.cw = 0.f; m.cy = 0.f; m.status = status; m.force_canonical = 0;
+            m.tabs_max = 0.0; m.wx2 = 0.0;
+            meta[c] = m;
+            if (u_status) u_status[c] = status;
+        }
+        return;
+    }
+
+    // pass 2: weighted mean
+    acc = 0.0;
+    for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
+        double s = (double)sigma[i];
+        acc += ((1.0 / (s * s)) / sw) * (double)mag[i];
+    }
+    const double mu = block_sum(acc, sh);
+
+    // pass 3: weighted variance (bounds every box sum, sets the fixed-point scale of qy)
+    acc = 0.0;
+    for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
+        double s = (double)sigma[i];
+        double w = (1.0 / (s * s)) / sw;
+        double x = (double)mag[i] - mu;
+        acc += w * x * x;
+    }
+    const double wx2 = block_sum(acc, sh);
+
+    const double SW = 4294967296.0 - 2.0 * (double)n - 2.0;
+    const double sigw = sqrt(wx2);
+    const double SY = (sigw > 0.0 && isfinite(sigw))
+                          ? (2147483648.0 - (double)n - 2.0) / (0.5 * sigw * (1.0 + 1e-12)) : 0.0;
+
+    for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
+        double s = (double)sigma[i];
+        double w = (1.0 / (s * s)) / sw;
+        double x = (double)mag[i] - mu;
+        PointRec r;
+        r.t = (double)t[i];
+        r.qw = (uint32_t)__double2ll_rn(w * SW);
+        r.qy = (int32_t)__double2ll_rn(w * x * SY);
+        pts[i] = r;
+    }
+    if (threadIdx.x == 0) {
+        CurveMeta m;
+        m.cw = (float)(1.0 / SW);
+        m.cy = SY > 0.0 ? (float)(1.0 / SY) : 0.f;
+        m.status = BLS_CURVE_OK;
+        // the fast phase needs |f t| < 2^19 cycles
+        m.force_canonical = (fmax_grid * tmax < 262144.0) ? 0 : 1;
+        m.tabs_max = tmax;
+        m.wx2 = wx2;
+        meta[c] = m;
+        if (u_status) u_status[c] = BLS_CURVE_OK;
+    }
+}
+
+cudaError_t launch_prep(const float *t, const float *mag, const float *sigma, const int64_t *offsets,
+                        int64_t n_curves, double fmax, PointRec *pts, CurveMeta *meta, int32_t *u_status,
+                        cudaStream_t st)
+{
+    if (n_curves <= 0) return cudaSuccess;
+    prep_kernel<<<(unsigned)n_curves, kPrepThreads, 0, st>>>(t, mag, sigma, offsets, fmax, pts, meta, u_status);
+    return cudaGetLastError();
+}
+
+}  // namespace bls

@@ -1,0 +1,273 @@
+"""-m gpu: the CUDA path, called through the C ABI, against the fp64 oracle on the same seeded inputs.
+
+Element by element at sizes the oracle finishes in seconds (several frequency tiles + a ragged
+tail, ragged curve lengths, both cadences), then the edge cases.  Tolerances: tests/comparator.py
+(north_star: SR within 1e-4 relative; boxes identical except near-ties < 1e-6; peak lists matching).
+"""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from comparator import compare_peaks, compare_spectrum
+from gpu_common import run_gpu
+
+pytestmark = pytest.mark.gpu
+
+
+def check_config(name, curve_ids=None, flags=0, scratch_bytes=0):
+    cfg = synth.config(name)
+    grid = cfg["grid"]
+    batch = synth.make_batch(cfg, curve_ids)
+    k = cfg["top_k"]
+    g = run_gpu(batch, grid, top_k=k, flags=flags, scratch_bytes=scratch_bytes)
+    assert (g["kmin"], g["kmax"]) == oracle.widths(grid.nb, grid.qmin, grid.qmax)
+    assert (g["status"] == 0).all()
+    freqs = g["freqs"]
+    rep = dict(max_rel_err=0.0, box_near_ties=0, peak_near_ties=0, worst_tie_gap=0.0, n=0)
+    for c in range(batch.n_curves):
+        t, mag, sig = batch.curve(c)
+        r = compare_spectrum(t, mag, sig, freqs, grid.nb, g["kmin"], g["kmax"],
+                             g["sr"][c], g["a"][c], g["k"][c], g["depth"][c], label="%s curve %d" % (name, c))
+        o_sr = r["oracle"][1]
+        pk = g["peaks"][c]
+        pr = compare_peaks(o_sr, pk["freq_index"], pk["sr"], k, label="%s curve %d" % (name, c))
+        # the peak records repeat the spectrum's values at their index
+        for p in pk:
+            if p["freq_index"] >= 0:
+                q = int(p["freq_index"])
+                assert p["sr"] == g["sr"][c][q] and p["depth"] == g["depth"][c][q]
+                assert (p["start_bin"], p["width_bins"]) == (g["a"][c][q], g["k"][c][q])
+                assert p["freq"] == freqs[q]
+                mid = (p["start_bin"] + 0.5 * p["width_bins"]) / grid.nb
+                assert p["epoch"] == pytest.approx(batch.t_origin[c] + mid / freqs[q], abs=1e-6)
+        rep["max_rel_err"] = max(rep["max_rel_err"], r["max_rel_err"])
+        rep["worst_tie_gap"] = max(rep["worst_tie_gap"], r["worst_tie_gap"])
+        rep["box_near_ties"] += r["box_near_ties"]
+        rep["peak_near_ties"] += pr["peak_near_ties"]
+        rep["n"] += len(freqs)
+    print("\n[parity %s] %d (curve,freq) pairs: max SR rel err %.3g, box near-ties %d (worst gap %.3g), "
+          "peak near-ties %d, canonical-rule point-folds %d" % (name, rep["n"], rep["max_rel_err"],
+          rep["box_near_ties"], rep["worst_tie_gap"], rep["peak_near_ties"], g["n_canonical"]))
+    # near-ties must stay rare (exact same-point-set ties resolve canonically on both sides)
+    assert rep["box_near_ties"] <= max(3, 0.01 * rep["n"])
+    return g, rep
+
+
+@pytest.mark.parametrize("name", ["T0", "T1", "T2"])
+def test_small_configs_element_by_element(name):
+    check_config(name)
+
+
+def test_c0_whole():
+    g, rep = check_config("C0")
+    cfg = synth.config("C0")
+    batch = synth.make_batch(cfg)
+    # the injected P = 0.40 d eclipse (f = 2.5 1/d) is the top peak, with positive depth near 0.05
+    top = g["peaks"][0][0]
+    assert abs(top["freq"] - 2.5) < 0.01
+    assert top["depth"] == pytest.approx(0.05, rel=0.25)
+
+
+def test_c1_subset_all_frequencies():
+    """configs[1] shapes (1,500 epochs, 20,000 frequencies, 200 bins, widths 1..30) on 3 curves."""
+    check_config("C1", curve_ids=[0, 7, 500])
+
+
+def test_chunked_scratch_gives_identical_results():
+    cfg = synth.config("T0")
+    batch = synth.make_batch(cfg)
+    g1 = run_gpu(batch, cfg["grid"], top_k=5)
+    g2 = run_gpu(batch, cfg["grid"], top_k=5, scratch_bytes=2 * cfg["grid"].nf * 12)  # 2 curves per chunk
+    for key in ("sr", "a", "k", "depth"):
+        assert np.array_equal(g1[key], g2[key])
+    assert np.array_equal(g1["peaks"], g2["peaks"])
+
+
+def test_canonical_phase_flag_gives_identical_results():
+    import paper_1112_1701_b200 as bls
+    cfg = synth.config("T2")
+    batch = synth.make_batch(cfg)
+    g1 = run_gpu(batch, cfg["grid"], top_k=5)
+    g2 = run_gpu(batch, cfg["grid"], top_k=5, flags=bls.BLS_FLAG_CANONICAL_PHASE)
+    for key in ("sr", "a", "k", "depth"):
+        assert np.array_equal(g1[key], g2[key])
+    assert g2["n_canonical"] >= batch.n_points * cfg["grid"].nf
+    # fast path: only the t = 0 first epoch of each curve (exactly on a bin edge at every
+    # frequency) plus a ~1e-6 fraction of the other point-folds fall in the guard band
+    assert g1["n_canonical"] < batch.n_curves * cfg["grid"].nf + 1e-4 * batch.n_points * cfg["grid"].nf
+
+
+def test_bitwise_reproducible_and_permutation_invariant():
+    """Integer accumulation: the result does not depend on the order of the points."""
+    cfg = synth.config("T1")
+    batch = synth.make_batch(cfg)
+    g1 = run_gpu(batch, cfg["grid"], top_k=4)
+    rng = np.random.default_rng(5)
+    b2 = synth.make_batch(cfg)
+    for c in range(b2.n_curves):
+        a, b = int(b2.offsets[c]), int(b2.offsets[c + 1])
+        perm = a + rng.permutation(b - a)
+        b2.t[a:b], b2.mag[a:b], b2.sigma[a:b] = b2.t[perm], b2.mag[perm], b2.sigma[perm]
+    g2 = run_gpu(b2, cfg["grid"], top_k=4)
+    g3 = run_gpu(batch, cfg["grid"], top_k=4)
+    assert np.array_equal(g1["sr"], g3["sr"]) and np.array_equal(g1["peaks"], g3["peaks"])
+    # the prep sums run in a different order after the permutation -> rounding-level differences only
+    np.testing.assert_allclose(g2["sr"], g1["sr"], rtol=2e-6, atol=0)
+
+
+def test_invariants_at_the_abi():
+    """mag -> mag - 16 (exact in fp32) and sigma -> 2 sigma leave the spectrum unchanged."""
+    rng = np.random.default_rng(21)
+    n = 400
+    t = np.sort(rng.integers(0, 40, n) + rng.uniform(0, 0.3, n)).astype(np.float32)
+    mag = (16.0 + np.round(rng.normal(2.0, 0.05, n) * 1024) / 1024).astype(np.float32)
+    sig = (0.01 * (1 + rng.integers(0, 4, n))).astype(np.float32)
+    grid = synth.Grid(200, 0.2, 4.0, 50, 0.02, 0.12)
+
+    def one(m, s):
+        b = synth.Batch(offsets=np.array([0, n]), t=t, mag=m, sigma=s, t_origin=np.zeros(1), curve_ids=np.zeros(1))
+        return run_gpu(b, grid, top_k=3)
+    g0 = one(mag, sig)
+    g1 = one(mag - np.float32(16.0), sig)
+    g2 = one(mag, sig * np.float32(2))
+    assert (g0["sr"] >= 0).all()
+    np.testing.assert_allclose(g1["sr"], g0["sr"], rtol=2e-6)
+    assert np.array_equal(g2["sr"], g0["sr"]) and np.array_equal(g2["a"], g0["a"]) and np.array_equal(g2["k"], g0["k"])
+    g3 = one(mag * np.float32(2), sig)
+    np.testing.assert_allclose(g3["sr"], 4 * g0["sr"], rtol=2e-6)
+    np.testing.assert_allclose(g3["depth"], 2 * g0["depth"], rtol=2e-6)
+
+
+def test_noiseless_injected_box_is_recovered_exactly():
+    n, nb = 2000, 50
+    t = ((np.arange(n) + 0.5) * 0.01).astype(np.float32)
+    binpos = np.floor((((np.arange(n) + 0.5) / 50.0) % 1.0) * nb).astype(int)
+    inside = (binpos >= 17) & (binpos < 22)
+    mag = np.where(inside, 16.0625, 16.0).astype(np.float32)
+    sig = np.full(n, 0.01, dtype=np.float32)
+    freqs = 1.0 + 0.125 * np.arange(33)
+    grid = synth.Grid(33, 1.0, 5.0, nb, 0.02, 0.16)
+    b = synth.Batch(offsets=np.array([0, n]), t=t, mag=mag, sigma=sig, t_origin=np.zeros(1), curve_ids=np.zeros(1))
+    g = run_gpu(b, grid, top_k=3, freqs=freqs)
+    top = g["peaks"][0][0]
+    assert top["freq"] == 2.0 and (top["start_bin"], top["width_bins"]) == (17, 5)
+    assert top["depth"] == pytest.approx(0.0625, rel=1e-6)
+    assert top["sr"] == pytest.approx(0.1 * 0.9 * 0.0625 ** 2, rel=1e-6)
+
+
+# ------------------------------------------------------------------------------------------------
+# edge cases
+# ------------------------------------------------------------------------------------------------
+def _batch(curves):
+    offs = np.zeros(len(curves) + 1, dtype=np.int64)
+    for i, c in enumerate(curves):
+        offs[i + 1] = offs[i] + len(c[0])
+    cat = lambda j: np.concatenate([np.asarray(c[j], dtype=np.float32) for c in curves]) if curves else np.zeros(0, np.float32)
+    return synth.Batch(offsets=offs, t=cat(0), mag=cat(1), sigma=cat(2), t_origin=np.arange(len(curves), dtype=np.float64),
+                       curve_ids=np.arange(len(curves)))
+
+
+def test_empty_batch():
+    grid = synth.Grid(40, 0.1, 2.0, 20, 0.05, 0.2)
+    g = run_gpu(_batch([]), grid, top_k=2, want_spectrum=False)
+    assert g["peaks"].shape == (0, 2)
+
+
+def test_bad_curves_do_not_sink_the_batch():
+    rng = np.random.default_rng(4)
+    def good(n):
+        t = np.sort(rng.uniform(0, 20, n)); return (t, 15 + rng.normal(0, 0.02, n), np.full(n, 0.02))
+    g0, g1 = good(120), good(77)
+    nanc = good(50); nanc[1][7] = np.nan
+    sig0 = good(50); sig0[2][3] = 0.0
+    one = good(1)
+    empty = (np.zeros(0), np.zeros(0), np.zeros(0))
+    const = (np.sort(rng.uniform(0, 20, 30)), np.full(30, 15.5), np.full(30, 0.01))
+    curves = [g0, nanc, empty, g1, one, sig0, const]
+    grid = synth.Grid(70, 0.1, 3.0, 32, 0.03, 0.2)
+    g = run_gpu(_batch(curves), grid, top_k=3)
+    assert list(g["status"]) == [0, 2, 1, 0, 1, 3, 0]
+    freqs = g["freqs"]
+    for c in (1, 2, 4, 5):
+        assert (g["sr"][c] == 0).all() and (g["depth"][c] == 0).all()
+        assert (g["a"][c] == 0).all() and (g["k"][c] == g["kmin"]).all()
+        assert (g["peaks"][c]["freq_index"] == -1).all()
+    assert (g["sr"][6] == 0).all() and (g["peaks"][6]["freq_index"] == -1).all()    # constant curve
+    for c in (0, 3):
+        t, mag, sig = [np.asarray(x, dtype=np.float32) for x in curves[c]]
+        r = compare_spectrum(t, mag, sig, freqs, grid.nb, g["kmin"], g["kmax"], g["sr"][c], g["a"][c], g["k"][c], g["depth"][c])
+        compare_peaks(r["oracle"][1], g["peaks"][c]["freq_index"], g["peaks"][c]["sr"], 3)
+
+
+def test_kmin_above_one_single_frequency_and_unsorted_negative_times():
+    rng = np.random.default_rng(9)
+    n = 300
+    t = rng.uniform(-10, 10, n)                      # unsorted, negative times allowed (R7, R8)
+    mag = 15 + rng.normal(0, 0.02, n) + 0.08 * (((t / 1.7) % 1.0) < 0.1)
+    sig = rng.uniform(0.01, 0.03, n)
+    b = _batch([(t, mag, sig)])
+    for grid, freqs in [(synth.Grid(1, 0.5882, 0.5882, 60, 0.05, 0.2), None),
+                        (synth.Grid(45, 0.2, 2.0, 37, 0.1, 0.3), None)]:
+        g = run_gpu(b, grid, top_k=2)
+        assert g["kmin"] > 1
+        tt, mm, ss = b.curve(0)
+        r = compare_spectrum(tt, mm, ss, g["freqs"], grid.nb, g["kmin"], g["kmax"], g["sr"][0], g["a"][0], g["k"][0], g["depth"][0])
+        compare_peaks(r["oracle"][1], g["peaks"][0]["freq_index"], g["peaks"][0]["sr"], 2)
+
+
+def test_all_points_in_one_box_is_degenerate_not_infinite():
+    """A single night at low frequency: every point falls in a few bins, boxes reach r = 1."""
+    rng = np.random.default_rng(10)
+    n = 64
+    t = np.sort(rng.uniform(0, 0.2, n))
+    mag = 15 + rng.normal(0, 0.02, n)
+    sig = np.full(n, 0.02)
+    b = _batch([(t, mag, sig)])
+    grid = synth.Grid(33, 0.05, 0.6, 16, 0.1, 0.5)
+    g = run_gpu(b, grid, top_k=2)
+    assert np.isfinite(g["sr"]).all() and np.isfinite(g["depth"]).all()
+    tt, mm, ss = b.curve(0)
+    compare_spectrum(tt, mm, ss, g["freqs"], grid.nb, g["kmin"], g["kmax"], g["sr"][0], g["a"][0], g["k"][0], g["depth"][0])
+
+
+def test_long_curve_read_through_l1():
+    """A curve too long to stage next to the bins in shared memory takes the global-memory path."""
+    rng = np.random.default_rng(13)
+    n = 14000                                           # 14000*16 B + 2*400*128 B > 227 KB
+    t = np.sort(rng.integers(0, 200, n) + rng.uniform(0, 0.3, n))
+    mag = 15 + rng.normal(0, 0.02, n) + 0.05 * ((((t - 0.3) / 2.345) % 1.0) < 0.04)
+    sig = rng.uniform(0.01, 0.03, n)
+    b = _batch([(t, mag, sig)])
+    grid = synth.Grid(40, 0.4, 0.45, 400, 0.01, 0.05)
+    g = run_gpu(b, grid, top_k=2)
+    tt, mm, ss = b.curve(0)
+    compare_spectrum(tt, mm, ss, g["freqs"], grid.nb, g["kmin"], g["kmax"], g["sr"][0], g["a"][0], g["k"][0], g["depth"][0])
+
+
+def test_bin_indices_equal_the_oracles_on_many_pairs():
+    """Reading R8: the fold's bin index equals the oracle's canonical rule bit for bit -- random
+    (f, t) pairs at every configuration's bin count, plus pairs constructed to sit on bin edges."""
+    import torch
+    import paper_1112_1701_b200 as bls
+    rng = np.random.default_rng(2024)
+    total = 0
+    n_canon = 0
+    for nb in (64, 100, 200, 400, 1000):
+        n = 8_000_000
+        f = rng.uniform(1.0 / 30.0, 5.0, n)
+        t = rng.uniform(0.0, 490.0, n).astype(np.float32).astype(np.float64)
+        # a slice of exact edge cases: f*t exactly on a bin edge (dyadic f, t), t = 0, negative t
+        m = 200_000
+        f[:m] = rng.integers(1, 40, m) / 8.0
+        t[:m] = rng.integers(0, 4000 * nb, m) / (8.0 * nb) if nb in (64,) else rng.integers(0, 40000, m) / 64.0
+        t[m:m + 1000] = 0.0
+        t[m + 1000:m + 50000] = -t[m + 1000:m + 50000] / 100.0
+        bins, nc = bls.debug_fold_bins(torch.from_numpy(f).cuda(), torch.from_numpy(t).cuda(), nb)
+        ob = oracle.bins_many(f, t, nb)
+        gb = bins.cpu().numpy()
+        assert np.array_equal(gb, ob), "nb=%d: %d mismatches" % (nb, int((gb != ob).sum()))
+        total += n
+        n_canon += nc
+    print("\n[bins] %d (f,t) pairs, 0 mismatches, %d took the canonical rule" % (total, n_canon))
+    assert n_canon > 0          # the edge cases must have exercised the guard band
