@@ -78,6 +78,9 @@ typedef struct {
 #define BLS_FLAG_CANONICAL_PHASE 1u /* compute every bin index with the slow 3-rounding fp64 rule
                                        (R8) instead of the guarded fast path; results identical   */
 
+#define BLS_FLAG_WARPS(n) (((uint32_t)(n) & 0xffu) << 8) /* tuning: warps per CTA of the search kernel
+                                       (1..16; 0 = the library's choice).  Never changes results. */
+
 /* Ragged CSR batch of light curves (per star a list of HJD times, calibrated
  * magnitudes and errors).  Curve c owns points [offsets[c], offsets[c+1]). */
 typedef struct {
@@ -125,6 +128,8 @@ typedef struct {
                                        (synchronises the stream of that run)                       */
 #define BLS_QUERY_TILE_FREQS 8      /* frequencies per CTA work item in the search kernel          */
 #define BLS_QUERY_SEARCH_CTAS 9     /* CTAs of the last search launch                              */
+#define BLS_QUERY_LAST_SEARCH_NS 10 /* device time (ns, CUDA events on the run's stream) the search
+                                       kernel launches of the last bls_run took (synchronises)    */
 
 /* Validate cfg, copy the grid to the device, derive kmin/kmax and launch geometry.  *out_plan is
  * set only on success. */

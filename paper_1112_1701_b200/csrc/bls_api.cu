@@ -45,6 +45,8 @@ struct bls_plan {
     int64_t last_search_ctas = 0;
     int last_tiles_per_item = 0;
     cudaStream_t last_stream = nullptr;
+    std::vector<cudaEvent_t> ev;    // event pairs bracketing each search launch of the last run
+    size_t ev_used = 0;
     int64_t bytes_owned = 0;
     char cuda_err[256] = {0};
 };
@@ -185,6 +187,7 @@ int bls_plan_destroy(bls_plan *p)
     release(p->d_origin); release(p->d_cand); release(p->d_sr); release(p->d_ak); release(p->d_depth);
     release(p->d_canon); release(p->d_ht); release(p->d_hmag); release(p->d_hsig);
     release(p->d_hpeaks); release(p->d_hstatus);
+    for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
     delete p;
     return BLS_OK;
 }
@@ -201,6 +204,19 @@ int bls_plan_query(const bls_plan *p, int32_t what, int64_t *value)
         case BLS_QUERY_LAST_LAUNCHES: *value = p->last_launches; break;
         case BLS_QUERY_TILE_FREQS: *value = (int64_t)p->last_tiles_per_item * kTileFreqs; break;
         case BLS_QUERY_SEARCH_CTAS: *value = p->last_search_ctas; break;
+        case BLS_QUERY_LAST_SEARCH_NS: {
+            if (p->last_n_curves < 0) return BLS_ERR_ARG;
+            if (cudaSetDevice(p->device) != cudaSuccess) return BLS_ERR_CUDA;
+            double ns = 0.0;
+            for (size_t i = 0; i + 1 < p->ev_used; i += 2) {
+                float ms = 0.f;
+                if (cudaEventSynchronize(p->ev[i + 1]) != cudaSuccess) return BLS_ERR_CUDA;
+                if (cudaEventElapsedTime(&ms, p->ev[i], p->ev[i + 1]) != cudaSuccess) return BLS_ERR_CUDA;
+                ns += (double)ms * 1e6;
+            }
+            *value = (int64_t)ns;
+            break;
+        }
         case BLS_QUERY_LAST_CANONICAL: {
             if (p->last_n_curves < 0) return BLS_ERR_ARG;
             unsigned long long v = 0;
@@ -293,9 +309,12 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
         pts_in_smem = 0;
         smem = search_smem_bytes(p->nb, 0);
     }
+    int warps = (int)((p->flags >> 8) & 0xffu);
+    if (warps < 1 || warps > kMaxSearchWarps) warps = kSearchThreads / 32;
+    const int threads = warps * 32;
     int ctas_per_sm = (int)((size_t)(228 * 1024) / (smem + 1024));
     if (ctas_per_sm < 1) ctas_per_sm = 1;
-    if (ctas_per_sm > 2048 / kSearchThreads) ctas_per_sm = 2048 / kSearchThreads;
+    if (ctas_per_sm > 2048 / threads) ctas_per_sm = 2048 / threads;
     const int64_t target_ctas = (int64_t)p->sm_count * ctas_per_sm * 12;   // >= 12 waves hides the tail
     int64_t items = (target_ctas + chunk - 1) / chunk;
     if (items < 1) items = 1;
@@ -309,6 +328,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     a.nf = (int)p->nf; a.nb = p->nb; a.kmin = p->kmin; a.kmax = p->kmax;
     a.tiles_per_item = tiles_per_item; a.items_per_curve = (int)items;
     a.pts_in_smem = pts_in_smem;
+    a.threads = threads;
     a.force_canonical = (p->flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0;
     a.sr = p->d_sr; a.ak = p->d_ak; a.depth = p->d_depth;
     a.u_sr = out ? out->sr : nullptr;
@@ -319,10 +339,19 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
 
     // ---- per chunk of curves: search -> peak candidates ------------------------------------------
     p->last_search_ctas = 0;
+    p->ev_used = 0;
     for (int64_t base = 0; base < nc; base += chunk) {
         const int64_t cc = (nc - base < chunk) ? nc - base : chunk;
         a.curve_base = base;
+        while (p->ev.size() < p->ev_used + 2) {
+            cudaEvent_t e;
+            BLS_CUDA(p, cudaEventCreate(&e));
+            p->ev.push_back(e);
+        }
+        BLS_CUDA(p, cudaEventRecord(p->ev[p->ev_used], st));
         BLS_CUDA(p, launch_search(a, cc, smem, st));
+        BLS_CUDA(p, cudaEventRecord(p->ev[p->ev_used + 1], st));
+        p->ev_used += 2;
         BLS_CUDA(p, launch_peaks(p->d_sr, p->d_ak, p->d_depth, p->d_meta, base, cc, (int)p->nf,
                                  p->max_top_k, p->d_cand, st));
         p->last_launches += 2;

@@ -35,7 +35,8 @@ struct PeakCand {
 };
 
 constexpr int kTileFreqs = 32;        // frequencies per tile = lanes of a warp
-constexpr int kSearchThreads = 256;   // 8 warps per CTA
+constexpr int kSearchThreads = 256;   // default: 8 warps per CTA
+constexpr int kMaxSearchWarps = 16;   // upper bound (BLS_FLAG_WARPS override)
 constexpr int kPrepThreads = 256;
 constexpr int kPeakThreads = 256;
 constexpr int kStartsPerThread = 4;   // register tile of the box search (A)
@@ -48,6 +49,7 @@ struct SearchArgs {
     int nf, nb, kmin, kmax;
     int tiles_per_item, items_per_curve;
     int64_t curve_base;         // first curve of this chunk
+    int threads;                // CTA size of the search kernel (multiple of 32, <= 32*kMaxSearchWarps)
     int pts_in_smem;            // 1: stage the curve in shared memory, 0: read it through L1
     int force_canonical;        // BLS_FLAG_CANONICAL_PHASE
     float *sr;                  // chunk scratch, [chunk_curves][nf]
@@ -71,14 +73,20 @@ __device__ __noinline__ int canonical_bin(double f, double t, int nb);
 // ph * nb as a 64-bit product = (bin, position inside the bin in units of 2^-32 bin).  If the
 // position is within G = nb + 8 units of a bin edge the canonical rule decides instead; outside
 // the guard band both rules provably give floor(nb frac(f t)) (needs |f t| < 2^18).
-__device__ __forceinline__ int fold_bin(double f, double t, int nb, uint32_t G, bool force_canon,
-                                        unsigned int &n_canon)
+__device__ __forceinline__ int fast_bin(double f, double t, int nb, uint32_t G, uint32_t &lo)
 {
     const double y = fma(f, t, kPhaseMagic);
     const uint32_t ph = (uint32_t)__double2loint(y);
     const unsigned long long pr = (unsigned long long)ph * (uint32_t)nb + (unsigned long long)G;
-    int bin = (int)(pr >> 32);
-    const uint32_t lo = (uint32_t)pr;                  // position * 2^32 + G
+    lo = (uint32_t)pr;                                 // position * 2^32 + G
+    return (int)(pr >> 32);
+}
+
+__device__ __forceinline__ int fold_bin(double f, double t, int nb, uint32_t G, bool force_canon,
+                                        unsigned int &n_canon)
+{
+    uint32_t lo;
+    int bin = fast_bin(f, t, nb, G, lo);
     if (force_canon || lo < 2u * G) {
         bin = canonical_bin(f, t, nb);
         ++n_canon;

@@ -15,20 +15,21 @@
 //     edge fall back to the canonical 3-rounding fp64 rule, so bin indices equal the oracle's
 //     bit for bit (DESIGN.md "Fold / fast phase" has the error bound);
 //   * the box search is register tiled: a thread owns 4 consecutive start bins of its lane's
-//     frequency and slides a 7-bin window, so one shared load feeds 4 boxes; sums are direct
-//     running sums in bin order (no prefix differences), so boxes holding the same point set tie
-//     bitwise and the canonical tie-break (smallest width, then smallest start) applies.
+//     frequency and slides an 8-row window over the bins, so one shared load feeds 4 boxes; sums
+//     are direct running sums in bin order (no prefix differences), so boxes holding the same
+//     point set tie bitwise;
+//   * boxes are ranked by |s| * rsqrt(r(1-r)) (one MUFU.RSQ + one FMUL; monotone in SR); a thread
+//     keeps only the maximum per block of 16 boxes (FMNMX3 tree) and the block's id, re-walks its
+//     winning block once at the end to find the box, and the merge step canonicalises exact ties
+//     (trim empty edge bins -> smallest width, then smallest start: reading R12).
 #include "bls_internal.cuh"
 
 namespace bls {
 
-constexpr int NW = kSearchThreads / 32;
-constexpr int A = kStartsPerThread;
-
 size_t search_smem_bytes(int nb, int64_t n_points_in_smem)
 {
     size_t bins = (size_t)2 * nb * kTileFreqs * 4;
-    size_t red = (size_t)2 * NW * kTileFreqs * 4;
+    size_t red = (size_t)2 * kMaxSearchWarps * kTileFreqs * 4;
     return bins + red + (size_t)n_points_in_smem * sizeof(PointRec);
 }
 
@@ -41,24 +42,41 @@ __device__ __noinline__ int canonical_bin(double f, double t, int nb)
     return b >= nb ? nb - 1 : b;
 }
 
-__device__ __forceinline__ float fast_rcp(float x)
+__device__ __forceinline__ float fast_rsqrt(float x)
 {
     float y;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 
-// Scalar, guarded re-search of one frequency column; only used when the fast search produced a
-// non-finite or impossible value (a box holding the entire weight, r == 1.0f).
-__device__ __noinline__ void careful_search(const float *Wf, const float *Yf, int lane, int nb, int kmin,
-                                            int kmax, float &bv, uint32_t &bkey)
+template <bool SMEM>
+__device__ __forceinline__ PointRec load_point(const PointRec *p)
+{
+    PointRec r;
+    // one 16-byte access at a warp-uniform address: LDS.128 broadcast (or LDG.128 through L1)
+    const uint4 raw = SMEM ? *reinterpret_cast<const uint4 *>(p) : __ldg(reinterpret_cast<const uint4 *>(p));
+    r.t = __hiloint2double((int)raw.y, (int)raw.x); r.qw = raw.z; r.qy = (int32_t)raw.w;
+    return r;
+}
+
+// Bins of one frequency column: row b holds W at col[b*64] and Y at col[b*64 + 32].
+struct Column {
+    const float *col;
+    int nb;
+    __device__ __forceinline__ float W(int b) const { return col[b * 64]; }
+    __device__ __forceinline__ float Y(int b) const { return col[b * 64 + 32]; }
+};
+
+// Scalar, guarded re-search of one frequency column in canonical order; only used when the fast
+// search produced a non-finite or impossible value (a box holding the entire weight, r == 1.0f).
+__device__ __noinline__ void careful_search(Column c, int kmin, int kmax, float &bv, uint32_t &bkey)
 {
     bv = 0.f; bkey = ((uint32_t)kmin << 16);
-    for (int a = 0; a < nb; ++a) {
+    for (int a = 0; a < c.nb; ++a) {
         float r = 0.f, s = 0.f;
         for (int k = 1; k <= kmax; ++k) {
-            int j = a + k - 1; if (j >= nb) j -= nb;
-            r += Wf[j * 32 + lane]; s += Yf[j * 32 + lane];
+            int j = a + k - 1; if (j >= c.nb) j -= c.nb;
+            r += c.W(j); s += c.Y(j);
             if (k < kmin) continue;
             float den = fmaf(-r, r, r);
             if (!(den > 0.f) || !(r < 1.f)) continue;
@@ -69,21 +87,160 @@ __device__ __noinline__ void careful_search(const float *Wf, const float *Yf, in
     }
 }
 
+// Reading R12: among boxes holding the same point set take the smallest width, then the smallest
+// start.  Given any box of that family: drop empty bins at both ends; if that falls below kmin,
+// re-grow to kmin over empty bins, as far left as the numeric start index allows.
+__device__ __forceinline__ void canonicalise(Column c, int kmin, int &a, int &k)
+{
+    const int nb = c.nb;
+    auto empty = [&](int b) { return c.W(b) == 0.f && c.Y(b) == 0.f; };
+    while (k > 1 && empty(a)) { a = a + 1 == nb ? 0 : a + 1; --k; }
+    while (k > 1) { int e = a + k - 1; if (e >= nb) e -= nb; if (!empty(e)) break; --k; }
+    if (k < kmin) {
+        const int need = kmin - k;
+        int L = 0, R = 0;
+        while (L < need) { int b = a - 1 - L; if (b < 0) b += nb; if (!empty(b)) break; ++L; }
+        while (R < need) { int b = a + k + R; if (b >= nb) b -= nb; if (!empty(b)) break; ++R; }
+        const int d_hi = L, d_lo = need - R;          // feasible left shifts: d_lo <= d <= d_hi
+        const int d = (d_lo <= a) ? min(d_hi, a) : d_hi;
+        a -= d; if (a < 0) a += nb;
+        k = kmin;
+    }
+}
+
+template <bool ALIGNED>
+__device__ __forceinline__ void load_group(const float *col, int g, int nb, float *w, float *y)
+{
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        int row = g + i;
+        if (!ALIGNED) row -= (row >= nb) ? nb : 0;
+        w[i] = col[row * 64];
+        y[i] = col[row * 64 + 32];
+    }
+}
+
+// 16 boxes: starts u = 0..3 (rows of the window), widths k0+1 .. k0+4.  Running sums advance by one
+// row per width; returns the largest |s| * rsqrt(r(1-r)).  NaN (empty box: 0 * inf, or r > 1 by
+// rounding: rsqrt of a negative) never wins an FMNMX.
+// The 8-row window is two halves (cur = rows g..g+3, nxt = rows g+4..g+7) so the caller can
+// ping-pong them instead of shifting registers.
+#define WIN(cur, nxt, i) ((i) < 4 ? cur[(i) & 3] : nxt[(i) & 3])
+
+template <bool CHECK>
+__device__ __forceinline__ float block_max(float (&r)[4], float (&s)[4], const float (&wc)[4], const float (&yc)[4],
+                                           const float (&wn)[4], const float (&yn)[4], int k0, int kmin, int kmax)
+{
+    float m = 0.f;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { r[u] += WIN(wc, wn, u + j); s[u] += WIN(yc, yn, u + j); }
+        if (!CHECK || (k0 + j + 1 >= kmin && k0 + j + 1 <= kmax)) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const float den = fmaf(-r[u], r[u], r[u]);       // r (1 - r)
+                const float t = s[u] * fast_rsqrt(den);
+                m = fmaxf(m, fabsf(t));
+            }
+        }
+    }
+    return m;
+}
+
+// Box search of one frequency column by one thread: start tiles tl = first, first+stride, ...
+// Returns the best |t| (t^2 = SR) and its (width << 16 | start) key; ties in any order.
+template <bool ALIGNED>
+__device__ __forceinline__ void search_column(const float *col, int nb, int kmin, int kmax, int first, int stride,
+                                              float &out_t, uint32_t &out_key)
+{
+    const int nst = (nb + 3) >> 2;
+    float best = 0.f;
+    int bcode = -1;
+    for (int tl = first; tl < nst; tl += stride) {
+        int g = tl * 4;
+        float r[4] = {0.f, 0.f, 0.f, 0.f}, s[4] = {0.f, 0.f, 0.f, 0.f}, wa[4], ya[4], wb[4], yb[4];
+        load_group<ALIGNED>(col, g, nb, wa, ya);
+        for (int k0 = 0; k0 < kmax; k0 += 8) {
+            g += 4; if (g >= nb) g -= nb;
+            load_group<ALIGNED>(col, g, nb, wb, yb);
+            {
+                const bool full = (k0 + 1 >= kmin) && (k0 + 4 <= kmax);
+                const float m = full ? block_max<false>(r, s, wa, ya, wb, yb, k0, kmin, kmax)
+                                     : block_max<true>(r, s, wa, ya, wb, yb, k0, kmin, kmax);
+                if (m > best) { best = m; bcode = (tl << 8) | (k0 >> 2); }
+            }
+            if (k0 + 4 < kmax) {
+                g += 4; if (g >= nb) g -= nb;
+                load_group<ALIGNED>(col, g, nb, wa, ya);
+                const int k1 = k0 + 4;
+                const bool full = (k1 + 1 >= kmin) && (k1 + 4 <= kmax);
+                const float m = full ? block_max<false>(r, s, wb, yb, wa, ya, k1, kmin, kmax)
+                                     : block_max<true>(r, s, wb, yb, wa, ya, k1, kmin, kmax);
+                if (m > best) { best = m; bcode = (tl << 8) | (k1 >> 2); }
+            }
+        }
+    }
+    out_t = 0.f;
+    out_key = (uint32_t)kmin << 16;
+    if (bcode < 0) return;
+    // re-walk the winning block to find the box: identical operations, so identical values
+    const int tl = bcode >> 8, k0s = (bcode & 255) << 2;
+    int g = tl * 4;
+    float r[4] = {0.f, 0.f, 0.f, 0.f}, s[4] = {0.f, 0.f, 0.f, 0.f}, w[8], y[8];
+    load_group<ALIGNED>(col, g, nb, w, y);
+    for (int k0 = 0; k0 <= k0s; k0 += 4) {
+        g += 4; if (g >= nb) g -= nb;
+        load_group<ALIGNED>(col, g, nb, w + 4, y + 4);
+        if (k0 < k0s) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { r[u] += w[u + j]; s[u] += y[u + j]; }
+        } else {
+            float bt = 0.f;
+            int bk = kmin, bu = 0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) { r[u] += w[u + j]; s[u] += y[u + j]; }
+                const int k = k0 + j + 1;
+                if (k >= kmin && k <= kmax) {
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const float den = fmaf(-r[u], r[u], r[u]);
+                        const float t = fabsf(s[u] * fast_rsqrt(den));
+                        if (t > bt) { bt = t; bk = k; bu = u; }
+                    }
+                }
+            }
+            int sa = tl * 4 + bu; if (sa >= nb) sa -= nb;
+            out_t = bt;
+            out_key = ((uint32_t)bk << 16) | (uint32_t)sa;
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { w[i] = w[i + 4]; y[i] = y[i + 4]; }
+    }
+}
+
 template <bool PTS_SMEM>
-__global__ void __launch_bounds__(kSearchThreads)
+__global__ void __launch_bounds__(kMaxSearchWarps * 32, 1)
 search_kernel(const SearchArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nb = a.nb;
-    uint32_t *Wb = reinterpret_cast<uint32_t *>(smem_raw);              // [nb][32]
-    int32_t *Yb = reinterpret_cast<int32_t *>(Wb + nb * 32);            // [nb][32]
-    float *red_v = reinterpret_cast<float *>(Yb + nb * 32);             // [NW][32]
-    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + NW * 32);  // [NW][32]
-    PointRec *pts_s = reinterpret_cast<PointRec *>(red_key + NW * 32);  // [n] if PTS_SMEM
+    // bins[bin][0][lane] = W, bins[bin][1][lane] = Y: lane l always hits bank l, and Y sits 128 B
+    // after W so both atomics share one address register
+    uint32_t *Wb = reinterpret_cast<uint32_t *>(smem_raw);                          // [nb][2][32]
+    int32_t *Yb = reinterpret_cast<int32_t *>(Wb + 32);
+    float *red_v = reinterpret_cast<float *>(Wb + nb * 64);                         // [warps][32]
+    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + kMaxSearchWarps * 32); // [warps][32]
+    PointRec *pts_s = reinterpret_cast<PointRec *>(red_key + kMaxSearchWarps * 32); // [n] if PTS_SMEM
     float *Wf = reinterpret_cast<float *>(Wb);
     float *Yf = reinterpret_cast<float *>(Yb);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nthr = blockDim.x, nw = nthr >> 5;
     const int64_t curve_local = blockIdx.x / a.items_per_curve;
     const int item = blockIdx.x % a.items_per_curve;
     const int64_t c = a.curve_base + curve_local;
@@ -96,7 +253,7 @@ search_kernel(const SearchArgs a)
     const int kmin = a.kmin, kmax = a.kmax;
 
     if (meta.status != BLS_CURVE_OK) {   // data fault: zero-filled spectrum (include/bls.h)
-        for (int q = tile0 * kTileFreqs + tid; q < min(tile1 * kTileFreqs, a.nf); q += kSearchThreads) {
+        for (int q = tile0 * kTileFreqs + tid; q < min(tile1 * kTileFreqs, a.nf); q += nthr) {
             a.sr[curve_local * a.nf + q] = 0.f;
             a.ak[curve_local * a.nf + q] = (uint32_t)kmin << 16;
             a.depth[curve_local * a.nf + q] = 0.f;
@@ -113,12 +270,13 @@ search_kernel(const SearchArgs a)
     if (PTS_SMEM) {
         const uint4 *src = reinterpret_cast<const uint4 *>(pts_g);
         uint4 *dst = reinterpret_cast<uint4 *>(pts_s);
-        for (int i = tid; i < n; i += kSearchThreads) dst[i] = __ldg(src + i);
+        for (int i = tid; i < n; i += nthr) dst[i] = __ldg(src + i);
     }
     const PointRec *P = PTS_SMEM ? pts_s : pts_g;
     const bool force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
     const float cw = meta.cw, cy = meta.cy;
     const uint32_t G = (uint32_t)nb + 8u;         // guard band, units of 2^-32 bin
+    const bool aligned = (nb & 3) == 0;
     unsigned int n_canon = 0;
 
     for (int tile = tile0; tile < tile1; ++tile) {
@@ -130,105 +288,92 @@ search_kernel(const SearchArgs a)
         {
             uint4 *z = reinterpret_cast<uint4 *>(Wb);
             const int nvec = nb * 16;              // 2 * nb * 32 words / 4
-            for (int i = tid; i < nvec; i += kSearchThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
+            for (int i = tid; i < nvec; i += nthr) z[i] = make_uint4(0u, 0u, 0u, 0u);
         }
         __syncthreads();
 
-        // ---- a2 Fold: warp w takes points w, w+NW, ...; lane l folds them at its frequency ------
-#pragma unroll 4
-        for (int i = warp; i < n; i += NW) {
-            PointRec p;
-            if (PTS_SMEM) p = P[i];
-            else {
-                uint4 raw = __ldg(reinterpret_cast<const uint4 *>(P + i));
-                p.t = __hiloint2double((int)raw.y, (int)raw.x); p.qw = raw.z; p.qy = (int32_t)raw.w;
+        // ---- a2 Fold: warp w takes points w, w+nw, ...; lane l folds them at its frequency ------
+        {
+            constexpr int U = 4;                   // points in flight per warp: hides LDS/DFMA latency
+            int i = warp;
+            for (; i + (U - 1) * nw < n; i += U * nw) {
+                PointRec p[U];
+                int bin[U];
+                uint32_t lo[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) p[u] = load_point<PTS_SMEM>(P + i + u * nw);
+                bool guard = force_canon;
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    bin[u] = fast_bin(f, p[u].t, nb, G, lo[u]);
+                    guard |= lo[u] < 2u * G;
+                }
+                if (guard) {                       // rare: some lane sits within G of a bin edge
+#pragma unroll
+                    for (int u = 0; u < U; ++u)
+                        if (force_canon || lo[u] < 2u * G) { bin[u] = canonical_bin(f, p[u].t, nb); ++n_canon; }
+                }
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    atomicAdd(&Wb[bin[u] * 64 + lane], p[u].qw);
+                    atomicAdd(&Yb[bin[u] * 64 + lane], p[u].qy);
+                }
             }
-            const int bin = fold_bin(f, p.t, nb, G, force_canon, n_canon);
-            atomicAdd(&Wb[bin * 32 + lane], p.qw);
-            atomicAdd(&Yb[bin * 32 + lane], p.qy);
+            for (; i < n; i += nw) {
+                const PointRec p = load_point<PTS_SMEM>(P + i);
+                const int bin = fold_bin(f, p.t, nb, G, force_canon, n_canon);
+                atomicAdd(&Wb[bin * 64 + lane], p.qw);
+                atomicAdd(&Yb[bin * 64 + lane], p.qy);
+            }
         }
         __syncthreads();
 
         // ---- fixed point -> fp32 weight fraction / weighted residual, in place -------------------
-        for (int i = tid; i < nb * 32; i += kSearchThreads) {
-            Wf[i] = (float)Wb[i] * cw;
-            Yf[i] = (float)Yb[i] * cy;
+        for (int i = tid; i < nb * 32; i += nthr) {
+            const int o = (i >> 5) * 64 + (i & 31);
+            Wf[o] = (float)Wb[o] * cw;
+            Yf[o] = (float)Yb[o] * cy;
         }
         __syncthreads();
 
-        // ---- a3/a4 box search: this thread owns start tiles warp, warp+NW, ... of column `lane` --
-        float tb_v = 0.f;
-        uint32_t tb_key = (uint32_t)kmin << 16;
-        const int nst = (nb + A - 1) / A;
-        for (int tl = warp; tl < nst; tl += NW) {
-            const int a0 = tl * A;
-            float r[A], s[A], ww[2 * A - 1], wy[2 * A - 1];
-#pragma unroll
-            for (int u = 0; u < A; ++u) { r[u] = 0.f; s[u] = 0.f; }
-#pragma unroll
-            for (int i = 0; i < A - 1; ++i) {
-                int j = a0 + i; while (j >= nb) j -= nb;
-                ww[i] = Wf[j * 32 + lane]; wy[i] = Yf[j * 32 + lane];
-            }
-            float lb_v = 0.f;
-            int lb_code = 0;                       // (k << 8) | u of the tile-local best
-            for (int k0 = 0; k0 < kmax; k0 += A) {
-#pragma unroll
-                for (int i = A - 1; i < 2 * A - 1; ++i) {
-                    int j = a0 + k0 + i; while (j >= nb) j -= nb;
-                    ww[i] = Wf[j * 32 + lane]; wy[i] = Yf[j * 32 + lane];
-                }
-#pragma unroll
-                for (int jstep = 0; jstep < A; ++jstep) {
-                    const int k = k0 + jstep + 1;
-#pragma unroll
-                    for (int u = 0; u < A; ++u) { r[u] += ww[u + jstep]; s[u] += wy[u + jstep]; }
-                    if (k >= kmin && k <= kmax) {
-#pragma unroll
-                        for (int u = 0; u < A; ++u) {
-                            const float den = fmaf(-r[u], r[u], r[u]);      // r (1 - r)
-                            const float v = (s[u] * s[u]) * fast_rcp(den);  // NaN (0 * inf) never wins
-                            if (v > lb_v) { lb_v = v; lb_code = (k << 8) | u; }
-                        }
-                    }
-                }
-#pragma unroll
-                for (int i = 0; i < A - 1; ++i) { ww[i] = ww[i + A]; wy[i] = wy[i + A]; }
-            }
-            if (lb_v > 0.f) {
-                int sa = a0 + (lb_code & 0xff); if (sa >= nb) sa -= nb;
-                const uint32_t key = ((uint32_t)(lb_code >> 8) << 16) | (uint32_t)sa;
-                if (lb_v > tb_v || (lb_v == tb_v && key < tb_key)) { tb_v = lb_v; tb_key = key; }
-            }
+        // ---- a3/a4 box search: this thread owns start tiles warp, warp+nw, ... of column `lane` --
+        {
+            float t_best; uint32_t key_best;
+            if (aligned) search_column<true>(Wf + lane, nb, kmin, kmax, warp, nw, t_best, key_best);
+            else search_column<false>(Wf + lane, nb, kmin, kmax, warp, nw, t_best, key_best);
+            red_v[warp * 32 + lane] = t_best;
+            red_key[warp * 32 + lane] = key_best;
         }
-        red_v[warp * 32 + lane] = tb_v;
-        red_key[warp * 32 + lane] = tb_key;
         __syncthreads();
 
-        // ---- merge the NW partial results of each column, recompute (r, s) of the winner ---------
+        // ---- merge the partial results of each column, canonicalise, recompute (r, s) ------------
         if (warp == 0) {
-            float bv = red_v[lane];
+            float bt = red_v[lane];
             uint32_t bkey = red_key[lane];
-#pragma unroll
-            for (int w = 1; w < NW; ++w) {
+            for (int w = 1; w < nw; ++w) {
                 const float v = red_v[w * 32 + lane];
-                const uint32_t key = red_key[w * 32 + lane];
-                if (v > bv || (v == bv && v > 0.f && key < bkey)) { bv = v; bkey = key; }
+                if (v > bt) { bt = v; bkey = red_key[w * 32 + lane]; }
             }
-            if (!(bv <= 1.001f * (float)meta.wx2 + 1e-30f))   // inf / impossible: r == 1.0f box
-                careful_search(Wf, Yf, lane, nb, kmin, kmax, bv, bkey);
-            const int bk = (int)(bkey >> 16), ba = (int)(bkey & 0xffffu);
+            const Column col{Wf + lane, nb};
+            float bv = bt * bt;
+            if (!(bv <= 1.001f * (float)meta.wx2 + 1e-30f)) {   // inf / impossible: r == 1.0f box
+                careful_search(col, kmin, kmax, bv, bkey);
+                bt = bv;
+            }
+            int bk = (int)(bkey >> 16), ba = (int)(bkey & 0xffffu);
+            if (bt > 0.f) canonicalise(col, kmin, ba, bk);
+            else { bk = kmin; ba = 0; }
             float r = 0.f, s = 0.f;
             for (int j = 0; j < bk; ++j) {
                 int b = ba + j; if (b >= nb) b -= nb;
-                r += Wf[b * 32 + lane]; s += Yf[b * 32 + lane];
+                r += col.W(b); s += col.Y(b);
             }
             const float den = fmaf(-r, r, r);
             float sr = 0.f, dp = 0.f;
-            if (bv > 0.f && den > 0.f) { sr = (s * s) / den; dp = s / den; }
+            if (bt > 0.f && den > 0.f) { sr = (s * s) / den; dp = s / den; }
             if (q0 + lane < a.nf) {
                 const int64_t o = curve_local * a.nf + q0 + lane;
-                a.sr[o] = sr; a.ak[o] = bkey; a.depth[o] = dp;
+                a.sr[o] = sr; a.ak[o] = ((uint32_t)bk << 16) | (uint32_t)ba; a.depth[o] = dp;
                 const int64_t uo = c * a.nf + q0 + lane;
                 if (a.u_sr) a.u_sr[uo] = sr;
                 if (a.u_start) a.u_start[uo] = (uint16_t)ba;
@@ -284,9 +429,9 @@ cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem
     if (grid <= 0) return cudaSuccess;
     if (grid > 2147483647LL) return cudaErrorInvalidConfiguration;
     if (a.pts_in_smem)
-        search_kernel<true><<<(unsigned)grid, kSearchThreads, smem, st>>>(a);
+        search_kernel<true><<<(unsigned)grid, a.threads, smem, st>>>(a);
     else
-        search_kernel<false><<<(unsigned)grid, kSearchThreads, smem, st>>>(a);
+        search_kernel<false><<<(unsigned)grid, a.threads, smem, st>>>(a);
     return cudaGetLastError();
 }
 
