@@ -1,0 +1,237 @@
+// Issue-rate microbenchmarks behind the "stated roofline" of the BLS search kernel (DESIGN.md
+// "Roofline").  The fold and box-search stages are bound by per-SM
+// issue rates, not by HBM or tensor throughput, so the denominators of bench.py's roofline are
+// measured here, on the box the bench runs on, in lane-operations per clock per SM:
+//
+//   atoms_add_cf    native 32-bit shared ATOMS.ADD, lane l -> bank l (the fold's access pattern)
+//   atoms_add_rand  same, pseudo-random banks (what a lane = point layout would see)
+//   lds128_bcast    LDS.128 at a warp-uniform address (how the fold reads one point)
+//   lds32_cf        LDS.32, lane l -> bank l (how the box search reads a bin row)
+//   mufu_rsq        MUFU.RSQ (one per box in the search)
+//   fadd / fadd2    FADD vs the packed FADD2 (add.rn.f32x2)
+//   ffma / ffma2    FFMA vs FFMA2
+//   fmnmx3          3-input FMNMX
+//   dfma            fp64 FMA (the fold's phase)
+//   imad_wide       IMAD.WIDE.U32 (phase -> bin)
+//   fold_mix        the fold's per-point-fold instruction mix (LDS.128 bcast amortised over 32 lanes,
+//                   DFMA, IMAD.WIDE, 2 x ATOMS.ADD)
+//   box_mix         the search's per-box mix (2 FADD, FFMA, MUFU.RSQ, FMUL, 1/2 FMNMX3)
+//
+// One CTA of 1024 threads per SM; cycles are clock64() deltas between two __syncthreads(), so the
+// numbers do not depend on the SM clock.  Prints one line per test: median and best over SMs.
+//
+//   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo -o issue_rates issue_rates.cu && ./issue_rates
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+
+#include <algorithm>
+#include <vector>
+
+constexpr int kThreads = 1024;
+constexpr int kIters = 2048;
+
+enum Test { ATOMS_CF, ATOMS_RAND, LDS128_BCAST, LDS32_CF, MUFU_RSQ, FADD, FADD2, FFMA, FFMA2, FMNMX3, DFMA, IMAD_WIDE,
+            FOLD_MIX, BOX_MIX, BOX_MIX2, ATOMS_CF2, LDS64_BCAST, LDS32_BCAST, LDS64_CF, N_TESTS };
+static const char *kNames[N_TESTS] = {"atoms_add_cf", "atoms_add_rand", "lds128_bcast", "lds32_cf", "mufu_rsq", "fadd",
+                                      "fadd2", "ffma", "ffma2", "fmnmx3", "dfma", "imad_wide", "fold_mix", "box_mix",
+                                      "box_mix_fadd2", "atoms_add_cf_min", "lds64_bcast", "lds32_bcast", "lds64_cf"};
+// lane-operations each thread performs per inner iteration (what the rate is quoted in)
+static const double kOpsPerIter[N_TESTS] = {8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 4, 8, 8, 8, 8, 8, 8};
+static const char *kUnit[N_TESTS] = {"ATOMS lane-ops", "ATOMS lane-ops", "LDS.128 lane-loads", "LDS.32 lane-loads",
+                                     "MUFU lane-ops", "FADD lane-ops", "FADD2 lane-instr (2 adds each)", "FFMA lane-ops",
+                                     "FFMA2 lane-instr (2 fmas each)", "FMNMX3 lane-ops (+1/8 FADD)", "DFMA lane-ops",
+                                     "IMAD.WIDE lane-ops", "point-folds", "boxes", "boxes", "ATOMS lane-ops", "LDS.64 lane-loads", "LDS.32 lane-loads", "LDS.64 lane-loads"};
+
+__device__ __forceinline__ float rsq(float x) { float y; asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ unsigned long long add2(unsigned long long a, unsigned long long b)
+{ unsigned long long c; asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(c) : "l"(a), "l"(b)); return c; }
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{ unsigned long long d; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ float fmax3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }
+
+template <int T>
+__global__ void __launch_bounds__(kThreads, 1) bench(long long *cycles, float *sink, int nb)
+{
+    extern __shared__ __align__(16) uint32_t sm[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int i = tid; i < nb * 64 + 4096; i += kThreads) sm[i] = (uint32_t)i * 2654435761u >> 20;
+    __syncthreads();
+    float f0 = 1.0f + tid * 1e-3f, f1 = 1.5f, f2 = 0.25f, f3 = 0.75f, f4 = 1.25f, f5 = 2.f, f6 = 3.f, f7 = 0.5f;
+    unsigned long long p0 = 0x3f8000003f800000ull, p1 = p0 + tid, p2 = p0 + 7, p3 = p0 + 11, p4 = p0, p5 = p1, p6 = p2, p7 = p3;
+    double d0 = 1.0 + tid, d1 = 2.0, d2 = 3.0, d3 = 4.0, d4 = 5.0, d5 = 6.0, d6 = 7.0, d7 = 8.0;
+    const double fr = 0.3712345 + 1e-6 * lane, dc = 1e-3 * (1 + lane);
+    float fc = 1e-3f * (1 + lane);
+    const float fm = 0.999f + 1e-6f * lane;
+    const unsigned long long pc = 0x3a83126f3a83126full + lane, pm = 0x3f7fbe773f7fbe77ull + lane;
+    uint32_t x = tid * 747796405u + 2891336453u;
+    unsigned long long acc = 0;
+    unsigned long long q[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) q[u] = ((unsigned long long)x << 20) + u * 77777ull;
+    uint32_t *pts = sm + nb * 64;            // 4096 words of "points" for the broadcast loads
+    long long t0 = 0, t1 = 0;
+    __syncthreads();
+    t0 = clock64();
+#pragma unroll 1
+    for (int it = 0; it < kIters; ++it) {
+        if (T == ATOMS_CF) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) { x = x * 1664525u + 1013904223u; atomicAdd(&sm[((x >> 8) & 127) * 64 + (u & 1) * 32 + lane], x); }
+        } else if (T == ATOMS_CF2) {
+            uint32_t *b = sm + ((it * 8) & 63) * 64 + lane;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) atomicAdd(b + u * 64 * 9 + (u & 1) * 32, x);
+        } else if (T == LDS64_BCAST) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const uint2 v = *reinterpret_cast<const uint2 *>(pts + (((it * 8 + u) * 37 + warp * 4) & 1023) * 4);
+                acc += v.x ^ v.y;
+            }
+        } else if (T == LDS32_BCAST) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) acc += pts[(((it * 8 + u) * 37 + warp * 4) & 1023) * 4];
+        } else if (T == LDS64_CF) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const uint2 v = *reinterpret_cast<const uint2 *>(sm + (((it * 8 + u) * 5 + warp) & 127) * 64 + lane * 2);
+                acc += v.x ^ v.y;
+            }
+        } else if (T == ATOMS_RAND) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) { x = x * 1664525u + 1013904223u; atomicAdd(&sm[(x >> 8) & 8191], x); }
+        } else if (T == LDS128_BCAST) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const uint4 v = *reinterpret_cast<const uint4 *>(pts + (((it * 8 + u) * 37 + warp * 4) & 1023) * 4);
+                acc += v.x ^ v.y ^ v.z ^ v.w;
+            }
+        } else if (T == LDS32_CF) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) acc += sm[(((it * 8 + u) * 5 + warp) & 127) * 64 + lane];
+        } else if (T == MUFU_RSQ) {
+            f0 = rsq(f0); f1 = rsq(f1); f2 = rsq(f2); f3 = rsq(f3); f4 = rsq(f4); f5 = rsq(f5); f6 = rsq(f6); f7 = rsq(f7);
+        } else if (T == FADD) {
+            f0 += fc; f1 += fc; f2 += fc; f3 += fc; f4 += fc; f5 += fc; f6 += fc; f7 += fc;
+        } else if (T == FADD2) {
+            p0 = add2(p0, pc); p1 = add2(p1, pc); p2 = add2(p2, pc); p3 = add2(p3, pc);
+            p4 = add2(p4, pc); p5 = add2(p5, pc); p6 = add2(p6, pc); p7 = add2(p7, pc);
+        } else if (T == FFMA) {
+            f0 = fmaf(f0, fm, fc); f1 = fmaf(f1, fm, fc); f2 = fmaf(f2, fm, fc); f3 = fmaf(f3, fm, fc);
+            f4 = fmaf(f4, fm, fc); f5 = fmaf(f5, fm, fc); f6 = fmaf(f6, fm, fc); f7 = fmaf(f7, fm, fc);
+        } else if (T == FFMA2) {
+            p0 = fma2(p0, pm, pc); p1 = fma2(p1, pm, pc); p2 = fma2(p2, pm, pc); p3 = fma2(p3, pm, pc);
+            p4 = fma2(p4, pm, pc); p5 = fma2(p5, pm, pc); p6 = fma2(p6, pm, pc); p7 = fma2(p7, pm, pc);
+        } else if (T == FMNMX3) {
+            f0 = fmax3(f0, fc, fm); f1 = fmax3(f1, fm, fc); f2 = fmax3(f2, fc, fm); f3 = fmax3(f3, fm, fc);
+            fc += 1.0f; f4 = fmax3(f4, fc, fm); f5 = fmax3(f5, fm, fc); f6 = fmax3(f6, fc, fm); f7 = fmax3(f7, fm, fc);
+        } else if (T == DFMA) {
+            d0 = fma(d0, fr, dc); d1 = fma(d1, fr, dc); d2 = fma(d2, fr, dc); d3 = fma(d3, fr, dc);
+            d4 = fma(d4, fr, dc); d5 = fma(d5, fr, dc); d6 = fma(d6, fr, dc); d7 = fma(d7, fr, dc);
+        } else if (T == IMAD_WIDE) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) { q[u] = (unsigned long long)(uint32_t)(q[u] >> 32) * (uint32_t)nb + q[u]; }
+        } else if (T == FOLD_MIX) {
+            // 4 points per iteration: LDS.128 broadcast, DFMA with the magic constant, IMAD.WIDE, 2 ATOMS.ADD
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint4 v = *reinterpret_cast<const uint4 *>(pts + (((it * 4 + u) * 8 + warp) & 1023) * 4);
+                const double t = __hiloint2double((int)(v.y & 0xfffffu) | 0x40000000, (int)v.x);
+                const double y = fma(fr, t, 1572864.0);
+                const unsigned long long pr = (unsigned long long)(uint32_t)__double2loint(y) * (uint32_t)nb;
+                const int bin = (int)(pr >> 32);
+                atomicAdd(&sm[bin * 64 + lane], v.z);
+                atomicAdd(&sm[bin * 64 + 32 + lane], v.w + (uint32_t)pr);
+            }
+        } else if (T == BOX_MIX) {
+            // 8 boxes: running sums of (r, s), den = r - r^2, t = |s| * rsqrt(den), max
+            const float w = __uint_as_float(sm[(it % nb) * 64 + lane]) * 1e-12f, y = w * 0.5f;
+            f0 += w; f1 += y; { float t = fabsf(f1) * rsq(fmaf(-f0, f0, f0)); float w2 = f0 + w, y2 = f1 + y;
+            float t2 = fabsf(y2) * rsq(fmaf(-w2, w2, w2)); f7 = fmax3(f7, t, t2); f0 = w2; f1 = y2; }
+            f2 += w; f3 += y; { float t = fabsf(f3) * rsq(fmaf(-f2, f2, f2)); float w2 = f2 + w, y2 = f3 + y;
+            float t2 = fabsf(y2) * rsq(fmaf(-w2, w2, w2)); f7 = fmax3(f7, t, t2); f2 = w2; f3 = y2; }
+            f4 += w; f5 += y; { float t = fabsf(f5) * rsq(fmaf(-f4, f4, f4)); float w2 = f4 + w, y2 = f5 + y;
+            float t2 = fabsf(y2) * rsq(fmaf(-w2, w2, w2)); f6 = fmax3(f6, t, t2); f4 = w2; f5 = y2; }
+            p0 = add2(p0, p1); p0 = add2(p0, p1);   // stand-ins for the 4th start: keeps the mix at 8 boxes
+            { float r = __uint_as_float((uint32_t)p0), s = __uint_as_float((uint32_t)(p0 >> 32));
+              float t = fabsf(s) * rsq(fmaf(-r, r, r)); float t2 = fabsf(s + y) * rsq(fmaf(-(r + w), r + w, r + w)); f6 = fmax3(f6, t, t2); }
+        } else if (T == BOX_MIX2) {
+            // 8 boxes with packed (r, s) running sums: FADD2, FFMA, MUFU, FMUL, 1/2 FMNMX3 per box
+            const unsigned long long wy = ((unsigned long long)sm[(it % nb) * 64 + lane] << 32) | 0x2b8cbccbu;
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                p0 = add2(p0, wy); p1 = add2(p1, wy); p2 = add2(p2, wy); p3 = add2(p3, wy);
+                float r0 = __uint_as_float((uint32_t)p0), s0 = __uint_as_float((uint32_t)(p0 >> 32));
+                float r1 = __uint_as_float((uint32_t)p1), s1 = __uint_as_float((uint32_t)(p1 >> 32));
+                float r2 = __uint_as_float((uint32_t)p2), s2 = __uint_as_float((uint32_t)(p2 >> 32));
+                float r3 = __uint_as_float((uint32_t)p3), s3 = __uint_as_float((uint32_t)(p3 >> 32));
+                float t0 = fabsf(s0) * rsq(fmaf(-r0, r0, r0)), t1 = fabsf(s1) * rsq(fmaf(-r1, r1, r1));
+                float t2 = fabsf(s2) * rsq(fmaf(-r2, r2, r2)), t3 = fabsf(s3) * rsq(fmaf(-r3, r3, r3));
+                f6 = fmax3(f6, t0, t1); f7 = fmax3(f7, t2, t3);
+            }
+        }
+    }
+    __syncthreads();
+    t1 = clock64();
+    if (tid == 0) cycles[blockIdx.x] = t1 - t0;
+    float out = f0 + f1 + f2 + f3 + f4 + f5 + f6 + f7 + (float)(d0 + d1 + d2 + d3 + d4 + d5 + d6 + d7) + (float)acc + (float)x + (float)(q[0] ^ q[1] ^ q[2] ^ q[3] ^ q[4] ^ q[5] ^ q[6] ^ q[7]) +
+                (float)(p0 ^ p1 ^ p2 ^ p3 ^ p4 ^ p5 ^ p6 ^ p7);
+    if (out == 12345.678f) sink[tid] = out + (float)sm[tid];
+}
+
+template <int T>
+void run(int n_sm, int nb, long long *d_cyc, float *d_sink)
+{
+    const size_t smem = (size_t)(nb * 64 + 4096) * 4;
+    cudaFuncSetAttribute(bench<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    std::vector<long long> h(n_sm);
+    double best = 0, med = 0;
+    for (int rep = 0; rep < 3; ++rep) {
+        bench<T><<<n_sm, kThreads, smem>>>(d_cyc, d_sink, nb);
+        cudaError_t e = cudaDeviceSynchronize();
+        if (e != cudaSuccess) { printf("%s: CUDA error %s\n", kNames[T], cudaGetErrorString(e)); exit(1); }
+        cudaMemcpy(h.data(), d_cyc, sizeof(long long) * n_sm, cudaMemcpyDeviceToHost);
+        std::sort(h.begin(), h.end());
+        const double ops = (double)kThreads * kIters * kOpsPerIter[T];
+        med = ops / (double)h[n_sm / 2];
+        best = std::max(best, ops / (double)h[0]);
+    }
+    printf("%-16s %8.2f %8.2f  %s / clk / SM\n", kNames[T], med, best, kUnit[T]);
+}
+
+int main()
+{
+    int n_sm = 0, clk = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, 0) != cudaSuccess) { printf("no CUDA device\n"); return 1; }
+    n_sm = prop.multiProcessorCount;
+    cudaDeviceGetAttribute(&clk, cudaDevAttrClockRate, 0);
+    printf("# %s, %d SMs, max SM clock %d MHz; %d threads/SM, %d iterations; nb = 200 bins x 64 columns\n", prop.name, n_sm,
+           clk / 1000, kThreads, kIters);
+    printf("# %-14s %8s %8s\n", "test", "median", "best");
+    long long *d_cyc; float *d_sink;
+    cudaMalloc(&d_cyc, sizeof(long long) * n_sm);
+    cudaMalloc(&d_sink, sizeof(float) * kThreads);
+    const int nb = 200;
+    run<ATOMS_CF>(n_sm, nb, d_cyc, d_sink);
+    run<ATOMS_RAND>(n_sm, nb, d_cyc, d_sink);
+    run<LDS128_BCAST>(n_sm, nb, d_cyc, d_sink);
+    run<LDS32_CF>(n_sm, nb, d_cyc, d_sink);
+    run<MUFU_RSQ>(n_sm, nb, d_cyc, d_sink);
+    run<FADD>(n_sm, nb, d_cyc, d_sink);
+    run<FADD2>(n_sm, nb, d_cyc, d_sink);
+    run<FFMA>(n_sm, nb, d_cyc, d_sink);
+    run<FFMA2>(n_sm, nb, d_cyc, d_sink);
+    run<FMNMX3>(n_sm, nb, d_cyc, d_sink);
+    run<DFMA>(n_sm, nb, d_cyc, d_sink);
+    run<IMAD_WIDE>(n_sm, nb, d_cyc, d_sink);
+    run<FOLD_MIX>(n_sm, nb, d_cyc, d_sink);
+    run<BOX_MIX>(n_sm, nb, d_cyc, d_sink);
+    run<BOX_MIX2>(n_sm, nb, d_cyc, d_sink);
+    run<ATOMS_CF2>(n_sm, nb, d_cyc, d_sink);
+    run<LDS64_BCAST>(n_sm, nb, d_cyc, d_sink);
+    run<LDS32_BCAST>(n_sm, nb, d_cyc, d_sink);
+    run<LDS64_CF>(n_sm, nb, d_cyc, d_sink);
+    return 0;
+}
