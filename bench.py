@@ -34,17 +34,27 @@ import synth  # noqa: E402
 METRIC = "bls_point_folds_per_sec"
 UNIT = "point-folds/s"
 
-# Roofline constants: measured on B200 with the microbenchmarks summarised in
-# profiles/r01_microbench.md.
-ATOMS_LANE_OPS_PER_CLK_SM = 17.5     # conflict-free shared ATOMS.ADD lane-ops / clk / SM
-BOX_EVALS_PER_CLK_SM = 16.0          # one MUFU.RCP per box, 16 lanes / clk / SM
+# Roofline constants, measured on B200 by paper_1112_1701_b200/microbench/issue_rates.cu
+# (profiles/r01a_microbench.md): lane-operations per clock per SM.
+LSU_LANE_OPS_PER_CLK_SM = 32.0       # shared wavefront pipe: conflict-free ATOMS.ADD 31.96
+XU_LANE_OPS_PER_CLK_SM = 16.0        # MUFU.RSQ 16.00: one per box
+ISSUE_LANE_INSTR_PER_CLK_SM = 128.0  # 4 schedulers x 32 lanes
+FOLD_MIN_INSTR, BOX_MIN_INSTR = 5.0, 4.5
 N_SM = 148
 
 
-def stated_peak_pf_per_s(n_mean, nb, nk, clk_hz, n_sm=N_SM):
-    """Whole-path ceiling: t_min(curve, freq) = 2N/A + nb*nk/E clocks."""
-    t_min = 2.0 * n_mean / ATOMS_LANE_OPS_PER_CLK_SM + nb * nk / BOX_EVALS_PER_CLK_SM
-    return n_sm * clk_hz * n_mean / t_min
+def pair_clocks(n_mean, nb, kmax, nk):
+    """Lower bounds, in SM clocks, for one (curve, frequency) pair on one SM."""
+    t_lsu = (2.0 * n_mean + 2.0 * (nb + kmax)) / LSU_LANE_OPS_PER_CLK_SM
+    t_xu = nb * nk / XU_LANE_OPS_PER_CLK_SM
+    t_issue = (FOLD_MIN_INSTR * n_mean + BOX_MIN_INSTR * nb * nk) / ISSUE_LANE_INSTR_PER_CLK_SM
+    t_sum = 2.0 * n_mean / LSU_LANE_OPS_PER_CLK_SM + nb * nk / XU_LANE_OPS_PER_CLK_SM   # SURVEY 8(d) sum form
+    return {"lsu": t_lsu, "xu": t_xu, "issue": t_issue, "min": max(t_lsu, t_xu, t_issue), "sum_form": t_sum}
+
+
+def stated_peak_pf_per_s(n_mean, nb, kmax, nk, clk_hz, n_sm=N_SM, which="min"):
+    """Whole-path ceiling n_SM * f * N / t_min, t_min = max over pipes."""
+    return n_sm * clk_hz * n_mean / pair_clocks(n_mean, nb, kmax, nk)[which]
 
 
 class ClockSampler:
@@ -147,6 +157,22 @@ def run_reference(args, cfg, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def rank_curve_ids(n_curves_per_rank, rank):
+    """Replicas only: rank r searches curve ids [r*n, (r+1)*n) of the configuration's
+    per-curve addressable generator -- disjoint across ranks, no data-path collective."""
+    return range(rank * n_curves_per_rank, (rank + 1) * n_curves_per_rank)
+
+
+def max_over_ranks(value, dist, device):
+    """Timing rule: the step time of a multi-rank run is the maximum over ranks."""
+    if dist is None:
+        return float(value)
+    import torch
+    tt = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
 def workload_name(name, cfg):
     g = cfg["grid"]
     return "%s: %d curves x %s epochs, %d freqs in [%.4g,%.4g]/d, %d bins, q in [%g,%g], top-%d" % (
@@ -193,7 +219,7 @@ def main():
     # weak scaling: every rank searches its own n_curves curves (curve ids offset by rank)
     grid = cfg["grid"]
     freqs = synth.freq_grid(grid)
-    ids = range(rank * cfg["n_curves"], (rank + 1) * cfg["n_curves"])
+    ids = rank_curve_ids(cfg["n_curves"], rank)
     batch = synth.make_batch(cfg, ids)
     k = cfg["top_k"]
     n_pts, n_curves = batch.n_points, batch.n_curves
@@ -233,10 +259,8 @@ def main():
     wall = time.perf_counter() - wall0
     clocks = sampler.stop()
     t_ms = sum(a.elapsed_time(b) for a, b in ev)
+    t_ms = max_over_ranks(t_ms, dist, dev)
     if dist:
-        tt = torch.tensor([t_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_ms = float(tt.item())
         dist.barrier()
     ms_per_step = t_ms / args.steps
     value = world * pf_per_step / (ms_per_step * 1e-3)
@@ -258,10 +282,7 @@ def main():
         for _ in range(n_e2e):
             hp, hst = plan.search_host(batch.offsets, ht, hm, hs, batch.t_origin, k)
         e2e_s = (time.perf_counter() - t0) / n_e2e
-        if dist:
-            tt = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            e2e_s = float(tt.item())
+        e2e_s = max_over_ranks(e2e_s, dist, dev)
         assert np.array_equal(hp["freq_index"], peaks["freq_index"])
         e2e = {"value": world * pf_per_step / e2e_s, "unit": UNIT,
                "h2d_bytes_per_step": int(3 * 4 * n_pts + 8 * (n_curves + 1) + 8 * n_curves),
@@ -280,8 +301,9 @@ def main():
     search_s = search_ns * 1e-9 / args.steps
     achieved = pf_per_step / search_s
     max_hz = (clocks.get("sm_max_mhz") or 1965) * 1e6
-    peak = stated_peak_pf_per_s(n_mean, grid.nb, nk, max_hz)
-    obs_hz = (clocks.get("sm_mhz") or 0) * 1e6
+    peak = stated_peak_pf_per_s(n_mean, grid.nb, kmax, nk, max_hz)
+    peak_sum = stated_peak_pf_per_s(n_mean, grid.nb, kmax, nk, max_hz, which="sum_form")
+    pc = pair_clocks(n_mean, grid.nb, kmax, nk)
     traffic = None
     tp = os.path.join(ROOT, "profiles", "search_kernel_dram_bytes.json")
     if os.path.exists(tp):
@@ -291,13 +313,18 @@ def main():
             traffic = None
     roofline = {"bound": "alu", "kernel": "search_kernel", "achieved": achieved, "peak": peak,
                 "unit": UNIT, "frac": achieved / peak, "traffic": traffic,
-                "peak_def": "n_SM*f_max*N/(2N/A + nb*nk/E), A=%.1f shared ATOMS.ADD lane-ops/clk/SM, E=%.0f box-evals/clk/SM "
-                            "(measured microbenchmarks, profiles/r01_microbench.md), f_max=%d MHz" % (
-                                ATOMS_LANE_OPS_PER_CLK_SM, BOX_EVALS_PER_CLK_SM, max_hz / 1e6),
-                "frac_at_observed_clock": (achieved / stated_peak_pf_per_s(n_mean, grid.nb, nk, obs_hz)) if obs_hz else None,
-                "fold_stage_peak": N_SM * max_hz * ATOMS_LANE_OPS_PER_CLK_SM / 2.0,
+                "peak_def": "n_SM*f_max*N/t_min per (curve,frequency) pair, t_min = max(LSU (2N+2(nb+kmax))/32, XU nb*nk/16, "
+                            "issue (5N+4.5 nb nk)/128) clk = max(%.0f, %.0f, %.0f); rates measured by microbench/issue_rates.cu "
+                            "(profiles/r01a_microbench.md); f_max=%d MHz, n_SM=%d (DESIGN.md section 7)" % (
+                                pc["lsu"], pc["xu"], pc["issue"], max_hz / 1e6, N_SM),
+                "clk_per_pair": N_SM * max_hz * search_s / (n_curves * grid.nf),
+                "frac_sum_form": achieved / peak_sum,
+                "fold_stage_peak": N_SM * max_hz * LSU_LANE_OPS_PER_CLK_SM / 2.0,
+                "frac_of_fold_stage_peak": achieved / (N_SM * max_hz * LSU_LANE_OPS_PER_CLK_SM / 2.0),
                 "kernel_ms": 1e3 * search_s, "kernel_share_of_step": search_s / (ms_per_step * 1e-3),
-                "box_evals_per_s": n_curves * grid.nf * grid.nb * nk / search_s}
+                "box_evals_per_s": n_curves * grid.nf * grid.nb * nk / search_s,
+                "peak_source": "derived from measured issue rates (no HBM/tensor bound applies); "
+                               "MEASURED_PEAKS.json hbm_gbs is not the bound of this kernel"}
 
     # ---- the oracle beside it (bounded sample; also a parity spot check of the timed result) -----
     cpu = None

@@ -19,7 +19,7 @@
  * Build: gcc -O2 -ffp-contract=off -shared -fPIC (no FMA contraction: the phase rule O4 is a
  * sequence of individually rounded IEEE operations).
  *
- * Pins (tests/test_oracle_pins.py, tests/test_oracle_bins.py, tests/test_oracle_peaks.py):
+ * Pins (tests/test_oracle_pins.py, tests/test_oracle_peaks.py):
  *   oracle_prepare      - weighted-mean identities, weight-scaling invariance          (pinned)
  *   oracle_widths       - table of DESIGN.md reading R9                               (pinned)
  *   oracle_bin          - exact rational arithmetic (fractions.Fraction) + edge cases (pinned)
