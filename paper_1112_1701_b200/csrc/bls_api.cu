@@ -170,7 +170,7 @@ int bls_plan_create(const bls_config *cfg, bls_plan **out_plan)
         return BLS_ERR_CUDA;
     }
     p->bytes_owned = p->nf * (int64_t)sizeof(double) + 8;
-    if (search_smem_bytes(p->nb, 0) > (size_t)p->max_smem_optin) {   // the bins alone must fit
+    if (search_smem_bytes(p->nb, p->kmax, kMaxSearchWarps, 0) > (size_t)p->max_smem_optin) {   // the bins alone must fit
         release(p->d_freqs); release(p->d_canon);
         delete p;
         return BLS_ERR_UNSUPPORTED;
@@ -303,15 +303,15 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
 
     // ---- launch geometry of the search ---------------------------------------------------------
     const int ntiles = (int)((p->nf + kTileFreqs - 1) / kTileFreqs);
-    size_t smem = search_smem_bytes(p->nb, max_n);
+    int warps = (int)((p->flags >> 8) & 0xffu);
+    if (warps < 1 || warps > kMaxSearchWarps) warps = search_default_warps(p->nb);
+    const int threads = warps * 32;
+    size_t smem = search_smem_bytes(p->nb, p->kmax, warps, max_n);
     int pts_in_smem = 1;
     if (smem > (size_t)p->max_smem_optin) {        // curve too long to stage: read it through L1/L2
         pts_in_smem = 0;
-        smem = search_smem_bytes(p->nb, 0);
+        smem = search_smem_bytes(p->nb, p->kmax, warps, 0);
     }
-    int warps = (int)((p->flags >> 8) & 0xffu);
-    if (warps < 1 || warps > kMaxSearchWarps) warps = kSearchThreads / 32;
-    const int threads = warps * 32;
     int ctas_per_sm = (int)((size_t)(228 * 1024) / (smem + 1024));
     if (ctas_per_sm < 1) ctas_per_sm = 1;
     if (ctas_per_sm > 2048 / threads) ctas_per_sm = 2048 / threads;

@@ -36,7 +36,7 @@ struct PeakCand {
 
 constexpr int kTileFreqs = 32;        // frequencies per tile = lanes of a warp
 constexpr int kSearchThreads = 256;   // default: 8 warps per CTA
-constexpr int kMaxSearchWarps = 16;   // upper bound (BLS_FLAG_WARPS override)
+constexpr int kMaxSearchWarps = 10;   // upper bound (BLS_FLAG_WARPS override); 2 CTAs x 10 warps x 96 registers fill an SM
 constexpr int kPrepThreads = 256;
 constexpr int kPeakThreads = 256;
 constexpr int kStartsPerThread = 4;   // register tile of the box search (A)
@@ -95,7 +95,11 @@ __device__ __forceinline__ int fold_bin(double f, double t, int nb, uint32_t G, 
 }
 #endif
 
-size_t search_smem_bytes(int nb, int64_t n_points_in_smem);
+// Bin rows a search CTA holds: the nb bins rounded up to whole start tiles of 4, plus the cyclic
+// extension the widest box of the last start tile reaches (kmax rounded up to whole width blocks).
+__host__ __device__ inline int search_rows(int nb, int kmax) { return ((nb + 3) & ~3) + ((kmax + 3) & ~3); }
+size_t search_smem_bytes(int nb, int kmax, int warps, int64_t n_points_in_smem);
+int search_default_warps(int nb);
 cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int nb, int force_canon,
                               int32_t *bins, unsigned long long *n_canon, cudaStream_t st);
 cudaError_t search_configure(int max_smem_optin);

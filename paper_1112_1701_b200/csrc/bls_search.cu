@@ -26,11 +26,25 @@
 
 namespace bls {
 
-size_t search_smem_bytes(int nb, int64_t n_points_in_smem)
+size_t search_smem_bytes(int nb, int kmax, int warps, int64_t n_points_in_smem)
 {
-    size_t bins = (size_t)2 * nb * kTileFreqs * 4;
-    size_t red = (size_t)2 * kMaxSearchWarps * kTileFreqs * 4;
+    size_t bins = (size_t)search_rows(nb, kmax) * kTileFreqs * 8;
+    size_t red = (size_t)2 * warps * kTileFreqs * 4;
     return bins + red + (size_t)n_points_in_smem * sizeof(PointRec);
+}
+
+// Warps per CTA: the box search splits the ceil(nb/4) start tiles of a column over the warps, so
+// pick the count in [6,10] that wastes the fewest thread-tiles (ties: more warps).
+int search_default_warps(int nb)
+{
+    const int nst = (nb + 3) / 4;
+    int best = 8, best_waste = 1 << 30;
+    for (int w = 6; w <= kMaxSearchWarps; ++w) {
+        const int per = (nst + w - 1) / w;
+        const int waste = (per * w - nst) * 1024 / nst;
+        if (waste <= best_waste) { best_waste = waste; best = w; }
+    }
+    return best;
 }
 
 __device__ __noinline__ int canonical_bin(double f, double t, int nb)
@@ -59,12 +73,12 @@ __device__ __forceinline__ PointRec load_point(const PointRec *p)
     return r;
 }
 
-// Bins of one frequency column: row b holds W at col[b*64] and Y at col[b*64 + 32].
+// Bins of one frequency column after the convert pass: row b holds the pair (W, Y) at col[b*32].
 struct Column {
-    const float *col;
+    const float2 *col;
     int nb;
-    __device__ __forceinline__ float W(int b) const { return col[b * 64]; }
-    __device__ __forceinline__ float Y(int b) const { return col[b * 64 + 32]; }
+    __device__ __forceinline__ float W(int b) const { return col[b * 32].x; }
+    __device__ __forceinline__ float Y(int b) const { return col[b * 32].y; }
 };
 
 // Scalar, guarded re-search of one frequency column in canonical order; only used when the fast
@@ -108,39 +122,58 @@ __device__ __forceinline__ void canonicalise(Column c, int kmin, int &a, int &k)
     }
 }
 
-template <bool ALIGNED>
-__device__ __forceinline__ void load_group(const float *col, int g, int nb, float *w, float *y)
+// ---- packed fp32 pairs -------------------------------------------------------------------------
+// After the fold a bin row holds, per frequency column, the pair (W, Y) as one 64-bit word, so a
+// box's running sums (r, s) advance with ONE packed add (FADD2) fed by ONE LDS.64.
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b)
+{
+    uint64_t c;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(c) : "l"(a), "l"(b));
+    return c;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t pack2(float lo, float hi)
+{
+    uint64_t v;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(lo), "f"(hi));
+    return v;
+}
+
+constexpr int kRowBytes = kTileFreqs * 8;   // one bin row: 32 columns x (W, Y)
+
+// rows g .. g+3 of this thread's column; `p` already points at row g of the column
+__device__ __forceinline__ void load4(const unsigned char *p, uint64_t (&v)[4])
 {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        int row = g + i;
-        if (!ALIGNED) row -= (row >= nb) ? nb : 0;
-        w[i] = col[row * 64];
-        y[i] = col[row * 64 + 32];
-    }
+    for (int i = 0; i < 4; ++i) v[i] = *reinterpret_cast<const uint64_t *>(p + i * kRowBytes);
 }
 
 // 16 boxes: starts u = 0..3 (rows of the window), widths k0+1 .. k0+4.  Running sums advance by one
 // row per width; returns the largest |s| * rsqrt(r(1-r)).  NaN (empty box: 0 * inf, or r > 1 by
-// rounding: rsqrt of a negative) never wins an FMNMX.
+// rounding: rsqrt of a negative, or an invalid start seeded with NaN) never wins an FMNMX.
 // The 8-row window is two halves (cur = rows g..g+3, nxt = rows g+4..g+7) so the caller can
 // ping-pong them instead of shifting registers.
 #define WIN(cur, nxt, i) ((i) < 4 ? cur[(i) & 3] : nxt[(i) & 3])
 
 template <bool CHECK>
-__device__ __forceinline__ float block_max(float (&r)[4], float (&s)[4], const float (&wc)[4], const float (&yc)[4],
-                                           const float (&wn)[4], const float (&yn)[4], int k0, int kmin, int kmax)
+__device__ __forceinline__ float block_max(uint64_t (&rs)[4], const uint64_t (&cur)[4], const uint64_t (&nxt)[4],
+                                           int k0, int kmin, int kmax)
 {
     float m = 0.f;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) { r[u] += WIN(wc, wn, u + j); s[u] += WIN(yc, yn, u + j); }
+        for (int u = 0; u < 4; ++u) rs[u] = add2(rs[u], WIN(cur, nxt, u + j));
         if (!CHECK || (k0 + j + 1 >= kmin && k0 + j + 1 <= kmax)) {
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const float den = fmaf(-r[u], r[u], r[u]);       // r (1 - r)
-                const float t = s[u] * fast_rsqrt(den);
+                float r, s;
+                unpack2(rs[u], r, s);
+                const float den = fmaf(-r, r, r);       // r (1 - r)
+                const float t = s * fast_rsqrt(den);
                 m = fmaxf(m, fabsf(t));
             }
         }
@@ -149,98 +182,117 @@ __device__ __forceinline__ float block_max(float (&r)[4], float (&s)[4], const f
 }
 
 // Box search of one frequency column by one thread: start tiles tl = first, first+stride, ...
-// Returns the best |t| (t^2 = SR) and its (width << 16 | start) key; ties in any order.
-template <bool ALIGNED>
-__device__ __forceinline__ void search_column(const float *col, int nb, int kmin, int kmax, int first, int stride,
-                                              float &out_t, uint32_t &out_key)
+// `col` points at row 0 of the column; rows nb .. are copies of rows 0 .. (cyclic boxes without
+// index arithmetic).  Returns the best |t| (t^2 = SR) and its (width << 16 | start) key; ties in
+// any order.
+__device__ __forceinline__ void search_column(const unsigned char *col, int nb, int kmin, int kmax, int first,
+                                              int stride, float &out_t, uint32_t &out_key)
 {
     const int nst = (nb + 3) >> 2;
+    const int nkb = (kmax + 3) >> 2;
+    const int kb_full_lo = (kmin + 2) >> 2;          // blocks kb in [kb_full_lo, kb_full_hi) need no width check
+    const int kb_full_hi = kmax >> 2;
+    const uint64_t nan2 = pack2(__int_as_float(0x7fc00000), 0.f);
     float best = 0.f;
     int bcode = -1;
     for (int tl = first; tl < nst; tl += stride) {
-        int g = tl * 4;
-        float r[4] = {0.f, 0.f, 0.f, 0.f}, s[4] = {0.f, 0.f, 0.f, 0.f}, wa[4], ya[4], wb[4], yb[4];
-        load_group<ALIGNED>(col, g, nb, wa, ya);
-        for (int k0 = 0; k0 < kmax; k0 += 8) {
-            g += 4; if (g >= nb) g -= nb;
-            load_group<ALIGNED>(col, g, nb, wb, yb);
+        const unsigned char *p = col + tl * (4 * kRowBytes);
+        uint64_t rs[4], wa[4], wb[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) rs[u] = (tl * 4 + u < nb) ? 0ull : nan2;
+        load4(p, wa);
+        for (int kb = 0; kb < nkb; kb += 2) {
+            load4(p + 4 * kRowBytes, wb);
             {
-                const bool full = (k0 + 1 >= kmin) && (k0 + 4 <= kmax);
-                const float m = full ? block_max<false>(r, s, wa, ya, wb, yb, k0, kmin, kmax)
-                                     : block_max<true>(r, s, wa, ya, wb, yb, k0, kmin, kmax);
-                if (m > best) { best = m; bcode = (tl << 8) | (k0 >> 2); }
+                const bool full = kb >= kb_full_lo && kb < kb_full_hi;
+                const float m = full ? block_max<false>(rs, wa, wb, kb * 4, kmin, kmax)
+                                     : block_max<true>(rs, wa, wb, kb * 4, kmin, kmax);
+                if (m > best) { best = m; bcode = (tl << 10) | kb; }
             }
-            if (k0 + 4 < kmax) {
-                g += 4; if (g >= nb) g -= nb;
-                load_group<ALIGNED>(col, g, nb, wa, ya);
-                const int k1 = k0 + 4;
-                const bool full = (k1 + 1 >= kmin) && (k1 + 4 <= kmax);
-                const float m = full ? block_max<false>(r, s, wb, yb, wa, ya, k1, kmin, kmax)
-                                     : block_max<true>(r, s, wb, yb, wa, ya, k1, kmin, kmax);
-                if (m > best) { best = m; bcode = (tl << 8) | (k1 >> 2); }
+            if (kb + 1 < nkb) {
+                load4(p + 8 * kRowBytes, wa);
+                const bool full = kb + 1 >= kb_full_lo && kb + 1 < kb_full_hi;
+                const float m = full ? block_max<false>(rs, wb, wa, kb * 4 + 4, kmin, kmax)
+                                     : block_max<true>(rs, wb, wa, kb * 4 + 4, kmin, kmax);
+                if (m > best) { best = m; bcode = (tl << 10) | (kb + 1); }
             }
+            p += 8 * kRowBytes;
         }
     }
     out_t = 0.f;
     out_key = (uint32_t)kmin << 16;
     if (bcode < 0) return;
     // re-walk the winning block to find the box: identical operations, so identical values
-    const int tl = bcode >> 8, k0s = (bcode & 255) << 2;
-    int g = tl * 4;
-    float r[4] = {0.f, 0.f, 0.f, 0.f}, s[4] = {0.f, 0.f, 0.f, 0.f}, w[8], y[8];
-    load_group<ALIGNED>(col, g, nb, w, y);
-    for (int k0 = 0; k0 <= k0s; k0 += 4) {
-        g += 4; if (g >= nb) g -= nb;
-        load_group<ALIGNED>(col, g, nb, w + 4, y + 4);
-        if (k0 < k0s) {
+    const int tl = bcode >> 10, kbs = bcode & 1023;
+    const unsigned char *p = col + tl * (4 * kRowBytes);
+    uint64_t rs[4], w[8];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) rs[u] = (tl * 4 + u < nb) ? 0ull : nan2;
+    {
+        uint64_t t4[4];
+        load4(p, t4);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) w[i] = t4[i];
+    }
+    for (int kb = 0; kb <= kbs; ++kb) {
+        p += 4 * kRowBytes;
+        {
+            uint64_t t4[4];
+            load4(p, t4);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) w[4 + i] = t4[i];
+        }
+        if (kb < kbs) {
 #pragma unroll
             for (int j = 0; j < 4; ++j)
 #pragma unroll
-                for (int u = 0; u < 4; ++u) { r[u] += w[u + j]; s[u] += y[u + j]; }
+                for (int u = 0; u < 4; ++u) rs[u] = add2(rs[u], w[u + j]);
         } else {
             float bt = 0.f;
             int bk = kmin, bu = 0;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
 #pragma unroll
-                for (int u = 0; u < 4; ++u) { r[u] += w[u + j]; s[u] += y[u + j]; }
-                const int k = k0 + j + 1;
+                for (int u = 0; u < 4; ++u) rs[u] = add2(rs[u], w[u + j]);
+                const int k = kb * 4 + j + 1;
                 if (k >= kmin && k <= kmax) {
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
-                        const float den = fmaf(-r[u], r[u], r[u]);
-                        const float t = fabsf(s[u] * fast_rsqrt(den));
+                        float r, s;
+                        unpack2(rs[u], r, s);
+                        const float den = fmaf(-r, r, r);
+                        const float t = fabsf(s * fast_rsqrt(den));
                         if (t > bt) { bt = t; bk = k; bu = u; }
                     }
                 }
             }
-            int sa = tl * 4 + bu; if (sa >= nb) sa -= nb;
             out_t = bt;
-            out_key = ((uint32_t)bk << 16) | (uint32_t)sa;
+            out_key = ((uint32_t)bk << 16) | (uint32_t)(tl * 4 + bu);
         }
 #pragma unroll
-        for (int i = 0; i < 4; ++i) { w[i] = w[i + 4]; y[i] = y[i + 4]; }
+        for (int i = 0; i < 4; ++i) w[i] = w[i + 4];
     }
 }
 
 template <bool PTS_SMEM>
-__global__ void __launch_bounds__(kMaxSearchWarps * 32, 1)
+__global__ void __launch_bounds__(kMaxSearchWarps * 32, 2)
 search_kernel(const SearchArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int nb = a.nb;
-    // bins[bin][0][lane] = W, bins[bin][1][lane] = Y: lane l always hits bank l, and Y sits 128 B
-    // after W so both atomics share one address register
-    uint32_t *Wb = reinterpret_cast<uint32_t *>(smem_raw);                          // [nb][2][32]
-    int32_t *Yb = reinterpret_cast<int32_t *>(Wb + 32);
-    float *red_v = reinterpret_cast<float *>(Wb + nb * 64);                         // [warps][32]
-    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + kMaxSearchWarps * 32); // [warps][32]
-    PointRec *pts_s = reinterpret_cast<PointRec *>(red_key + kMaxSearchWarps * 32); // [n] if PTS_SMEM
-    float *Wf = reinterpret_cast<float *>(Wb);
-    float *Yf = reinterpret_cast<float *>(Yb);
-
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nthr = blockDim.x, nw = nthr >> 5;
+    const int nrows = search_rows(nb, a.kmax);
+    // During the fold row b holds int32 planes  W[b][lane] | Y[b][lane]  (lane l always hits bank l,
+    // Y sits 128 B after W so both atomics share one address register); the convert pass rewrites
+    // the row in place as fp32 pairs (W, Y)[lane] and fills the cyclic extension rows nb .. nrows-1.
+    uint32_t *Wb = reinterpret_cast<uint32_t *>(smem_raw);                          // [nrows][64]
+    int32_t *Yb = reinterpret_cast<int32_t *>(Wb + 32);
+    float *red_v = reinterpret_cast<float *>(Wb + nrows * 64);                      // [nw][32]
+    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + nw * 32);              // [nw][32]
+    PointRec *pts_s = reinterpret_cast<PointRec *>(red_key + nw * 32);              // [n] if PTS_SMEM
+    const float2 *rows2 = reinterpret_cast<const float2 *>(smem_raw);               // [nrows][32] after convert
+
     const int64_t curve_local = blockIdx.x / a.items_per_curve;
     const int item = blockIdx.x % a.items_per_curve;
     const int64_t c = a.curve_base + curve_local;
@@ -276,7 +328,6 @@ search_kernel(const SearchArgs a)
     const bool force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
     const float cw = meta.cw, cy = meta.cy;
     const uint32_t G = (uint32_t)nb + 8u;         // guard band, units of 2^-32 bin
-    const bool aligned = (nb & 3) == 0;
     unsigned int n_canon = 0;
 
     for (int tile = tile0; tile < tile1; ++tile) {
@@ -328,19 +379,21 @@ search_kernel(const SearchArgs a)
         }
         __syncthreads();
 
-        // ---- fixed point -> fp32 weight fraction / weighted residual, in place -------------------
-        for (int i = tid; i < nb * 32; i += nthr) {
-            const int o = (i >> 5) * 64 + (i & 31);
-            Wf[o] = (float)Wb[o] * cw;
-            Yf[o] = (float)Yb[o] * cy;
+        // ---- fixed point -> fp32 pairs (weight fraction, weighted residual), in place; a warp owns
+        //      whole rows, so reading both planes before writing the pairs needs only a warp sync ----
+        for (int j = warp; j < nb; j += nw) {
+            const uint32_t qw = Wb[j * 64 + lane];
+            const int32_t qy = Yb[j * 64 + lane];
+            __syncwarp();
+            const float2 v = make_float2((float)qw * cw, (float)qy * cy);
+            for (int x = j; x < nrows; x += nb) const_cast<float2 *>(rows2)[x * 32 + lane] = v;
         }
         __syncthreads();
 
         // ---- a3/a4 box search: this thread owns start tiles warp, warp+nw, ... of column `lane` --
         {
             float t_best; uint32_t key_best;
-            if (aligned) search_column<true>(Wf + lane, nb, kmin, kmax, warp, nw, t_best, key_best);
-            else search_column<false>(Wf + lane, nb, kmin, kmax, warp, nw, t_best, key_best);
+            search_column(smem_raw + lane * 8, nb, kmin, kmax, warp, nw, t_best, key_best);
             red_v[warp * 32 + lane] = t_best;
             red_key[warp * 32 + lane] = key_best;
         }
@@ -354,7 +407,7 @@ search_kernel(const SearchArgs a)
                 const float v = red_v[w * 32 + lane];
                 if (v > bt) { bt = v; bkey = red_key[w * 32 + lane]; }
             }
-            const Column col{Wf + lane, nb};
+            const Column col{rows2 + lane, nb};
             float bv = bt * bt;
             if (!(bv <= 1.001f * (float)meta.wx2 + 1e-30f)) {   // inf / impossible: r == 1.0f box
                 careful_search(col, kmin, kmax, bv, bkey);
