@@ -303,8 +303,10 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
 
     // ---- launch geometry of the search ---------------------------------------------------------
     const int ntiles = (int)((p->nf + kTileFreqs - 1) / kTileFreqs);
-    int warps = (int)((p->flags >> 8) & 0xffu);
-    if (warps < 1 || warps > kMaxSearchWarps) warps = search_default_warps(p->nb);
+    int starts = 4, warps = 8;
+    search_geometry(p->nb, &starts, &warps);
+    const int warps_flag = (int)((p->flags >> 8) & 0xffu);
+    if (warps_flag >= 1 && warps_flag <= kMaxSearchWarps) warps = warps_flag;
     const int threads = warps * 32;
     size_t smem = search_smem_bytes(p->nb, p->kmax, warps, max_n);
     int pts_in_smem = 1;
@@ -328,6 +330,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     a.nf = (int)p->nf; a.nb = p->nb; a.kmin = p->kmin; a.kmax = p->kmax;
     a.tiles_per_item = tiles_per_item; a.items_per_curve = (int)items;
     a.pts_in_smem = pts_in_smem;
+    a.starts_per_thread = starts;
     a.threads = threads;
     a.force_canonical = (p->flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0;
     a.sr = p->d_sr; a.ak = p->d_ak; a.depth = p->d_depth;

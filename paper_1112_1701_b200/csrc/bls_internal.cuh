@@ -51,6 +51,7 @@ struct SearchArgs {
     int64_t curve_base;         // first curve of this chunk
     int threads;                // CTA size of the search kernel (multiple of 32, <= 32*kMaxSearchWarps)
     int pts_in_smem;            // 1: stage the curve in shared memory, 0: read it through L1
+    int starts_per_thread;      // S of the box search (4 or 5)
     int force_canonical;        // BLS_FLAG_CANONICAL_PHASE
     float *sr;                  // chunk scratch, [chunk_curves][nf]
     uint32_t *ak;
@@ -82,6 +83,14 @@ __device__ __forceinline__ int fast_bin(double f, double t, int nb, uint32_t G, 
     return (int)(pr >> 32);
 }
 
+// Same, returning the whole product: high word = bin, low word = position * 2^32 + G.
+__device__ __forceinline__ unsigned long long fast_bin_pos(double f, double t, int nb, uint32_t G)
+{
+    const double y = fma(f, t, kPhaseMagic);
+    const uint32_t ph = (uint32_t)__double2loint(y);
+    return (unsigned long long)ph * (uint32_t)nb + (unsigned long long)G;
+}
+
 __device__ __forceinline__ int fold_bin(double f, double t, int nb, uint32_t G, bool force_canon,
                                         unsigned int &n_canon)
 {
@@ -95,11 +104,11 @@ __device__ __forceinline__ int fold_bin(double f, double t, int nb, uint32_t G, 
 }
 #endif
 
-// Bin rows a search CTA holds: the nb bins rounded up to whole start tiles of 4, plus the cyclic
-// extension the widest box of the last start tile reaches (kmax rounded up to whole width blocks).
-__host__ __device__ inline int search_rows(int nb, int kmax) { return ((nb + 3) & ~3) + ((kmax + 3) & ~3); }
+// Bin rows a search CTA holds: the nb bins plus the cyclic extension the widest box of the last
+// start tile reaches (kmax rounded up to whole width blocks, plus the window's slack).
+__host__ __device__ inline int search_rows(int nb, int kmax) { return nb + ((kmax + 3) & ~3) + 4; }
 size_t search_smem_bytes(int nb, int kmax, int warps, int64_t n_points_in_smem);
-int search_default_warps(int nb);
+void search_geometry(int nb, int *starts_per_thread, int *warps);
 cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int nb, int force_canon,
                               int32_t *bins, unsigned long long *n_canon, cudaStream_t st);
 cudaError_t search_configure(int max_smem_optin);

@@ -33,18 +33,25 @@ size_t search_smem_bytes(int nb, int kmax, int warps, int64_t n_points_in_smem)
     return bins + red + (size_t)n_points_in_smem * sizeof(PointRec);
 }
 
-// Warps per CTA: the box search splits the ceil(nb/4) start tiles of a column over the warps, so
-// pick the count in [6,10] that wastes the fewest thread-tiles (ties: more warps).
-int search_default_warps(int nb)
+// Geometry of the box search: a thread owns S consecutive start bins (S = 4 or 5), the
+// ceil(nb/S) start tiles of a column are dealt to the warps.  Pick (S, warps in [6,10]) that wastes
+// the fewest thread-tiles; ties go to S = 5 (fewer loads per box), then to more warps.
+void search_geometry(int nb, int *starts_per_thread, int *warps)
 {
-    const int nst = (nb + 3) / 4;
-    int best = 8, best_waste = 1 << 30;
-    for (int w = 6; w <= kMaxSearchWarps; ++w) {
-        const int per = (nst + w - 1) / w;
-        const int waste = (per * w - nst) * 1024 / nst;
-        if (waste <= best_waste) { best_waste = waste; best = w; }
+    int best_s = 4, best_w = 8;
+    double best_cost = 1e30;
+    for (int s = 4; s <= 5; ++s) {
+        const int nst = (nb + s - 1) / s;
+        for (int w = 6; w <= kMaxSearchWarps; ++w) {
+            const int per = (nst + w - 1) / w;
+            const double cost = (double)per * w * s / nb;      // thread-starts issued per useful start
+            if (cost < best_cost - 1e-9 || (cost < best_cost + 1e-9 && (s > best_s || (s == best_s && w > best_w)))) {
+                best_cost = cost; best_s = s; best_w = w;
+            }
+        }
     }
-    return best;
+    *starts_per_thread = best_s;
+    *warps = best_w;
 }
 
 __device__ __noinline__ int canonical_bin(double f, double t, int nb)
@@ -144,11 +151,51 @@ __device__ __forceinline__ uint64_t pack2(float lo, float hi)
 
 constexpr int kRowBytes = kTileFreqs * 8;   // one bin row: 32 columns x (W, Y)
 
-// rows g .. g+3 of this thread's column; `p` already points at row g of the column
-__device__ __forceinline__ void load4(const unsigned char *p, uint64_t (&v)[4])
+// Shared memory is addressed by 32-bit shared-window addresses with immediate offsets in the hot
+// loops (one address register per stream, no generic-pointer arithmetic).
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint64_t lds64(uint32_t addr)
+{
+    uint64_t v;
+    asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts64(uint32_t addr, uint64_t v)
+{
+    asm volatile("st.shared.b64 [%0], %1;" ::"r"(addr), "l"(v) : "memory");
+}
+__device__ __forceinline__ void red_add(uint32_t addr, uint32_t v)      // ATOMS.ADD, no return value
+{
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+
+// base + row * kRowBytes as ONE instruction (kept opaque so the compiler does not fold it into a
+// 64-bit shift of the IMAD.WIDE result it comes from)
+__device__ __forceinline__ uint32_t row_addr(uint32_t base, uint32_t row)
+{
+    uint32_t a;
+    asm volatile("mad.lo.u32 %0, %1, 256, %2;" : "=r"(a) : "r"(row), "r"(base));
+    return a;
+}
+static_assert(kRowBytes == 256, "row_addr hard-codes the row pitch");
+
+// rows g .. g+3 of this thread's column; `p` is the shared address of row g of the column
+__device__ __forceinline__ void load4(uint32_t p, uint64_t (&v)[4])
 {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) v[i] = *reinterpret_cast<const uint64_t *>(p + i * kRowBytes);
+    for (int i = 0; i < 4; ++i) v[i] = lds64(p + i * kRowBytes);
 }
 
 // 16 boxes: starts u = 0..3 (rows of the window), widths k0+1 .. k0+4.  Running sums advance by one
@@ -158,18 +205,18 @@ __device__ __forceinline__ void load4(const unsigned char *p, uint64_t (&v)[4])
 // ping-pong them instead of shifting registers.
 #define WIN(cur, nxt, i) ((i) < 4 ? cur[(i) & 3] : nxt[(i) & 3])
 
-template <bool CHECK>
-__device__ __forceinline__ float block_max(uint64_t (&rs)[4], const uint64_t (&cur)[4], const uint64_t (&nxt)[4],
+template <int S, bool CHECK>
+__device__ __forceinline__ float block_max(uint64_t (&rs)[S], const uint64_t (&cur)[4], const uint64_t (&nxt)[4],
                                            int k0, int kmin, int kmax)
 {
     float m = 0.f;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) rs[u] = add2(rs[u], WIN(cur, nxt, u + j));
+        for (int u = 0; u < S; ++u) rs[u] = add2(rs[u], WIN(cur, nxt, u + j));
         if (!CHECK || (k0 + j + 1 >= kmin && k0 + j + 1 <= kmax)) {
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
+            for (int u = 0; u < S; ++u) {
                 float r, s;
                 unpack2(rs[u], r, s);
                 const float den = fmaf(-r, r, r);       // r (1 - r)
@@ -181,14 +228,17 @@ __device__ __forceinline__ float block_max(uint64_t (&rs)[4], const uint64_t (&c
     return m;
 }
 
-// Box search of one frequency column by one thread: start tiles tl = first, first+stride, ...
-// `col` points at row 0 of the column; rows nb .. are copies of rows 0 .. (cyclic boxes without
-// index arithmetic).  Returns the best |t| (t^2 = SR) and its (width << 16 | start) key; ties in
-// any order.
-__device__ __forceinline__ void search_column(const unsigned char *col, int nb, int kmin, int kmax, int first,
-                                              int stride, float &out_t, uint32_t &out_key)
+// Box search of one frequency column by one thread: start tiles tl = first, first+stride, ... of
+// S consecutive start bins each (S = 4 or 5: S + 3 rows fit the 8-row window).
+// `col` is the shared address of row 0 of the column; rows nb .. are copies of rows 0 .. (cyclic
+// boxes without index arithmetic).  Returns the best |t| (t^2 = SR) and its (width << 16 | start)
+// key; ties in any order.
+template <int S>
+__device__ __forceinline__ void search_column(uint32_t col, int nb, int kmin, int kmax, int first, int stride,
+                                              float &out_t, uint32_t &out_key)
 {
-    const int nst = (nb + 3) >> 2;
+    static_assert(S == 4 || S == 5, "the 8-row window holds S + 3 rows");
+    const int nst = (nb + S - 1) / S;
     const int nkb = (kmax + 3) >> 2;
     const int kb_full_lo = (kmin + 2) >> 2;          // blocks kb in [kb_full_lo, kb_full_hi) need no width check
     const int kb_full_hi = kmax >> 2;
@@ -196,85 +246,96 @@ __device__ __forceinline__ void search_column(const unsigned char *col, int nb, 
     float best = 0.f;
     int bcode = -1;
     for (int tl = first; tl < nst; tl += stride) {
-        const unsigned char *p = col + tl * (4 * kRowBytes);
-        uint64_t rs[4], wa[4], wb[4];
+        uint32_t p = col + tl * (S * kRowBytes);
+        const int tcode = tl << 10;
+        uint64_t rs[S], wa[4], wb[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) rs[u] = (tl * 4 + u < nb) ? 0ull : nan2;
+        for (int u = 0; u < S; ++u) rs[u] = (tl * S + u < nb) ? 0ull : nan2;
         load4(p, wa);
-        for (int kb = 0; kb < nkb; kb += 2) {
+        int kb = 0;
+        // head blocks below kmin (only when kmin > 4), one at a time, window shifted through registers
+        for (; kb < kb_full_lo && kb < nkb; ++kb) {
+            p += 4 * kRowBytes;
+            load4(p, wb);
+            const float m = block_max<S, true>(rs, wa, wb, kb * 4, kmin, kmax);
+            if (m > best) { best = m; bcode = tcode | kb; }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) wa[i] = wb[i];
+        }
+        // two full blocks per iteration, the window halves ping-pong
+        for (; kb + 2 <= kb_full_hi; kb += 2) {
             load4(p + 4 * kRowBytes, wb);
-            {
-                const bool full = kb >= kb_full_lo && kb < kb_full_hi;
-                const float m = full ? block_max<false>(rs, wa, wb, kb * 4, kmin, kmax)
-                                     : block_max<true>(rs, wa, wb, kb * 4, kmin, kmax);
-                if (m > best) { best = m; bcode = (tl << 10) | kb; }
-            }
-            if (kb + 1 < nkb) {
-                load4(p + 8 * kRowBytes, wa);
-                const bool full = kb + 1 >= kb_full_lo && kb + 1 < kb_full_hi;
-                const float m = full ? block_max<false>(rs, wb, wa, kb * 4 + 4, kmin, kmax)
-                                     : block_max<true>(rs, wb, wa, kb * 4 + 4, kmin, kmax);
-                if (m > best) { best = m; bcode = (tl << 10) | (kb + 1); }
-            }
+            float m = block_max<S, false>(rs, wa, wb, 0, 0, 0);
+            if (m > best) { best = m; bcode = tcode | kb; }
+            load4(p + 8 * kRowBytes, wa);
+            m = block_max<S, false>(rs, wb, wa, 0, 0, 0);
+            if (m > best) { best = m; bcode = tcode | (kb + 1); }
             p += 8 * kRowBytes;
+        }
+        // tail: at most one full block and the block that holds kmax
+        if (kb + 2 <= nkb) {
+            load4(p + 4 * kRowBytes, wb);
+            float m = block_max<S, true>(rs, wa, wb, kb * 4, kmin, kmax);
+            if (m > best) { best = m; bcode = tcode | kb; }
+            load4(p + 8 * kRowBytes, wa);
+            m = block_max<S, true>(rs, wb, wa, kb * 4 + 4, kmin, kmax);
+            if (m > best) { best = m; bcode = tcode | (kb + 1); }
+        } else if (kb < nkb) {
+            load4(p + 4 * kRowBytes, wb);
+            const float m = block_max<S, true>(rs, wa, wb, kb * 4, kmin, kmax);
+            if (m > best) { best = m; bcode = tcode | kb; }
         }
     }
     out_t = 0.f;
     out_key = (uint32_t)kmin << 16;
     if (bcode < 0) return;
-    // re-walk the winning block to find the box: identical operations, so identical values
+    // Re-walk to the winning block: first only the running sums (lanes differ in how far they
+    // go, so this loop holds nothing else), then that block's boxes once, with the argmax.
+    // Identical operations in identical order, so identical values.
     const int tl = bcode >> 10, kbs = bcode & 1023;
-    const unsigned char *p = col + tl * (4 * kRowBytes);
-    uint64_t rs[4], w[8];
+    uint32_t p = col + tl * (S * kRowBytes);
+    uint64_t rs[S], w[8];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) rs[u] = (tl * 4 + u < nb) ? 0ull : nan2;
-    {
-        uint64_t t4[4];
-        load4(p, t4);
+    for (int u = 0; u < S; ++u) rs[u] = (tl * S + u < nb) ? 0ull : nan2;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) w[i] = t4[i];
-    }
-    for (int kb = 0; kb <= kbs; ++kb) {
+    for (int i = 0; i < 4; ++i) w[i] = lds64(p + i * kRowBytes);
+    for (int kb = 0; kb < kbs; ++kb) {
         p += 4 * kRowBytes;
-        {
-            uint64_t t4[4];
-            load4(p, t4);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) w[4 + i] = t4[i];
-        }
-        if (kb < kbs) {
+        for (int i = 0; i < 4; ++i) w[4 + i] = lds64(p + i * kRowBytes);
 #pragma unroll
-            for (int j = 0; j < 4; ++j)
+        for (int j = 0; j < 4; ++j)
 #pragma unroll
-                for (int u = 0; u < 4; ++u) rs[u] = add2(rs[u], w[u + j]);
-        } else {
-            float bt = 0.f;
-            int bk = kmin, bu = 0;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-#pragma unroll
-                for (int u = 0; u < 4; ++u) rs[u] = add2(rs[u], w[u + j]);
-                const int k = kb * 4 + j + 1;
-                if (k >= kmin && k <= kmax) {
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        float r, s;
-                        unpack2(rs[u], r, s);
-                        const float den = fmaf(-r, r, r);
-                        const float t = fabsf(s * fast_rsqrt(den));
-                        if (t > bt) { bt = t; bk = k; bu = u; }
-                    }
-                }
-            }
-            out_t = bt;
-            out_key = ((uint32_t)bk << 16) | (uint32_t)(tl * 4 + bu);
-        }
+            for (int u = 0; u < S; ++u) rs[u] = add2(rs[u], w[u + j]);
 #pragma unroll
         for (int i = 0; i < 4; ++i) w[i] = w[i + 4];
     }
+    p += 4 * kRowBytes;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) w[4 + i] = lds64(p + i * kRowBytes);
+    float bt = 0.f;
+    int bk = kmin, bu = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+#pragma unroll
+        for (int u = 0; u < S; ++u) rs[u] = add2(rs[u], w[u + j]);
+        const int k = kbs * 4 + j + 1;
+        if (k >= kmin && k <= kmax) {
+#pragma unroll
+            for (int u = 0; u < S; ++u) {
+                float r, s;
+                unpack2(rs[u], r, s);
+                const float den = fmaf(-r, r, r);
+                const float t = fabsf(s * fast_rsqrt(den));
+                if (t > bt) { bt = t; bk = k; bu = u; }
+            }
+        }
+    }
+    out_t = bt;
+    out_key = ((uint32_t)bk << 16) | (uint32_t)(tl * S + bu);
 }
 
-template <bool PTS_SMEM>
+template <bool PTS_SMEM, int S>
 __global__ void __launch_bounds__(kMaxSearchWarps * 32, 2)
 search_kernel(const SearchArgs a)
 {
@@ -325,10 +386,12 @@ search_kernel(const SearchArgs a)
         for (int i = tid; i < n; i += nthr) dst[i] = __ldg(src + i);
     }
     const PointRec *P = PTS_SMEM ? pts_s : pts_g;
+    const uint32_t bins_s = smem_u32(smem_raw), pts_sa = smem_u32(pts_s);
     const bool force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
     const float cw = meta.cw, cy = meta.cy;
     const uint32_t G = (uint32_t)nb + 8u;         // guard band, units of 2^-32 bin
     unsigned int n_canon = 0;
+    const int tail_warp = (n >> 2) % nw;
 
     for (int tile = tile0; tile < tile1; ++tile) {
         const int q0 = tile * kTileFreqs;
@@ -343,64 +406,104 @@ search_kernel(const SearchArgs a)
         }
         __syncthreads();
 
-        // ---- a2 Fold: warp w takes points w, w+nw, ...; lane l folds them at its frequency ------
+        // ---- a2 Fold: warp w takes groups of 4 consecutive points w, w+nw, ...; lane l folds them
+        //      at its frequency.  Four points in flight hide the LDS / DFMA latency. --------------
         {
-            constexpr int U = 4;                   // points in flight per warp: hides LDS/DFMA latency
-            int i = warp;
-            for (; i + (U - 1) * nw < n; i += U * nw) {
-                PointRec p[U];
-                int bin[U];
-                uint32_t lo[U];
+            const uint32_t colw = bins_s + lane * 4;       // W plane of this lane's column, row 0
+            const int ngroups = n >> 2;
+            if (PTS_SMEM) {
+                const uint32_t pa_end = pts_sa + ngroups * 64;
+                for (uint32_t pa = pts_sa + warp * 64; pa < pa_end; pa += nw * 64) {
+                    uint4 raw[4];
+                    unsigned long long pr[4];
 #pragma unroll
-                for (int u = 0; u < U; ++u) p[u] = load_point<PTS_SMEM>(P + i + u * nw);
-                bool guard = force_canon;
+                    for (int u = 0; u < 4; ++u) raw[u] = lds128(pa + u * 16);
 #pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    bin[u] = fast_bin(f, p[u].t, nb, G, lo[u]);
-                    guard |= lo[u] < 2u * G;
+                    for (int u = 0; u < 4; ++u)
+                        pr[u] = fast_bin_pos(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb, G);
+                    const uint32_t lomin = min(min((uint32_t)pr[0], (uint32_t)pr[1]), min((uint32_t)pr[2], (uint32_t)pr[3]));
+                    if (!force_canon && lomin >= 2u * G) {
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            const uint32_t addr = row_addr(colw, (uint32_t)(pr[u] >> 32));
+                            red_add(addr, raw[u].z);
+                            red_add(addr + 128, raw[u].w);
+                        }
+                    } else {                       // rare: some point sits within G of a bin edge
+#pragma unroll
+                        for (int u = 0; u < 4; ++u) {
+                            int bin = (int)(pr[u] >> 32);
+                            if (force_canon || (uint32_t)pr[u] < 2u * G) {
+                                bin = canonical_bin(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb);
+                                ++n_canon;
+                            }
+                            const uint32_t addr = colw + bin * kRowBytes;
+                            red_add(addr, raw[u].z);
+                            red_add(addr + 128, raw[u].w);
+                        }
+                    }
                 }
-                if (guard) {                       // rare: some lane sits within G of a bin edge
+            } else {
+                for (int g = warp; g < ngroups; g += nw) {
+                    PointRec p[4];
+                    int bin[4];
+                    uint32_t lo[4];
 #pragma unroll
-                    for (int u = 0; u < U; ++u)
-                        if (force_canon || lo[u] < 2u * G) { bin[u] = canonical_bin(f, p[u].t, nb); ++n_canon; }
-                }
+                    for (int u = 0; u < 4; ++u) p[u] = load_point<false>(pts_g + g * 4 + u);
 #pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    atomicAdd(&Wb[bin[u] * 64 + lane], p[u].qw);
-                    atomicAdd(&Yb[bin[u] * 64 + lane], p[u].qy);
+                    for (int u = 0; u < 4; ++u) bin[u] = fast_bin(f, p[u].t, nb, G, lo[u]);
+                    if (force_canon || min(min(lo[0], lo[1]), min(lo[2], lo[3])) < 2u * G) {
+#pragma unroll
+                        for (int u = 0; u < 4; ++u)
+                            if (force_canon || lo[u] < 2u * G) { bin[u] = canonical_bin(f, p[u].t, nb); ++n_canon; }
+                    }
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const uint32_t addr = colw + bin[u] * kRowBytes;
+                        red_add(addr, p[u].qw);
+                        red_add(addr + 128, (uint32_t)p[u].qy);
+                    }
                 }
             }
-            for (; i < n; i += nw) {
-                const PointRec p = load_point<PTS_SMEM>(P + i);
-                const int bin = fold_bin(f, p.t, nb, G, force_canon, n_canon);
-                atomicAdd(&Wb[bin * 64 + lane], p.qw);
-                atomicAdd(&Yb[bin * 64 + lane], p.qy);
+            if (warp == tail_warp) {               // the n % 4 points after the last whole group
+                for (int i = ngroups * 4; i < n; ++i) {
+                    const PointRec p = load_point<PTS_SMEM>(P + i);
+                    const int bin = fold_bin(f, p.t, nb, G, force_canon, n_canon);
+                    const uint32_t addr = colw + bin * kRowBytes;
+                    red_add(addr, p.qw);
+                    red_add(addr + 128, (uint32_t)p.qy);
+                }
             }
         }
         __syncthreads();
 
         // ---- fixed point -> fp32 pairs (weight fraction, weighted residual), in place; a warp owns
         //      whole rows, so reading both planes before writing the pairs needs only a warp sync ----
-        for (int j = warp; j < nb; j += nw) {
-            const uint32_t qw = Wb[j * 64 + lane];
-            const int32_t qy = Yb[j * 64 + lane];
-            __syncwarp();
-            const float2 v = make_float2((float)qw * cw, (float)qy * cy);
-            for (int x = j; x < nrows; x += nb) const_cast<float2 *>(rows2)[x * 32 + lane] = v;
+        {
+            uint32_t ra = bins_s + warp * kRowBytes + lane * 4;
+            for (int j = warp; j < nb; j += nw, ra += nw * kRowBytes) {
+                const uint32_t qw = lds32(ra);
+                const int32_t qy = (int32_t)lds32(ra + 128);
+                __syncwarp();
+                const uint64_t v = pack2((float)qw * cw, (float)qy * cy);
+                uint32_t wa = ra + lane * 4;
+                sts64(wa, v);
+                for (int x = j + nb; x < nrows; x += nb) { wa += nb * kRowBytes; sts64(wa, v); }
+            }
         }
         __syncthreads();
 
         // ---- a3/a4 box search: this thread owns start tiles warp, warp+nw, ... of column `lane` --
         {
             float t_best; uint32_t key_best;
-            search_column(smem_raw + lane * 8, nb, kmin, kmax, warp, nw, t_best, key_best);
+            search_column<S>(bins_s + lane * 8, nb, kmin, kmax, warp, nw, t_best, key_best);
             red_v[warp * 32 + lane] = t_best;
             red_key[warp * 32 + lane] = key_best;
         }
         __syncthreads();
 
         // ---- merge the partial results of each column, canonicalise, recompute (r, s) ------------
-        if (warp == 0) {
+        if (warp < 4 && (lane >> 3) == warp) {    // 4 warps x 8 columns: the chains below are serial per column
             float bt = red_v[lane];
             uint32_t bkey = red_key[lane];
             for (int w = 1; w < nw; ++w) {
@@ -469,11 +572,11 @@ cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int n
 
 cudaError_t search_configure(int max_smem_optin)
 {
-    cudaError_t e = cudaFuncSetAttribute(search_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         max_smem_optin);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(search_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                max_smem_optin);
+    cudaError_t e = cudaFuncSetAttribute(search_kernel<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(search_kernel<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(search_kernel<true, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(search_kernel<false, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+    return e;
 }
 
 cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem, cudaStream_t st)
@@ -481,10 +584,13 @@ cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem
     const int64_t grid = chunk_curves * (int64_t)a.items_per_curve;
     if (grid <= 0) return cudaSuccess;
     if (grid > 2147483647LL) return cudaErrorInvalidConfiguration;
-    if (a.pts_in_smem)
-        search_kernel<true><<<(unsigned)grid, a.threads, smem, st>>>(a);
-    else
-        search_kernel<false><<<(unsigned)grid, a.threads, smem, st>>>(a);
+    if (a.starts_per_thread == 5) {
+        if (a.pts_in_smem) search_kernel<true, 5><<<(unsigned)grid, a.threads, smem, st>>>(a);
+        else search_kernel<false, 5><<<(unsigned)grid, a.threads, smem, st>>>(a);
+    } else {
+        if (a.pts_in_smem) search_kernel<true, 4><<<(unsigned)grid, a.threads, smem, st>>>(a);
+        else search_kernel<false, 4><<<(unsigned)grid, a.threads, smem, st>>>(a);
+    }
     return cudaGetLastError();
 }
 
