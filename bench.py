@@ -190,6 +190,7 @@ def main():
     ap.add_argument("--max-curves", type=int, default=0, help="run only a prefix of the configuration")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--flags", type=lambda v: int(v, 0), default=0, help="bls_config.flags (tuning only)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -225,7 +226,7 @@ def main():
     n_pts, n_curves = batch.n_points, batch.n_curves
     pf_per_step = float(n_pts) * grid.nf
 
-    plan = bls.Plan(n_bins=grid.nb, q_min=grid.qmin, q_max=grid.qmax, freqs=freqs, max_top_k=k, device=local_rank)
+    plan = bls.Plan(n_bins=grid.nb, q_min=grid.qmin, q_max=grid.qmax, freqs=freqs, max_top_k=k, device=local_rank, flags=args.flags)
     kmin, kmax = plan.kmin, plan.kmax
     t_d = torch.from_numpy(batch.t).to(dev)
     m_d = torch.from_numpy(batch.mag).to(dev)

@@ -78,8 +78,14 @@ typedef struct {
 #define BLS_FLAG_CANONICAL_PHASE 1u /* compute every bin index with the slow 3-rounding fp64 rule
                                        (R8) instead of the guarded fast path; results identical   */
 
-#define BLS_FLAG_WARPS(n) (((uint32_t)(n) & 0xffu) << 8) /* tuning: warps per CTA of the search kernel
-                                       (1..16; 0 = the library's choice).  Never changes results. */
+#define BLS_FLAG_SINGLE_BUFFER 2u    /* tuning: always use the single-buffer search kernel (every warp
+                                       does every phase) instead of the warp-specialised, double-
+                                       buffered one.  Never changes results.                       */
+#define BLS_FLAG_WARPS(n) (((uint32_t)(n) & 0xffu) << 8) /* tuning: warps per CTA that walk the boxes
+                                       (1..10; 0 = the library's choice).  Never changes results. */
+#define BLS_FLAG_FOLD_WARPS(n) (((uint32_t)(n) & 0xffu) << 16) /* tuning: warps per CTA that fold, in
+                                       the warp-specialised kernel (0 = the library's choice; box +
+                                       fold warps <= 20).  Never changes results.                  */
 
 /* Ragged CSR batch of light curves (per star a list of HJD times, calibrated
  * magnitudes and errors).  Curve c owns points [offsets[c], offsets[c+1]). */

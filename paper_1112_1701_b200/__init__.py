@@ -3,7 +3,10 @@ C-ABI library libbls_b200.so.  The CUDA kernels are the product; this package on
 arguments.  Importing it never builds or falls back to anything on the CPU."""
 from .binding import (  # noqa: F401
     BLS_FLAG_CANONICAL_PHASE,
+    BLS_FLAG_FOLD_WARPS,
     BLS_FLAG_NONE,
+    BLS_FLAG_SINGLE_BUFFER,
+    BLS_FLAG_WARPS,
     BlsError,
     EXPORTS,
     LIB_PATH,

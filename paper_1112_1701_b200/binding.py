@@ -21,7 +21,15 @@ EXPORTS = ["bls_plan_create", "bls_run", "bls_topk", "bls_search_host", "bls_pla
 
 BLS_OK = 0
 BLS_ERR_NULL, BLS_ERR_CONFIG, BLS_ERR_BATCH, BLS_ERR_ARG, BLS_ERR_CUDA, BLS_ERR_UNSUPPORTED = -1, -2, -3, -4, -5, -6
-BLS_FLAG_NONE, BLS_FLAG_CANONICAL_PHASE = 0, 1
+BLS_FLAG_NONE, BLS_FLAG_CANONICAL_PHASE, BLS_FLAG_SINGLE_BUFFER = 0, 1, 2
+
+
+def BLS_FLAG_WARPS(n):
+    return (int(n) & 0xff) << 8
+
+
+def BLS_FLAG_FOLD_WARPS(n):
+    return (int(n) & 0xff) << 16
 (QUERY_KMIN, QUERY_KMAX, QUERY_NBINS, QUERY_NFREQ, QUERY_SCRATCH_BYTES, QUERY_LAST_LAUNCHES,
  QUERY_LAST_CANONICAL, QUERY_TILE_FREQS, QUERY_SEARCH_CTAS, QUERY_LAST_SEARCH_NS) = range(1, 11)
 

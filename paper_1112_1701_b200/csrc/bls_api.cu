@@ -170,7 +170,7 @@ int bls_plan_create(const bls_config *cfg, bls_plan **out_plan)
         return BLS_ERR_CUDA;
     }
     p->bytes_owned = p->nf * (int64_t)sizeof(double) + 8;
-    if (search_smem_bytes(p->nb, p->kmax, kMaxSearchWarps, 0) > (size_t)p->max_smem_optin) {   // the bins alone must fit
+    if (search_smem_bytes(p->nb, p->kmax, kMaxSearchWarps, 1, 0) > (size_t)p->max_smem_optin) {   // the bins alone must fit
         release(p->d_freqs); release(p->d_canon);
         delete p;
         return BLS_ERR_UNSUPPORTED;
@@ -303,21 +303,32 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
 
     // ---- launch geometry of the search ---------------------------------------------------------
     const int ntiles = (int)((p->nf + kTileFreqs - 1) / kTileFreqs);
+    // Kernel 2 (warp-specialised, two bin buffers) whenever its buffers fit shared memory, with the
+    // curve staged in shared memory if that fits too; otherwise kernel 1 (one buffer, two CTAs per SM).
+    const size_t optin = (size_t)p->max_smem_optin;
+    const bool ws = !(p->flags & BLS_FLAG_SINGLE_BUFFER) &&
+                    search_smem_bytes(p->nb, p->kmax, kMaxSearchWarps, 2, 0) <= optin;
     int starts = 4, warps = 8;
-    search_geometry(p->nb, &starts, &warps);
+    // kernel 2 runs 8 box-search warps beside 12 fold warps (measured best at C1: the fold side is
+    // latency bound and wants the warps); kernel 1 uses up to 10 warps for everything
+    search_geometry(p->nb, ws ? 8 : kMaxSearchWarps, &starts, &warps);
     const int warps_flag = (int)((p->flags >> 8) & 0xffu);
     if (warps_flag >= 1 && warps_flag <= kMaxSearchWarps) warps = warps_flag;
-    const int threads = warps * 32;
-    size_t smem = search_smem_bytes(p->nb, p->kmax, warps, max_n);
+    int fold_warps = (int)((p->flags >> 16) & 0xffu);
+    if (fold_warps < 1 || warps + fold_warps > kWsMaxWarps) fold_warps = kWsMaxWarps - warps;
+    const int buffers = ws ? 2 : 1;
     int pts_in_smem = 1;
-    if (smem > (size_t)p->max_smem_optin) {        // curve too long to stage: read it through L1/L2
+    size_t smem = search_smem_bytes(p->nb, p->kmax, warps, buffers, max_n);
+    if (smem > optin) {                            // curve too long to stage: read it through L1/L2
         pts_in_smem = 0;
-        smem = search_smem_bytes(p->nb, p->kmax, warps, 0);
+        smem = search_smem_bytes(p->nb, p->kmax, warps, buffers, 0);
     }
+    const int threads = (ws ? warps + fold_warps : warps) * 32;
     int ctas_per_sm = (int)((size_t)(228 * 1024) / (smem + 1024));
     if (ctas_per_sm < 1) ctas_per_sm = 1;
-    if (ctas_per_sm > 2048 / threads) ctas_per_sm = 2048 / threads;
-    const int64_t target_ctas = (int64_t)p->sm_count * ctas_per_sm * 12;   // >= 12 waves hides the tail
+    if (ctas_per_sm > (ws ? 1 : 2)) ctas_per_sm = ws ? 1 : 2;      // register-limited (launch bounds)
+    const int waves = ws ? 24 : 12;                                 // enough waves to hide the tail
+    const int64_t target_ctas = (int64_t)p->sm_count * ctas_per_sm * waves;
     int64_t items = (target_ctas + chunk - 1) / chunk;
     if (items < 1) items = 1;
     if (items > ntiles) items = ntiles;
@@ -331,6 +342,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     a.tiles_per_item = tiles_per_item; a.items_per_curve = (int)items;
     a.pts_in_smem = pts_in_smem;
     a.starts_per_thread = starts;
+    a.search_warps = ws ? warps : 0;
     a.threads = threads;
     a.force_canonical = (p->flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0;
     a.sr = p->d_sr; a.ak = p->d_ak; a.depth = p->d_depth;

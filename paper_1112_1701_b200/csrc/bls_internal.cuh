@@ -37,6 +37,7 @@ struct PeakCand {
 constexpr int kTileFreqs = 32;        // frequencies per tile = lanes of a warp
 constexpr int kSearchThreads = 256;   // default: 8 warps per CTA
 constexpr int kMaxSearchWarps = 10;   // upper bound (BLS_FLAG_WARPS override); 2 CTAs x 10 warps x 96 registers fill an SM
+constexpr int kWsMaxWarps = 20;       // warp-specialised kernel: search warps + fold warps
 constexpr int kPrepThreads = 256;
 constexpr int kPeakThreads = 256;
 constexpr int kStartsPerThread = 4;   // register tile of the box search (A)
@@ -52,6 +53,7 @@ struct SearchArgs {
     int threads;                // CTA size of the search kernel (multiple of 32, <= 32*kMaxSearchWarps)
     int pts_in_smem;            // 1: stage the curve in shared memory, 0: read it through L1
     int starts_per_thread;      // S of the box search (4 or 5)
+    int search_warps;           // > 0: warp-specialised kernel with this many search warps (the rest fold)
     int force_canonical;        // BLS_FLAG_CANONICAL_PHASE
     float *sr;                  // chunk scratch, [chunk_curves][nf]
     uint32_t *ak;
@@ -107,8 +109,8 @@ __device__ __forceinline__ int fold_bin(double f, double t, int nb, uint32_t G, 
 // Bin rows a search CTA holds: the nb bins plus the cyclic extension the widest box of the last
 // start tile reaches (kmax rounded up to whole width blocks, plus the window's slack).
 __host__ __device__ inline int search_rows(int nb, int kmax) { return nb + ((kmax + 3) & ~3) + 4; }
-size_t search_smem_bytes(int nb, int kmax, int warps, int64_t n_points_in_smem);
-void search_geometry(int nb, int *starts_per_thread, int *warps);
+size_t search_smem_bytes(int nb, int kmax, int warps, int buffers, int64_t n_points_in_smem);
+void search_geometry(int nb, int max_warps, int *starts_per_thread, int *warps);
 cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int nb, int force_canon,
                               int32_t *bins, unsigned long long *n_canon, cudaStream_t st);
 cudaError_t search_configure(int max_smem_optin);

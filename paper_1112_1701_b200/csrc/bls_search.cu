@@ -26,23 +26,24 @@
 
 namespace bls {
 
-size_t search_smem_bytes(int nb, int kmax, int warps, int64_t n_points_in_smem)
+// `buffers` = 1 (search_kernel) or 2 (search_ws_kernel); `warps` = warps that write partial results
+size_t search_smem_bytes(int nb, int kmax, int warps, int buffers, int64_t n_points_in_smem)
 {
     size_t bins = (size_t)search_rows(nb, kmax) * kTileFreqs * 8;
     size_t red = (size_t)2 * warps * kTileFreqs * 4;
-    return bins + red + (size_t)n_points_in_smem * sizeof(PointRec);
+    return (size_t)buffers * (bins + red) + (size_t)n_points_in_smem * sizeof(PointRec);
 }
 
 // Geometry of the box search: a thread owns S consecutive start bins (S = 4 or 5), the
 // ceil(nb/S) start tiles of a column are dealt to the warps.  Pick (S, warps in [6,10]) that wastes
 // the fewest thread-tiles; ties go to S = 5 (fewer loads per box), then to more warps.
-void search_geometry(int nb, int *starts_per_thread, int *warps)
+void search_geometry(int nb, int max_warps, int *starts_per_thread, int *warps)
 {
     int best_s = 4, best_w = 8;
     double best_cost = 1e30;
     for (int s = 4; s <= 5; ++s) {
         const int nst = (nb + s - 1) / s;
-        for (int w = 6; w <= kMaxSearchWarps; ++w) {
+        for (int w = 6; w <= max_warps; ++w) {
             const int per = (nst + w - 1) / w;
             const double cost = (double)per * w * s / nb;      // thread-starts issued per useful start
             if (cost < best_cost - 1e-9 || (cost < best_cost + 1e-9 && (s > best_s || (s == best_s && w > best_w)))) {
@@ -209,7 +210,7 @@ template <int S, bool CHECK>
 __device__ __forceinline__ float block_max(uint64_t (&rs)[S], const uint64_t (&cur)[4], const uint64_t (&nxt)[4],
                                            int k0, int kmin, int kmax)
 {
-    float m = 0.f;
+    float mj[4] = {0.f, 0.f, 0.f, 0.f};           // one short FMNMX chain per width, joined at the end
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
 #pragma unroll
@@ -221,11 +222,11 @@ __device__ __forceinline__ float block_max(uint64_t (&rs)[S], const uint64_t (&c
                 unpack2(rs[u], r, s);
                 const float den = fmaf(-r, r, r);       // r (1 - r)
                 const float t = s * fast_rsqrt(den);
-                m = fmaxf(m, fabsf(t));
+                mj[j] = fmaxf(mj[j], fabsf(t));
             }
         }
     }
-    return m;
+    return fmaxf(fmaxf(mj[0], mj[1]), fmaxf(mj[2], mj[3]));
 }
 
 // Box search of one frequency column by one thread: start tiles tl = first, first+stride, ... of
@@ -335,46 +336,249 @@ __device__ __forceinline__ void search_column(uint32_t col, int nb, int kmin, in
     out_key = ((uint32_t)bk << 16) | (uint32_t)(tl * S + bu);
 }
 
+// ---- the phases of one tile (32 trial frequencies, one per lane), written for a GROUP of warps:
+//      `gw` = this warp's index in the group, `gnw` = warps in the group -------------------------
+
+struct TileCtx {
+    int nb, nrows, kmin, kmax, n;
+    uint32_t G;
+    bool force_canon;
+    float cw, cy, wx2;
+};
+
+__device__ __forceinline__ void zero_bins(uint32_t bins_s, int nb, int gtid, int gthreads)
+{
+    const int nvec = nb * (kRowBytes / 16);
+    for (int i = gtid; i < nvec; i += gthreads)
+        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(bins_s + i * 16), "r"(0u) : "memory");
+}
+
+// a2 Fold: warp gw takes groups of 4 consecutive points gw, gw+gnw, ...; lane l folds them at its
+// frequency f.  During the fold row b holds int32 planes W[b][lane] | Y[b][lane]: lane l always
+// hits bank l (and Y sits 128 B after W, one address register), so the native ATOMS.ADD is
+// conflict-free by construction.  Four points in flight hide the LDS / DFMA latency.
+template <bool PTS_SMEM>
+__device__ __forceinline__ void fold_tile(const TileCtx &c, double f, uint32_t bins_s, uint32_t pts_sa,
+                                          const PointRec *pts_g, int lane, int gw, int gnw, unsigned int &n_canon)
+{
+    const int nb = c.nb;
+    const uint32_t G = c.G;
+    const bool force_canon = c.force_canon;
+    const uint32_t colw = bins_s + lane * 4;       // W plane of this lane's column, row 0
+    const int ngroups = c.n >> 2;
+    if (PTS_SMEM) {
+        const uint32_t pa_end = pts_sa + ngroups * 64;
+        for (uint32_t pa = pts_sa + gw * 64; pa < pa_end; pa += gnw * 64) {
+            uint4 raw[4];
+            unsigned long long pr[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) raw[u] = lds128(pa + u * 16);
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                pr[u] = fast_bin_pos(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb, G);
+            const uint32_t lomin = min(min((uint32_t)pr[0], (uint32_t)pr[1]), min((uint32_t)pr[2], (uint32_t)pr[3]));
+            if (!force_canon && lomin >= 2u * G) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t addr = row_addr(colw, (uint32_t)(pr[u] >> 32));
+                    red_add(addr, raw[u].z);
+                    red_add(addr + 128, raw[u].w);
+                }
+            } else {                       // rare: some point sits within G of a bin edge
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    int bin = (int)(pr[u] >> 32);
+                    if (force_canon || (uint32_t)pr[u] < 2u * G) {
+                        bin = canonical_bin(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb);
+                        ++n_canon;
+                    }
+                    const uint32_t addr = colw + bin * kRowBytes;
+                    red_add(addr, raw[u].z);
+                    red_add(addr + 128, raw[u].w);
+                }
+            }
+        }
+    } else {
+        for (int g = gw; g < ngroups; g += gnw) {
+            PointRec p[4];
+            int bin[4];
+            uint32_t lo[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) p[u] = load_point<false>(pts_g + g * 4 + u);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) bin[u] = fast_bin(f, p[u].t, nb, G, lo[u]);
+            if (force_canon || min(min(lo[0], lo[1]), min(lo[2], lo[3])) < 2u * G) {
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (force_canon || lo[u] < 2u * G) { bin[u] = canonical_bin(f, p[u].t, nb); ++n_canon; }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t addr = colw + bin[u] * kRowBytes;
+                red_add(addr, p[u].qw);
+                red_add(addr + 128, (uint32_t)p[u].qy);
+            }
+        }
+    }
+    if (gw == ngroups % gnw) {             // the n % 4 points after the last whole group
+        for (int i = ngroups * 4; i < c.n; ++i) {
+            PointRec p;
+            if (PTS_SMEM) {
+                const uint4 raw = lds128(pts_sa + i * 16);
+                p.t = __hiloint2double((int)raw.y, (int)raw.x); p.qw = raw.z; p.qy = (int32_t)raw.w;
+            } else {
+                p = load_point<false>(pts_g + i);
+            }
+            const int bin = fold_bin(f, p.t, nb, G, force_canon, n_canon);
+            const uint32_t addr = colw + bin * kRowBytes;
+            red_add(addr, p.qw);
+            red_add(addr + 128, (uint32_t)p.qy);
+        }
+    }
+}
+
+// fixed point -> fp32 pairs (weight fraction, weighted residual), in place, plus the cyclic
+// extension rows nb .. nrows-1.  A warp owns whole rows, so reading both int planes before
+// writing the pairs needs only a warp sync.
+__device__ __forceinline__ void convert_rows(const TileCtx &c, uint32_t bins_s, int lane, int gw, int gnw)
+{
+    const int nb = c.nb;
+    const int next = c.nrows - nb;                // extension rows
+    uint32_t ra = bins_s + gw * kRowBytes + lane * 4;
+    if (next <= nb) {                             // every shape but tiny nb with wide boxes
+        for (int j = gw; j < nb; j += gnw, ra += gnw * kRowBytes) {
+            const uint32_t qw = lds32(ra);
+            const int32_t qy = (int32_t)lds32(ra + 128);
+            __syncwarp();
+            const uint64_t v = pack2((float)qw * c.cw, (float)qy * c.cy);
+            const uint32_t wa = ra + lane * 4;
+            sts64(wa, v);
+            if (j < next) sts64(wa + nb * kRowBytes, v);
+        }
+    } else {
+        for (int j = gw; j < nb; j += gnw, ra += gnw * kRowBytes) {
+            const uint32_t qw = lds32(ra);
+            const int32_t qy = (int32_t)lds32(ra + 128);
+            __syncwarp();
+            const uint64_t v = pack2((float)qw * c.cw, (float)qy * c.cy);
+            uint32_t wa = ra + lane * 4;
+            sts64(wa, v);
+            for (int x = j + nb; x < c.nrows; x += nb) { wa += nb * kRowBytes; sts64(wa, v); }
+        }
+    }
+}
+
+// Outputs of one (curve, frequency).
+struct OutPtrs {
+    float *sr; uint32_t *ak; float *depth;        // chunk scratch, row of this curve
+    float *u_sr; uint16_t *u_start; uint16_t *u_width; float *u_depth;   // user rows or NULL
+};
+
+// Merge the per-warp partial results of column `lane`, canonicalise exact ties (R12), recompute
+// (r, s) of the chosen box by direct summation and write SR = s^2/den, depth = s/den (IEEE
+// division).  The chains below are serial per column, so callers spread the 32 columns over
+// several warps.
+__device__ __forceinline__ void merge_column(const TileCtx &c, const float2 *rows2, const float *red_v,
+                                             const uint32_t *red_key, int nparts, int lane, int q, int nf,
+                                             const OutPtrs &o)
+{
+    const int nb = c.nb, kmin = c.kmin, kmax = c.kmax;
+    float bt = red_v[lane];
+    uint32_t bkey = red_key[lane];
+    for (int w = 1; w < nparts; ++w) {
+        const float v = red_v[w * 32 + lane];
+        if (v > bt) { bt = v; bkey = red_key[w * 32 + lane]; }
+    }
+    const Column col{rows2 + lane, nb};
+    float bv = bt * bt;
+    if (!(bv <= 1.001f * c.wx2 + 1e-30f)) {   // inf / impossible: r == 1.0f box
+        careful_search(col, kmin, kmax, bv, bkey);
+        bt = bv;
+    }
+    int bk = (int)(bkey >> 16), ba = (int)(bkey & 0xffffu);
+    if (bt > 0.f) canonicalise(col, kmin, ba, bk);
+    else { bk = kmin; ba = 0; }
+    float r = 0.f, s = 0.f;
+    for (int j = 0; j < bk; ++j) {
+        int b = ba + j; if (b >= nb) b -= nb;
+        r += col.W(b); s += col.Y(b);
+    }
+    const float den = fmaf(-r, r, r);
+    float sr = 0.f, dp = 0.f;
+    if (bt > 0.f && den > 0.f) { sr = (s * s) / den; dp = s / den; }
+    if (q < nf) {
+        o.sr[q] = sr; o.ak[q] = ((uint32_t)bk << 16) | (uint32_t)ba; o.depth[q] = dp;
+        if (o.u_sr) o.u_sr[q] = sr;
+        if (o.u_start) o.u_start[q] = (uint16_t)ba;
+        if (o.u_width) o.u_width[q] = (uint16_t)bk;
+        if (o.u_depth) o.u_depth[q] = dp;
+    }
+}
+
+__device__ __forceinline__ OutPtrs out_rows(const SearchArgs &a, int64_t curve_local, int64_t c)
+{
+    OutPtrs o;
+    o.sr = a.sr + curve_local * a.nf; o.ak = a.ak + curve_local * a.nf; o.depth = a.depth + curve_local * a.nf;
+    o.u_sr = a.u_sr ? a.u_sr + c * a.nf : nullptr;
+    o.u_start = a.u_start ? a.u_start + c * a.nf : nullptr;
+    o.u_width = a.u_width ? a.u_width + c * a.nf : nullptr;
+    o.u_depth = a.u_depth ? a.u_depth + c * a.nf : nullptr;
+    return o;
+}
+
+// data fault: zero-filled spectrum (include/bls.h)
+__device__ __forceinline__ void zero_fill_outputs(const OutPtrs &o, int q_begin, int q_end, int kmin, int tid, int nthr)
+{
+    for (int q = q_begin + tid; q < q_end; q += nthr) {
+        o.sr[q] = 0.f; o.ak[q] = (uint32_t)kmin << 16; o.depth[q] = 0.f;
+        if (o.u_sr) o.u_sr[q] = 0.f;
+        if (o.u_start) o.u_start[q] = 0;
+        if (o.u_width) o.u_width[q] = (uint16_t)kmin;
+        if (o.u_depth) o.u_depth[q] = 0.f;
+    }
+}
+
+__device__ __forceinline__ void count_canonical(const SearchArgs &a, unsigned int n_canon, int lane)
+{
+    if (a.canon_count) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) n_canon += __shfl_xor_sync(0xffffffffu, n_canon, o);
+        if (lane == 0 && n_canon) atomicAdd(a.canon_count, (unsigned long long)n_canon);
+    }
+}
+
+// ---- kernel 1: every warp does every phase, phases separated by CTA barriers.  Used where the
+//      double-buffered bins of kernel 2 do not fit shared memory (e.g. nb = 400).  Two CTAs per
+//      SM overlap each other's LSU-bound fold and XU-bound box search only by chance. -----------
 template <bool PTS_SMEM, int S>
 __global__ void __launch_bounds__(kMaxSearchWarps * 32, 2)
 search_kernel(const SearchArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int nb = a.nb;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nthr = blockDim.x, nw = nthr >> 5;
-    const int nrows = search_rows(nb, a.kmax);
-    // During the fold row b holds int32 planes  W[b][lane] | Y[b][lane]  (lane l always hits bank l,
-    // Y sits 128 B after W so both atomics share one address register); the convert pass rewrites
-    // the row in place as fp32 pairs (W, Y)[lane] and fills the cyclic extension rows nb .. nrows-1.
-    uint32_t *Wb = reinterpret_cast<uint32_t *>(smem_raw);                          // [nrows][64]
-    int32_t *Yb = reinterpret_cast<int32_t *>(Wb + 32);
-    float *red_v = reinterpret_cast<float *>(Wb + nrows * 64);                      // [nw][32]
-    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + nw * 32);              // [nw][32]
-    PointRec *pts_s = reinterpret_cast<PointRec *>(red_key + nw * 32);              // [n] if PTS_SMEM
-    const float2 *rows2 = reinterpret_cast<const float2 *>(smem_raw);               // [nrows][32] after convert
+    TileCtx c;
+    c.nb = a.nb; c.kmin = a.kmin; c.kmax = a.kmax;
+    c.nrows = search_rows(a.nb, a.kmax);
+    // smem: bins [nrows][256 B] | red_v [nw][32] | red_key [nw][32] | points [n] (if PTS_SMEM)
+    float *red_v = reinterpret_cast<float *>(smem_raw + (size_t)c.nrows * kRowBytes);
+    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + nw * 32);
+    PointRec *pts_s = reinterpret_cast<PointRec *>(red_key + nw * 32);
+    const float2 *rows2 = reinterpret_cast<const float2 *>(smem_raw);
 
     const int64_t curve_local = blockIdx.x / a.items_per_curve;
     const int item = blockIdx.x % a.items_per_curve;
-    const int64_t c = a.curve_base + curve_local;
-    const int64_t beg = a.offsets[c];
-    const int n = (int)(a.offsets[c + 1] - beg);
-    const CurveMeta meta = a.meta[c];
+    const int64_t cv = a.curve_base + curve_local;
+    const int64_t beg = a.offsets[cv];
+    c.n = (int)(a.offsets[cv + 1] - beg);
+    const CurveMeta meta = a.meta[cv];
     const int ntiles = (a.nf + kTileFreqs - 1) / kTileFreqs;
     const int tile0 = item * a.tiles_per_item;
     const int tile1 = min(tile0 + a.tiles_per_item, ntiles);
-    const int kmin = a.kmin, kmax = a.kmax;
+    const OutPtrs out = out_rows(a, curve_local, cv);
 
-    if (meta.status != BLS_CURVE_OK) {   // data fault: zero-filled spectrum (include/bls.h)
-        for (int q = tile0 * kTileFreqs + tid; q < min(tile1 * kTileFreqs, a.nf); q += nthr) {
-            a.sr[curve_local * a.nf + q] = 0.f;
-            a.ak[curve_local * a.nf + q] = (uint32_t)kmin << 16;
-            a.depth[curve_local * a.nf + q] = 0.f;
-            if (a.u_sr) a.u_sr[c * a.nf + q] = 0.f;
-            if (a.u_start) a.u_start[c * a.nf + q] = 0;
-            if (a.u_width) a.u_width[c * a.nf + q] = (uint16_t)kmin;
-            if (a.u_depth) a.u_depth[c * a.nf + q] = 0.f;
-        }
+    if (meta.status != BLS_CURVE_OK) {
+        zero_fill_outputs(out, tile0 * kTileFreqs, min(tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
         return;
     }
 
@@ -383,167 +587,145 @@ search_kernel(const SearchArgs a)
     if (PTS_SMEM) {
         const uint4 *src = reinterpret_cast<const uint4 *>(pts_g);
         uint4 *dst = reinterpret_cast<uint4 *>(pts_s);
-        for (int i = tid; i < n; i += nthr) dst[i] = __ldg(src + i);
+        for (int i = tid; i < c.n; i += nthr) dst[i] = __ldg(src + i);
     }
-    const PointRec *P = PTS_SMEM ? pts_s : pts_g;
     const uint32_t bins_s = smem_u32(smem_raw), pts_sa = smem_u32(pts_s);
-    const bool force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
-    const float cw = meta.cw, cy = meta.cy;
-    const uint32_t G = (uint32_t)nb + 8u;         // guard band, units of 2^-32 bin
+    c.force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
+    c.cw = meta.cw; c.cy = meta.cy; c.wx2 = (float)meta.wx2;
+    c.G = (uint32_t)a.nb + 8u;                    // guard band, units of 2^-32 bin
     unsigned int n_canon = 0;
-    const int tail_warp = (n >> 2) % nw;
 
     for (int tile = tile0; tile < tile1; ++tile) {
         const int q0 = tile * kTileFreqs;
-        const int q = min(q0 + lane, a.nf - 1);    // ragged last tile: surplus lanes repeat the last f
-        const double f = a.freqs[q];
-
-        // ---- zero the tile's bins -------------------------------------------------------------
-        {
-            uint4 *z = reinterpret_cast<uint4 *>(Wb);
-            const int nvec = nb * 16;              // 2 * nb * 32 words / 4
-            for (int i = tid; i < nvec; i += nthr) z[i] = make_uint4(0u, 0u, 0u, 0u);
-        }
+        const double f = a.freqs[min(q0 + lane, a.nf - 1)];   // ragged last tile: surplus lanes repeat the last f
+        zero_bins(bins_s, c.nb, tid, nthr);
         __syncthreads();
-
-        // ---- a2 Fold: warp w takes groups of 4 consecutive points w, w+nw, ...; lane l folds them
-        //      at its frequency.  Four points in flight hide the LDS / DFMA latency. --------------
-        {
-            const uint32_t colw = bins_s + lane * 4;       // W plane of this lane's column, row 0
-            const int ngroups = n >> 2;
-            if (PTS_SMEM) {
-                const uint32_t pa_end = pts_sa + ngroups * 64;
-                for (uint32_t pa = pts_sa + warp * 64; pa < pa_end; pa += nw * 64) {
-                    uint4 raw[4];
-                    unsigned long long pr[4];
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) raw[u] = lds128(pa + u * 16);
-#pragma unroll
-                    for (int u = 0; u < 4; ++u)
-                        pr[u] = fast_bin_pos(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb, G);
-                    const uint32_t lomin = min(min((uint32_t)pr[0], (uint32_t)pr[1]), min((uint32_t)pr[2], (uint32_t)pr[3]));
-                    if (!force_canon && lomin >= 2u * G) {
-#pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            const uint32_t addr = row_addr(colw, (uint32_t)(pr[u] >> 32));
-                            red_add(addr, raw[u].z);
-                            red_add(addr + 128, raw[u].w);
-                        }
-                    } else {                       // rare: some point sits within G of a bin edge
-#pragma unroll
-                        for (int u = 0; u < 4; ++u) {
-                            int bin = (int)(pr[u] >> 32);
-                            if (force_canon || (uint32_t)pr[u] < 2u * G) {
-                                bin = canonical_bin(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb);
-                                ++n_canon;
-                            }
-                            const uint32_t addr = colw + bin * kRowBytes;
-                            red_add(addr, raw[u].z);
-                            red_add(addr + 128, raw[u].w);
-                        }
-                    }
-                }
-            } else {
-                for (int g = warp; g < ngroups; g += nw) {
-                    PointRec p[4];
-                    int bin[4];
-                    uint32_t lo[4];
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) p[u] = load_point<false>(pts_g + g * 4 + u);
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) bin[u] = fast_bin(f, p[u].t, nb, G, lo[u]);
-                    if (force_canon || min(min(lo[0], lo[1]), min(lo[2], lo[3])) < 2u * G) {
-#pragma unroll
-                        for (int u = 0; u < 4; ++u)
-                            if (force_canon || lo[u] < 2u * G) { bin[u] = canonical_bin(f, p[u].t, nb); ++n_canon; }
-                    }
-#pragma unroll
-                    for (int u = 0; u < 4; ++u) {
-                        const uint32_t addr = colw + bin[u] * kRowBytes;
-                        red_add(addr, p[u].qw);
-                        red_add(addr + 128, (uint32_t)p[u].qy);
-                    }
-                }
-            }
-            if (warp == tail_warp) {               // the n % 4 points after the last whole group
-                for (int i = ngroups * 4; i < n; ++i) {
-                    const PointRec p = load_point<PTS_SMEM>(P + i);
-                    const int bin = fold_bin(f, p.t, nb, G, force_canon, n_canon);
-                    const uint32_t addr = colw + bin * kRowBytes;
-                    red_add(addr, p.qw);
-                    red_add(addr + 128, (uint32_t)p.qy);
-                }
-            }
-        }
+        fold_tile<PTS_SMEM>(c, f, bins_s, pts_sa, pts_g, lane, warp, nw, n_canon);
         __syncthreads();
-
-        // ---- fixed point -> fp32 pairs (weight fraction, weighted residual), in place; a warp owns
-        //      whole rows, so reading both planes before writing the pairs needs only a warp sync ----
-        {
-            uint32_t ra = bins_s + warp * kRowBytes + lane * 4;
-            for (int j = warp; j < nb; j += nw, ra += nw * kRowBytes) {
-                const uint32_t qw = lds32(ra);
-                const int32_t qy = (int32_t)lds32(ra + 128);
-                __syncwarp();
-                const uint64_t v = pack2((float)qw * cw, (float)qy * cy);
-                uint32_t wa = ra + lane * 4;
-                sts64(wa, v);
-                for (int x = j + nb; x < nrows; x += nb) { wa += nb * kRowBytes; sts64(wa, v); }
-            }
-        }
+        convert_rows(c, bins_s, lane, warp, nw);
         __syncthreads();
-
         // ---- a3/a4 box search: this thread owns start tiles warp, warp+nw, ... of column `lane` --
         {
             float t_best; uint32_t key_best;
-            search_column<S>(bins_s + lane * 8, nb, kmin, kmax, warp, nw, t_best, key_best);
+            search_column<S>(bins_s + lane * 8, c.nb, c.kmin, c.kmax, warp, nw, t_best, key_best);
             red_v[warp * 32 + lane] = t_best;
             red_key[warp * 32 + lane] = key_best;
         }
         __syncthreads();
-
-        // ---- merge the partial results of each column, canonicalise, recompute (r, s) ------------
-        if (warp < 4 && (lane >> 3) == warp) {    // 4 warps x 8 columns: the chains below are serial per column
-            float bt = red_v[lane];
-            uint32_t bkey = red_key[lane];
-            for (int w = 1; w < nw; ++w) {
-                const float v = red_v[w * 32 + lane];
-                if (v > bt) { bt = v; bkey = red_key[w * 32 + lane]; }
-            }
-            const Column col{rows2 + lane, nb};
-            float bv = bt * bt;
-            if (!(bv <= 1.001f * (float)meta.wx2 + 1e-30f)) {   // inf / impossible: r == 1.0f box
-                careful_search(col, kmin, kmax, bv, bkey);
-                bt = bv;
-            }
-            int bk = (int)(bkey >> 16), ba = (int)(bkey & 0xffffu);
-            if (bt > 0.f) canonicalise(col, kmin, ba, bk);
-            else { bk = kmin; ba = 0; }
-            float r = 0.f, s = 0.f;
-            for (int j = 0; j < bk; ++j) {
-                int b = ba + j; if (b >= nb) b -= nb;
-                r += col.W(b); s += col.Y(b);
-            }
-            const float den = fmaf(-r, r, r);
-            float sr = 0.f, dp = 0.f;
-            if (bt > 0.f && den > 0.f) { sr = (s * s) / den; dp = s / den; }
-            if (q0 + lane < a.nf) {
-                const int64_t o = curve_local * a.nf + q0 + lane;
-                a.sr[o] = sr; a.ak[o] = ((uint32_t)bk << 16) | (uint32_t)ba; a.depth[o] = dp;
-                const int64_t uo = c * a.nf + q0 + lane;
-                if (a.u_sr) a.u_sr[uo] = sr;
-                if (a.u_start) a.u_start[uo] = (uint16_t)ba;
-                if (a.u_width) a.u_width[uo] = (uint16_t)bk;
-                if (a.u_depth) a.u_depth[uo] = dp;
-            }
-        }
+        if (warp < 4 && (lane >> 3) == warp)      // 4 warps x 8 columns
+            merge_column(c, rows2, red_v, red_key, nw, lane, q0 + lane, a.nf, out);
         __syncthreads();
     }
+    count_canonical(a, n_canon, lane);
+}
 
-    if (a.canon_count) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) n_canon += __shfl_xor_sync(0xffffffffu, n_canon, o);
-        if (lane == 0 && n_canon) atomicAdd(a.canon_count, (unsigned long long)n_canon);
+// ---- kernel 2: warp-specialised, double-buffered.  The fold is bound by the LSU pipe (shared
+//      atomics + point broadcasts), the box search by the XU pipe (one MUFU.RSQ per box): run
+//      them CONCURRENTLY on different warps so the SM is busy for max(fold, search), not their
+//      sum.  "Fold warps" zero / fold / convert tile i+1 (and merge tile i-1) into one bin buffer
+//      while "search warps" walk the boxes of tile i in the other.  Hand-off by named barriers
+//      (bar.arrive by the producer side, bar.sync by the consumer side). --------------------------
+__device__ __forceinline__ void named_sync(int id, int count)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
+__device__ __forceinline__ void named_arrive(int id, int count)
+{
+    __threadfence_block();
+    asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory");
+}
+enum { kBarFull0 = 1, kBarFull1 = 2, kBarDone0 = 3, kBarDone1 = 4, kBarFoldGroup = 5 };
+
+template <bool PTS_SMEM, int S>
+__global__ void __launch_bounds__(kWsMaxWarps * 32, 1)
+search_ws_kernel(const SearchArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nthr = blockDim.x;
+    const int nsw = a.search_warps, nfw = (nthr >> 5) - nsw;      // search warps come first
+    TileCtx c;
+    c.nb = a.nb; c.kmin = a.kmin; c.kmax = a.kmax;
+    c.nrows = search_rows(a.nb, a.kmax);
+    // smem: bins[2] [nrows][256 B] | red_v[2] [nsw][32] | red_key[2] [nsw][32] | points [n]
+    const size_t buf_bytes = (size_t)c.nrows * kRowBytes;
+    float *red_v = reinterpret_cast<float *>(smem_raw + 2 * buf_bytes);
+    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + 2 * nsw * 32);
+    PointRec *pts_s = reinterpret_cast<PointRec *>(red_key + 2 * nsw * 32);
+
+    const int64_t curve_local = blockIdx.x / a.items_per_curve;
+    const int item = blockIdx.x % a.items_per_curve;
+    const int64_t cv = a.curve_base + curve_local;
+    const int64_t beg = a.offsets[cv];
+    c.n = (int)(a.offsets[cv + 1] - beg);
+    const CurveMeta meta = a.meta[cv];
+    const int ntiles = (a.nf + kTileFreqs - 1) / kTileFreqs;
+    const int tile0 = item * a.tiles_per_item;
+    const int tile1 = min(tile0 + a.tiles_per_item, ntiles);
+    const OutPtrs out = out_rows(a, curve_local, cv);
+
+    if (meta.status != BLS_CURVE_OK) {
+        zero_fill_outputs(out, tile0 * kTileFreqs, min(tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
+        return;
+    }
+
+    const PointRec *pts_g = a.pts + beg;
+    if (PTS_SMEM) {                               // a1 Load, by all warps
+        const uint4 *src = reinterpret_cast<const uint4 *>(pts_g);
+        uint4 *dst = reinterpret_cast<uint4 *>(pts_s);
+        for (int i = tid; i < c.n; i += nthr) dst[i] = __ldg(src + i);
+    }
+    __syncthreads();
+    const uint32_t bins_s = smem_u32(smem_raw), pts_sa = smem_u32(pts_s);
+    c.force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
+    c.cw = meta.cw; c.cy = meta.cy; c.wx2 = (float)meta.wx2;
+    c.G = (uint32_t)a.nb + 8u;
+
+    if (warp < nsw) {
+        // ================= search warps: a3/a4 only =================
+        for (int tile = tile0, it = 0; tile < tile1; ++tile, ++it) {
+            const int b = it & 1;
+            named_sync(kBarFull0 + b, nthr);                      // buffer b holds tile's fp32 rows
+            float t_best; uint32_t key_best;
+            search_column<S>(bins_s + b * (uint32_t)buf_bytes + lane * 8, c.nb, c.kmin, c.kmax, warp, nsw, t_best, key_best);
+            red_v[(b * nsw + warp) * 32 + lane] = t_best;
+            red_key[(b * nsw + warp) * 32 + lane] = key_best;
+            named_arrive(kBarDone0 + b, nthr);                    // done with buffer b
+        }
+    } else {
+        // ================= fold warps: zero, a2 fold, convert, merge =================
+        const int gw = warp - nsw, gtid = tid - nsw * 32, gthreads = nfw * 32;
+        unsigned int n_canon = 0;
+        auto merge = [&](int tile, int b) {
+            const int mw = min(nfw, 4), per = (32 + mw - 1) / mw;  // mw warps x ceil(32/mw) columns
+            if (gw < mw && lane / per == gw)
+                merge_column(c, reinterpret_cast<const float2 *>(smem_raw + b * buf_bytes), red_v + b * nsw * 32,
+                             red_key + b * nsw * 32, nsw, lane, tile * kTileFreqs + lane, a.nf, out);
+        };
+        for (int tile = tile0, it = 0; tile < tile1; ++tile, ++it) {
+            const int b = it & 1;
+            const uint32_t buf = bins_s + b * (uint32_t)buf_bytes;
+            if (it >= 2) {                                        // tile-2 used this buffer: wait, then merge it
+                named_sync(kBarDone0 + b, nthr);
+                merge(tile - 2, b);
+                named_sync(kBarFoldGroup, gthreads);
+            }
+            const double f = a.freqs[min(tile * kTileFreqs + lane, a.nf - 1)];
+            zero_bins(buf, c.nb, gtid, gthreads);
+            named_sync(kBarFoldGroup, gthreads);
+            fold_tile<PTS_SMEM>(c, f, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
+            named_sync(kBarFoldGroup, gthreads);
+            convert_rows(c, buf, lane, gw, nfw);
+            named_arrive(kBarFull0 + b, nthr);
+        }
+        // drain: the last (up to) two tiles
+        const int nt = tile1 - tile0;
+        for (int it = max(nt - 2, 0); it < nt; ++it) {
+            const int b = it & 1;
+            named_sync(kBarDone0 + b, nthr);
+            merge(tile0 + it, b);
+        }
+        count_canonical(a, n_canon, lane);
     }
 }
 
@@ -572,11 +754,15 @@ cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int n
 
 cudaError_t search_configure(int max_smem_optin)
 {
-    cudaError_t e = cudaFuncSetAttribute(search_kernel<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(search_kernel<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(search_kernel<true, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(search_kernel<false, 5>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
-    return e;
+    const void *fns[] = {(const void *)search_kernel<true, 4>,    (const void *)search_kernel<false, 4>,
+                         (const void *)search_kernel<true, 5>,    (const void *)search_kernel<false, 5>,
+                         (const void *)search_ws_kernel<true, 4>, (const void *)search_ws_kernel<false, 4>,
+                         (const void *)search_ws_kernel<true, 5>, (const void *)search_ws_kernel<false, 5>};
+    for (const void *f : fns) {
+        cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem, cudaStream_t st)
@@ -584,13 +770,20 @@ cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem
     const int64_t grid = chunk_curves * (int64_t)a.items_per_curve;
     if (grid <= 0) return cudaSuccess;
     if (grid > 2147483647LL) return cudaErrorInvalidConfiguration;
-    if (a.starts_per_thread == 5) {
-        if (a.pts_in_smem) search_kernel<true, 5><<<(unsigned)grid, a.threads, smem, st>>>(a);
-        else search_kernel<false, 5><<<(unsigned)grid, a.threads, smem, st>>>(a);
-    } else {
-        if (a.pts_in_smem) search_kernel<true, 4><<<(unsigned)grid, a.threads, smem, st>>>(a);
-        else search_kernel<false, 4><<<(unsigned)grid, a.threads, smem, st>>>(a);
-    }
+    const unsigned g = (unsigned)grid;
+#define BLS_LAUNCH(K)                                                                   \
+    do {                                                                                \
+        if (a.starts_per_thread == 5) {                                                 \
+            if (a.pts_in_smem) K<true, 5><<<g, a.threads, smem, st>>>(a);               \
+            else K<false, 5><<<g, a.threads, smem, st>>>(a);                            \
+        } else {                                                                        \
+            if (a.pts_in_smem) K<true, 4><<<g, a.threads, smem, st>>>(a);               \
+            else K<false, 4><<<g, a.threads, smem, st>>>(a);                            \
+        }                                                                               \
+    } while (0)
+    if (a.search_warps > 0) BLS_LAUNCH(search_ws_kernel);
+    else BLS_LAUNCH(search_kernel);
+#undef BLS_LAUNCH
     return cudaGetLastError();
 }
 

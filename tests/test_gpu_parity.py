@@ -59,6 +59,31 @@ def test_small_configs_element_by_element(name):
     check_config(name)
 
 
+@pytest.mark.parametrize("name", ["T0", "T1", "T2"])
+def test_small_configs_single_buffer_kernel(name):
+    """The same cases through the single-buffer search kernel (the one shapes too large for the
+    double-buffered, warp-specialised kernel fall back to)."""
+    import paper_1112_1701_b200 as bls
+    check_config(name, flags=bls.BLS_FLAG_SINGLE_BUFFER)
+
+
+def test_kernel_variants_give_identical_results():
+    """Warp counts and kernel choice are tuning only.  Bins are exact integers and every box is scored by
+    the same instructions, so spectra agree to rounding; they are not bitwise equal because boxes whose
+    approximate rank (MUFU.RSQ) ties exactly are merged in warp order."""
+    import paper_1112_1701_b200 as bls
+    cfg = synth.config("T1")
+    batch = synth.make_batch(cfg)
+    ref = run_gpu(batch, cfg["grid"], top_k=5)
+    for flags in (bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_WARPS(6) | bls.BLS_FLAG_FOLD_WARPS(3),
+                  bls.BLS_FLAG_WARPS(7) | bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_WARPS(10) | bls.BLS_FLAG_FOLD_WARPS(1)):
+        g = run_gpu(batch, cfg["grid"], top_k=5, flags=flags)
+        np.testing.assert_allclose(g["sr"], ref["sr"], rtol=2e-6, atol=0)
+        same = (g["a"] == ref["a"]) & (g["k"] == ref["k"])
+        assert same.mean() > 0.999
+        assert (g["sr"] == ref["sr"])[same].all() and (g["depth"] == ref["depth"])[same].all()
+
+
 def test_c0_whole():
     g, rep = check_config("C0")
     cfg = synth.config("C0")
