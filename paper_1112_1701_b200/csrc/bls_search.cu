@@ -353,6 +353,47 @@ __device__ __forceinline__ void zero_bins(uint32_t bins_s, int nb, int gtid, int
         asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(bins_s + i * 16), "r"(0u) : "memory");
 }
 
+// NG groups of 4 consecutive points (group g at shared address pa + g*step) folded at frequency f:
+// all loads first, then the phases, then the atomics, so 4*NG points are in flight per warp.
+template <int NG>
+__device__ __forceinline__ void fold_groups(const TileCtx &c, double f, uint32_t colw, uint32_t pa, uint32_t step,
+                                            unsigned int &n_canon)
+{
+    constexpr int NP = 4 * NG;
+    const int nb = c.nb;
+    const uint32_t G = c.G;
+    uint4 raw[NP];
+    unsigned long long pr[NP];
+#pragma unroll
+    for (int u = 0; u < NP; ++u) raw[u] = lds128(pa + (u >> 2) * step + (u & 3) * 16);
+    uint32_t lomin = 0xffffffffu;
+#pragma unroll
+    for (int u = 0; u < NP; ++u) {
+        pr[u] = fast_bin_pos(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb, G);
+        lomin = min(lomin, (uint32_t)pr[u]);
+    }
+    if (!c.force_canon && lomin >= 2u * G) {
+#pragma unroll
+        for (int u = 0; u < NP; ++u) {
+            const uint32_t addr = row_addr(colw, (uint32_t)(pr[u] >> 32));
+            red_add(addr, raw[u].z);
+            red_add(addr + 128, raw[u].w);
+        }
+    } else {                       // rare: some point sits within G of a bin edge
+#pragma unroll
+        for (int u = 0; u < NP; ++u) {
+            int bin = (int)(pr[u] >> 32);
+            if (c.force_canon || (uint32_t)pr[u] < 2u * G) {
+                bin = canonical_bin(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb);
+                ++n_canon;
+            }
+            const uint32_t addr = colw + bin * kRowBytes;
+            red_add(addr, raw[u].z);
+            red_add(addr + 128, raw[u].w);
+        }
+    }
+}
+
 // a2 Fold: warp gw takes groups of 4 consecutive points gw, gw+gnw, ...; lane l folds them at its
 // frequency f.  During the fold row b holds int32 planes W[b][lane] | Y[b][lane]: lane l always
 // hits bank l (and Y sits 128 B after W, one address register), so the native ATOMS.ADD is
@@ -367,37 +408,9 @@ __device__ __forceinline__ void fold_tile(const TileCtx &c, double f, uint32_t b
     const uint32_t colw = bins_s + lane * 4;       // W plane of this lane's column, row 0
     const int ngroups = c.n >> 2;
     if (PTS_SMEM) {
-        const uint32_t pa_end = pts_sa + ngroups * 64;
-        for (uint32_t pa = pts_sa + gw * 64; pa < pa_end; pa += gnw * 64) {
-            uint4 raw[4];
-            unsigned long long pr[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) raw[u] = lds128(pa + u * 16);
-#pragma unroll
-            for (int u = 0; u < 4; ++u)
-                pr[u] = fast_bin_pos(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb, G);
-            const uint32_t lomin = min(min((uint32_t)pr[0], (uint32_t)pr[1]), min((uint32_t)pr[2], (uint32_t)pr[3]));
-            if (!force_canon && lomin >= 2u * G) {
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const uint32_t addr = row_addr(colw, (uint32_t)(pr[u] >> 32));
-                    red_add(addr, raw[u].z);
-                    red_add(addr + 128, raw[u].w);
-                }
-            } else {                       // rare: some point sits within G of a bin edge
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    int bin = (int)(pr[u] >> 32);
-                    if (force_canon || (uint32_t)pr[u] < 2u * G) {
-                        bin = canonical_bin(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb);
-                        ++n_canon;
-                    }
-                    const uint32_t addr = colw + bin * kRowBytes;
-                    red_add(addr, raw[u].z);
-                    red_add(addr + 128, raw[u].w);
-                }
-            }
-        }
+        const uint32_t pa_end = pts_sa + ngroups * 64, step = gnw * 64;
+        uint32_t pa = pts_sa + gw * 64;
+        for (; pa < pa_end; pa += step) fold_groups<1>(c, f, colw, pa, step, n_canon);
     } else {
         for (int g = gw; g < ngroups; g += gnw) {
             PointRec p[4];
@@ -446,7 +459,21 @@ __device__ __forceinline__ void convert_rows(const TileCtx &c, uint32_t bins_s, 
     const int next = c.nrows - nb;                // extension rows
     uint32_t ra = bins_s + gw * kRowBytes + lane * 4;
     if (next <= nb) {                             // every shape but tiny nb with wide boxes
-        for (int j = gw; j < nb; j += gnw, ra += gnw * kRowBytes) {
+        int j = gw;
+        for (; j + gnw < nb; j += 2 * gnw, ra += 2 * gnw * kRowBytes) {     // two rows in flight
+            const uint32_t rb = ra + gnw * kRowBytes;
+            const uint32_t qw0 = lds32(ra), qw1 = lds32(rb);
+            const int32_t qy0 = (int32_t)lds32(ra + 128), qy1 = (int32_t)lds32(rb + 128);
+            __syncwarp();
+            const uint64_t v0 = pack2((float)qw0 * c.cw, (float)qy0 * c.cy);
+            const uint64_t v1 = pack2((float)qw1 * c.cw, (float)qy1 * c.cy);
+            const uint32_t wa = ra + lane * 4, wb = rb + lane * 4;
+            sts64(wa, v0);
+            sts64(wb, v1);
+            if (j < next) sts64(wa + nb * kRowBytes, v0);
+            if (j + gnw < next) sts64(wb + nb * kRowBytes, v1);
+        }
+        for (; j < nb; j += gnw, ra += gnw * kRowBytes) {
             const uint32_t qw = lds32(ra);
             const int32_t qy = (int32_t)lds32(ra + 128);
             __syncwarp();
@@ -485,9 +512,11 @@ __device__ __forceinline__ void merge_column(const TileCtx &c, const float2 *row
     const int nb = c.nb, kmin = c.kmin, kmax = c.kmax;
     float bt = red_v[lane];
     uint32_t bkey = red_key[lane];
+#pragma unroll 4
     for (int w = 1; w < nparts; ++w) {
         const float v = red_v[w * 32 + lane];
-        if (v > bt) { bt = v; bkey = red_key[w * 32 + lane]; }
+        const uint32_t key = red_key[w * 32 + lane];
+        if (v > bt) { bt = v; bkey = key; }
     }
     const Column col{rows2 + lane, nb};
     float bv = bt * bt;
@@ -499,9 +528,14 @@ __device__ __forceinline__ void merge_column(const TileCtx &c, const float2 *row
     if (bt > 0.f) canonicalise(col, kmin, ba, bk);
     else { bk = kmin; ba = 0; }
     float r = 0.f, s = 0.f;
-    for (int j = 0; j < bk; ++j) {
-        int b = ba + j; if (b >= nb) b -= nb;
-        r += col.W(b); s += col.Y(b);
+    {   // bins in order (as the oracle sums them); rows nb .. repeat rows 0 .., so no wrap; loads 4 ahead
+        const float2 *pr = col.col + ba * 32;
+        int j = 0;
+        for (; j + 4 <= bk; j += 4, pr += 128) {
+            const float2 v0 = pr[0], v1 = pr[32], v2 = pr[64], v3 = pr[96];
+            r += v0.x; s += v0.y; r += v1.x; s += v1.y; r += v2.x; s += v2.y; r += v3.x; s += v3.y;
+        }
+        for (; j < bk; ++j, pr += 32) { r += pr[0].x; s += pr[0].y; }
     }
     const float den = fmaf(-r, r, r);
     float sr = 0.f, dp = 0.f;
