@@ -299,6 +299,7 @@ def main():
     # ---- roofline of the dominant kernel (search) -----------------------------------------------
     nk = kmax - kmin + 1
     n_mean = n_pts / n_curves
+    plan_kernel_name = "search_ws_kernel" if plan.query(B.QUERY_SEARCH_KERNEL) == 2 else "search_kernel"
     search_s = search_ns * 1e-9 / args.steps
     achieved = pf_per_step / search_s
     max_hz = (clocks.get("sm_max_mhz") or 1965) * 1e6
@@ -312,7 +313,7 @@ def main():
             traffic = json.load(open(tp)).get(args.config)
         except Exception:
             traffic = None
-    roofline = {"bound": "alu", "kernel": "search_kernel", "achieved": achieved, "peak": peak,
+    roofline = {"bound": "alu", "kernel": plan_kernel_name, "achieved": achieved, "peak": peak,
                 "unit": UNIT, "frac": achieved / peak, "traffic": traffic,
                 "peak_def": "n_SM*f_max*N/t_min per (curve,frequency) pair, t_min = max(LSU (2N+2(nb+kmax))/32, XU nb*nk/16, "
                             "issue (5N+4.5 nb nk)/128) clk = max(%.0f, %.0f, %.0f); rates measured by microbench/issue_rates.cu "
@@ -332,7 +333,10 @@ def main():
     if not args.no_cpu_baseline and world == 1:           # rank 0 at N = 1 only
         import oracle
         cores = oracle.host_cores()
-        n_s = min(n_curves, max(2 * cores, 16))
+        # bounded sample: a short probe sizes the sample to about 15 s of wall time on this box's cores
+        probe = list(range(min(n_curves, cores)))
+        _, cv_probe, _, _ = oracle_rate(cfg, batch, freqs, kmin, kmax, probe)
+        n_s = int(min(n_curves, max(len(probe), 15.0 * cv_probe)))
         curves = list(range(n_s))
         pf_s, cv_s, used, dt = oracle_rate(cfg, batch, freqs, kmin, kmax, curves)
         cpu = {"value": pf_s, "unit": UNIT, "cores": used, "kind": "oracle", "curves_per_sec": cv_s,

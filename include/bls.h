@@ -136,6 +136,8 @@ typedef struct {
 #define BLS_QUERY_SEARCH_CTAS 9     /* CTAs of the last search launch                              */
 #define BLS_QUERY_LAST_SEARCH_NS 10 /* device time (ns, CUDA events on the run's stream) the search
                                        kernel launches of the last bls_run took (synchronises)    */
+#define BLS_QUERY_SEARCH_KERNEL 11  /* search kernel the last bls_run used: 1 = single buffer,
+                                       2 = warp-specialised double buffer (0 = none yet)           */
 
 /* Validate cfg, copy the grid to the device, derive kmin/kmax and launch geometry.  *out_plan is
  * set only on success. */

@@ -44,6 +44,7 @@ struct bls_plan {
     int64_t last_launches = 0;
     int64_t last_search_ctas = 0;
     int last_tiles_per_item = 0;
+    int last_kernel = 0;
     cudaStream_t last_stream = nullptr;
     std::vector<cudaEvent_t> ev;    // event pairs bracketing each search launch of the last run
     size_t ev_used = 0;
@@ -204,6 +205,7 @@ int bls_plan_query(const bls_plan *p, int32_t what, int64_t *value)
         case BLS_QUERY_LAST_LAUNCHES: *value = p->last_launches; break;
         case BLS_QUERY_TILE_FREQS: *value = (int64_t)p->last_tiles_per_item * kTileFreqs; break;
         case BLS_QUERY_SEARCH_CTAS: *value = p->last_search_ctas; break;
+        case BLS_QUERY_SEARCH_KERNEL: *value = p->last_kernel; break;
         case BLS_QUERY_LAST_SEARCH_NS: {
             if (p->last_n_curves < 0) return BLS_ERR_ARG;
             if (cudaSetDevice(p->device) != cudaSuccess) return BLS_ERR_CUDA;
@@ -335,6 +337,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     int tiles_per_item = (int)((ntiles + items - 1) / items);
     items = (ntiles + tiles_per_item - 1) / tiles_per_item;
     p->last_tiles_per_item = tiles_per_item;
+    p->last_kernel = ws ? 2 : 1;
 
     SearchArgs a;
     a.pts = p->d_pts; a.offsets = p->d_offsets; a.meta = p->d_meta; a.freqs = p->d_freqs;

@@ -31,7 +31,7 @@ def check_config(name, curve_ids=None, flags=0, scratch_bytes=0):
                              g["sr"][c], g["a"][c], g["k"][c], g["depth"][c], label="%s curve %d" % (name, c))
         o_sr = r["oracle"][1]
         pk = g["peaks"][c]
-        pr = compare_peaks(o_sr, pk["freq_index"], pk["sr"], k, label="%s curve %d" % (name, c))
+        pr = compare_peaks(o_sr, pk["freq_index"], pk["sr"], k, label="%s curve %d" % (name, c), g_spectrum=g["sr"][c])
         # the peak records repeat the spectrum's values at their index
         for p in pk:
             if p["freq_index"] >= 0:
@@ -297,3 +297,79 @@ def test_bin_indices_equal_the_oracles_on_many_pairs():
         n_canon += nc
     print("\n[bins] %d (f,t) pairs, 0 mismatches, %d took the canonical rule" % (total, n_canon))
     assert n_canon > 0          # the edge cases must have exercised the guard band
+
+
+# ---- BASELINE.json configs[2..4] at full size: the launch configuration bench.py times (full
+#      frequency grid, the library's own geometry), on sampled curves / sampled outputs ------------
+
+def _first_injected(cfg, limit):
+    for cid in range(limit):
+        if synth.make_curve(cfg, cid)[4] is not None:
+            return cid
+    return None
+
+
+def check_peak_properties(g_sr, pk, k, label=""):
+    """Properties that hold at any size: peaks are local maxima of the spectrum they come from (R14),
+    ranked by SR then index, and no better local maximum was left out."""
+    idx = pk["freq_index"]
+    n = int((idx >= 0).sum())
+    assert np.all(idx[n:] == -1)
+    v = g_sr
+    nf = len(v)
+    is_pk = (v > 0) & np.concatenate(([True], v[1:] > v[:-1])) & np.concatenate((v[:-1] >= v[1:], [True]))
+    assert is_pk[idx[:n]].all(), label + " a reported peak is not a local maximum"
+    srs = v[idx[:n]]
+    assert np.array_equal(srs, pk["sr"][:n])
+    order = np.lexsort((idx[:n], -srs))
+    assert np.array_equal(order, np.arange(n)), label + " peaks not ranked"
+    rest = is_pk.copy()
+    rest[idx[:n]] = False
+    if n == k and rest.any():
+        assert v[rest].max() <= srs[-1], label + " a better local maximum was left out"
+    else:
+        assert n == min(k, int(is_pk.sum()))
+
+
+def test_c2_shape_ragged_lengths_all_frequencies():
+    """configs[2]: N in 500..4000, 50,000 frequencies, 200 bins, widths 1..30, top-5; three curves
+    (one of them injected) against the oracle at every frequency."""
+    cfg = synth.config("C2")
+    inj = _first_injected(cfg, 600)
+    ids = [0, 1] + ([inj] if inj is not None else [2])
+    g, rep = check_config("C2", curve_ids=ids)
+    if inj is not None:
+        tr = synth.make_curve(cfg, inj)[4]
+        top = g["peaks"][2][0]
+        ratio = top["freq"] * tr["P"]
+        if tr["depth"] > 0.05:      # a deep eclipse: the top peak is the period or a harmonic of it
+            assert min(abs(ratio * m - round(ratio * m)) for m in (1, 2, 3, 4)) < 0.02
+
+
+def test_c3_shape_full_grid_sampled_frequencies():
+    """configs[3]: 5,000 epochs over two seasons, 500,000 frequencies, 400 bins, widths 1..40.  The
+    CUDA path runs the full grid (its launch configuration); the oracle scores every 193rd
+    frequency, element by element; the peak list is checked by its properties."""
+    cfg = synth.config("C3")
+    grid = cfg["grid"]
+    batch = synth.make_batch(cfg, [3])
+    g = run_gpu(batch, grid, top_k=cfg["top_k"])
+    assert (g["kmin"], g["kmax"]) == oracle.widths(grid.nb, grid.qmin, grid.qmax) == (1, 40)
+    assert g["status"][0] == 0
+    idx = np.arange(7, grid.nf, 193)
+    t, mag, sig = batch.curve(0)
+    r = compare_spectrum(t, mag, sig, g["freqs"][idx], grid.nb, g["kmin"], g["kmax"], g["sr"][0][idx],
+                         g["a"][0][idx], g["k"][0][idx], g["depth"][0][idx], label="C3 curve 3")
+    print("\n[parity C3] %d sampled frequencies of %d: max SR rel err %.3g, box near-ties %d" % (
+        len(idx), grid.nf, r["max_rel_err"], r["box_near_ties"]))
+    check_peak_properties(g["sr"][0], g["peaks"][0], cfg["top_k"], "C3")
+    assert np.isfinite(g["sr"]).all() and (g["sr"] >= 0).all()
+    assert (g["a"] < grid.nb).all() and (g["k"] >= 1).all() and (g["k"] <= 40).all()
+
+
+def test_c4_shape_many_short_curves():
+    """configs[4]: 200 epochs, 5,000 frequencies, 64 bins, widths 1..10; 96 curves at every frequency."""
+    cfg = synth.config("C4")
+    inj = _first_injected(cfg, 400)
+    ids = list(range(95)) + [inj if inj is not None else 95]
+    check_config("C4", curve_ids=ids)
