@@ -299,7 +299,7 @@ def main():
     # ---- roofline of the dominant kernel (search) -----------------------------------------------
     nk = kmax - kmin + 1
     n_mean = n_pts / n_curves
-    plan_kernel_name = "search_ws_kernel" if plan.query(B.QUERY_SEARCH_KERNEL) == 2 else "search_kernel"
+    plan_kernel_name = {1: "search_kernel", 2: "search_ws_kernel", 3: "search_wt_kernel"}.get(plan.query(B.QUERY_SEARCH_KERNEL), "?")
     search_s = search_ns * 1e-9 / args.steps
     achieved = pf_per_step / search_s
     max_hz = (clocks.get("sm_max_mhz") or 1965) * 1e6

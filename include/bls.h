@@ -81,6 +81,8 @@ typedef struct {
 #define BLS_FLAG_SINGLE_BUFFER 2u    /* tuning: always use the single-buffer search kernel (every warp
                                        does every phase) instead of the warp-specialised, double-
                                        buffered one.  Never changes results.                       */
+#define BLS_FLAG_NO_WARP_PER_TILE 4u /* tuning: never use the one-warp-per-tile search kernel that small
+                                       shapes get by default.  Never changes results.               */
 #define BLS_FLAG_WARPS(n) (((uint32_t)(n) & 0xffu) << 8) /* tuning: warps per CTA that walk the boxes
                                        (1..10; 0 = the library's choice).  Never changes results. */
 #define BLS_FLAG_FOLD_WARPS(n) (((uint32_t)(n) & 0xffu) << 16) /* tuning: warps per CTA that fold, in
@@ -137,7 +139,8 @@ typedef struct {
 #define BLS_QUERY_LAST_SEARCH_NS 10 /* device time (ns, CUDA events on the run's stream) the search
                                        kernel launches of the last bls_run took (synchronises)    */
 #define BLS_QUERY_SEARCH_KERNEL 11  /* search kernel the last bls_run used: 1 = single buffer,
-                                       2 = warp-specialised double buffer (0 = none yet)           */
+                                       2 = warp-specialised double buffer, 3 = one warp per tile
+                                       (0 = none yet)                                              */
 
 /* Validate cfg, copy the grid to the device, derive kmin/kmax and launch geometry.  *out_plan is
  * set only on success. */

@@ -325,11 +325,22 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
         pts_in_smem = 0;
         smem = search_smem_bytes(p->nb, p->kmax, warps, buffers, 0);
     }
-    const int threads = (ws ? warps + fold_warps : warps) * 32;
+    int threads = (ws ? warps + fold_warps : warps) * 32;
+    int kernel = ws ? 2 : 1;
+    // Kernel 3 (one warp per tile, warp-private bins) for small shapes: when two CTAs of kWtWarps
+    // warps, each with the curve staged, fit an SM.  There a tile is too little work to pay for the
+    // hand-offs of kernels 1 and 2 (C4: 200 epochs, 64 bins).
+    const size_t wt_smem = (size_t)kWtWarps * ((size_t)search_rows(p->nb, p->kmax) * kTileFreqs * 8 + 256) +
+                           (size_t)max_n * sizeof(PointRec);
+    const bool wt_fits = 2 * (wt_smem + 1024) <= (size_t)228 * 1024;
+    if (!(p->flags & (BLS_FLAG_SINGLE_BUFFER | BLS_FLAG_NO_WARP_PER_TILE)) && wt_fits) {
+        kernel = 3; smem = wt_smem; pts_in_smem = 1; threads = kWtWarps * 32;
+    }
     int ctas_per_sm = (int)((size_t)(228 * 1024) / (smem + 1024));
     if (ctas_per_sm < 1) ctas_per_sm = 1;
-    if (ctas_per_sm > (ws ? 1 : 2)) ctas_per_sm = ws ? 1 : 2;      // register-limited (launch bounds)
-    const int waves = ws ? 24 : 12;                                 // enough waves to hide the tail
+    const int max_ctas = kernel == 2 ? 1 : 2;                       // register-limited (launch bounds)
+    if (ctas_per_sm > max_ctas) ctas_per_sm = max_ctas;
+    const int waves = kernel == 1 ? 12 : 24;                        // enough waves to hide the tail
     const int64_t target_ctas = (int64_t)p->sm_count * ctas_per_sm * waves;
     int64_t items = (target_ctas + chunk - 1) / chunk;
     if (items < 1) items = 1;
@@ -337,7 +348,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     int tiles_per_item = (int)((ntiles + items - 1) / items);
     items = (ntiles + tiles_per_item - 1) / tiles_per_item;
     p->last_tiles_per_item = tiles_per_item;
-    p->last_kernel = ws ? 2 : 1;
+    p->last_kernel = kernel;
 
     SearchArgs a;
     a.pts = p->d_pts; a.offsets = p->d_offsets; a.meta = p->d_meta; a.freqs = p->d_freqs;
@@ -345,7 +356,8 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     a.tiles_per_item = tiles_per_item; a.items_per_curve = (int)items;
     a.pts_in_smem = pts_in_smem;
     a.starts_per_thread = starts;
-    a.search_warps = ws ? warps : 0;
+    a.search_warps = kernel == 2 ? warps : 0;
+    a.kernel = kernel;
     a.threads = threads;
     a.force_canonical = (p->flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0;
     a.sr = p->d_sr; a.ak = p->d_ak; a.depth = p->d_depth;

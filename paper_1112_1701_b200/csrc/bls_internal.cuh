@@ -38,6 +38,7 @@ constexpr int kTileFreqs = 32;        // frequencies per tile = lanes of a warp
 constexpr int kSearchThreads = 256;   // default: 8 warps per CTA
 constexpr int kMaxSearchWarps = 10;   // upper bound (BLS_FLAG_WARPS override); 2 CTAs x 10 warps x 96 registers fill an SM
 constexpr int kWsMaxWarps = 20;       // warp-specialised kernel: search warps + fold warps
+constexpr int kWtWarps = 5;           // warp-per-tile kernel: warps per CTA (two CTAs per SM)
 constexpr int kPrepThreads = 256;
 constexpr int kPeakThreads = 256;
 constexpr int kStartsPerThread = 4;   // register tile of the box search (A)
@@ -53,7 +54,8 @@ struct SearchArgs {
     int threads;                // CTA size of the search kernel (multiple of 32, <= 32*kMaxSearchWarps)
     int pts_in_smem;            // 1: stage the curve in shared memory, 0: read it through L1
     int starts_per_thread;      // S of the box search (4 or 5)
-    int search_warps;           // > 0: warp-specialised kernel with this many search warps (the rest fold)
+    int search_warps;           // kernel 2: this many search warps (the rest fold)
+    int kernel;                 // 1 single buffer, 2 warp-specialised double buffer, 3 one warp per tile
     int force_canonical;        // BLS_FLAG_CANONICAL_PHASE
     float *sr;                  // chunk scratch, [chunk_curves][nf]
     uint32_t *ak;

@@ -763,6 +763,76 @@ search_ws_kernel(const SearchArgs a)
     }
 }
 
+// ---- kernel 3: one warp per tile.  For small shapes (C4: 200 epochs, 64 bins) a tile is a few
+//      thousand instructions and the hand-offs of kernels 1/2 cost more than the work.  Here every
+//      warp owns private bins and runs zero / fold / convert / search / merge of its own tiles with
+//      warp syncs only; warps of an SM sit in different phases, so the LSU-bound fold of one overlaps
+//      the XU-bound search of another without any CTA-level barrier. ------------------------------
+template <bool PTS_SMEM, int S>
+__global__ void __launch_bounds__(kWtWarps * 32, 2)
+search_wt_kernel(const SearchArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nthr = blockDim.x, nw = nthr >> 5;
+    TileCtx c;
+    c.nb = a.nb; c.kmin = a.kmin; c.kmax = a.kmax;
+    c.nrows = search_rows(a.nb, a.kmax);
+    // smem: per warp { bins [nrows][256 B] | red_v [32] | red_key [32] } ... | points [n]
+    const size_t per_warp = (size_t)c.nrows * kRowBytes + 256;
+    unsigned char *mine = smem_raw + warp * per_warp;
+    float *red_v = reinterpret_cast<float *>(mine + (size_t)c.nrows * kRowBytes);
+    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + 32);
+    PointRec *pts_s = reinterpret_cast<PointRec *>(smem_raw + nw * per_warp);
+
+    const int64_t curve_local = blockIdx.x / a.items_per_curve;
+    const int item = blockIdx.x % a.items_per_curve;
+    const int64_t cv = a.curve_base + curve_local;
+    const int64_t beg = a.offsets[cv];
+    c.n = (int)(a.offsets[cv + 1] - beg);
+    const CurveMeta meta = a.meta[cv];
+    const int ntiles = (a.nf + kTileFreqs - 1) / kTileFreqs;
+    const int tile0 = item * a.tiles_per_item;
+    const int tile1 = min(tile0 + a.tiles_per_item, ntiles);
+    const OutPtrs out = out_rows(a, curve_local, cv);
+
+    if (meta.status != BLS_CURVE_OK) {
+        zero_fill_outputs(out, tile0 * kTileFreqs, min(tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
+        return;
+    }
+    const PointRec *pts_g = a.pts + beg;
+    if (PTS_SMEM) {
+        const uint4 *src = reinterpret_cast<const uint4 *>(pts_g);
+        uint4 *dst = reinterpret_cast<uint4 *>(pts_s);
+        for (int i = tid; i < c.n; i += nthr) dst[i] = __ldg(src + i);
+    }
+    __syncthreads();                              // the only CTA barrier
+    const uint32_t buf = smem_u32(mine), pts_sa = smem_u32(pts_s);
+    c.force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
+    c.cw = meta.cw; c.cy = meta.cy; c.wx2 = (float)meta.wx2;
+    c.G = (uint32_t)a.nb + 8u;
+    unsigned int n_canon = 0;
+
+    for (int tile = tile0 + warp; tile < tile1; tile += nw) {
+        const int q0 = tile * kTileFreqs;
+        const double f = a.freqs[min(q0 + lane, a.nf - 1)];
+        zero_bins(buf, c.nb, lane, 32);
+        __syncwarp();
+        fold_tile<PTS_SMEM>(c, f, buf, pts_sa, pts_g, lane, 0, 1, n_canon);
+        __syncwarp();
+        convert_rows(c, buf, lane, 0, 1);
+        __syncwarp();
+        float t_best; uint32_t key_best;
+        search_column<S>(buf + lane * 8, c.nb, c.kmin, c.kmax, 0, 1, t_best, key_best);
+        red_v[lane] = t_best;
+        red_key[lane] = key_best;
+        __syncwarp();
+        merge_column(c, reinterpret_cast<const float2 *>(mine), red_v, red_key, 1, lane, q0 + lane, a.nf, out);
+        __syncwarp();
+    }
+    count_canonical(a, n_canon, lane);
+}
+
 // Diagnostic: the bin index the fold assigns to each (f, t) pair -- the same fold_bin() the search
 // kernel inlines.  Lets tests compare bin indices with the oracle on very many pairs.
 __global__ void debug_bins_kernel(const double *__restrict__ f, const double *__restrict__ t, int64_t n,
@@ -791,7 +861,9 @@ cudaError_t search_configure(int max_smem_optin)
     const void *fns[] = {(const void *)search_kernel<true, 4>,    (const void *)search_kernel<false, 4>,
                          (const void *)search_kernel<true, 5>,    (const void *)search_kernel<false, 5>,
                          (const void *)search_ws_kernel<true, 4>, (const void *)search_ws_kernel<false, 4>,
-                         (const void *)search_ws_kernel<true, 5>, (const void *)search_ws_kernel<false, 5>};
+                         (const void *)search_ws_kernel<true, 5>, (const void *)search_ws_kernel<false, 5>,
+                         (const void *)search_wt_kernel<true, 4>, (const void *)search_wt_kernel<false, 4>,
+                         (const void *)search_wt_kernel<true, 5>, (const void *)search_wt_kernel<false, 5>};
     for (const void *f : fns) {
         cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
         if (e != cudaSuccess) return e;
@@ -815,7 +887,8 @@ cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem
             else K<false, 4><<<g, a.threads, smem, st>>>(a);                            \
         }                                                                               \
     } while (0)
-    if (a.search_warps > 0) BLS_LAUNCH(search_ws_kernel);
+    if (a.kernel == 3) BLS_LAUNCH(search_wt_kernel);
+    else if (a.kernel == 2) BLS_LAUNCH(search_ws_kernel);
     else BLS_LAUNCH(search_kernel);
 #undef BLS_LAUNCH
     return cudaGetLastError();

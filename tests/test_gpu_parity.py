@@ -67,6 +67,14 @@ def test_small_configs_single_buffer_kernel(name):
     check_config(name, flags=bls.BLS_FLAG_SINGLE_BUFFER)
 
 
+@pytest.mark.parametrize("name", ["T1", "C4"])
+def test_small_shapes_without_the_warp_per_tile_kernel(name):
+    """nb = 64 shapes default to the one-warp-per-tile kernel; the same cases through the
+    warp-specialised kernel."""
+    import paper_1112_1701_b200 as bls
+    check_config(name, curve_ids=None if name == "T1" else list(range(8)), flags=bls.BLS_FLAG_NO_WARP_PER_TILE)
+
+
 def test_kernel_variants_give_identical_results():
     """Warp counts and kernel choice are tuning only.  Bins are exact integers and every box is scored by
     the same instructions, so spectra agree to rounding; they are not bitwise equal because boxes whose
@@ -75,8 +83,10 @@ def test_kernel_variants_give_identical_results():
     cfg = synth.config("T1")
     batch = synth.make_batch(cfg)
     ref = run_gpu(batch, cfg["grid"], top_k=5)
-    for flags in (bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_WARPS(6) | bls.BLS_FLAG_FOLD_WARPS(3),
-                  bls.BLS_FLAG_WARPS(7) | bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_WARPS(10) | bls.BLS_FLAG_FOLD_WARPS(1)):
+    for flags in (bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_NO_WARP_PER_TILE,
+                  bls.BLS_FLAG_NO_WARP_PER_TILE | bls.BLS_FLAG_WARPS(6) | bls.BLS_FLAG_FOLD_WARPS(3),
+                  bls.BLS_FLAG_WARPS(7) | bls.BLS_FLAG_SINGLE_BUFFER,
+                  bls.BLS_FLAG_NO_WARP_PER_TILE | bls.BLS_FLAG_WARPS(10) | bls.BLS_FLAG_FOLD_WARPS(1)):
         g = run_gpu(batch, cfg["grid"], top_k=5, flags=flags)
         np.testing.assert_allclose(g["sr"], ref["sr"], rtol=2e-6, atol=0)
         same = (g["a"] == ref["a"]) & (g["k"] == ref["k"])
