@@ -398,7 +398,7 @@ __device__ __forceinline__ void fold_groups(const TileCtx &c, double f, uint32_t
 // frequency f.  During the fold row b holds int32 planes W[b][lane] | Y[b][lane]: lane l always
 // hits bank l (and Y sits 128 B after W, one address register), so the native ATOMS.ADD is
 // conflict-free by construction.  Four points in flight hide the LDS / DFMA latency.
-template <bool PTS_SMEM>
+template <bool PTS_SMEM, int NG = 1>
 __device__ __forceinline__ void fold_tile(const TileCtx &c, double f, uint32_t bins_s, uint32_t pts_sa,
                                           const PointRec *pts_g, int lane, int gw, int gnw, unsigned int &n_canon)
 {
@@ -410,6 +410,8 @@ __device__ __forceinline__ void fold_tile(const TileCtx &c, double f, uint32_t b
     if (PTS_SMEM) {
         const uint32_t pa_end = pts_sa + ngroups * 64, step = gnw * 64;
         uint32_t pa = pts_sa + gw * 64;
+        if (NG == 2)
+            for (; pa + step < pa_end; pa += 2 * step) fold_groups<2>(c, f, colw, pa, step, n_canon);
         for (; pa < pa_end; pa += step) fold_groups<1>(c, f, colw, pa, step, n_canon);
     } else {
         for (int g = gw; g < ngroups; g += gnw) {
@@ -818,7 +820,7 @@ search_wt_kernel(const SearchArgs a)
         const double f = a.freqs[min(q0 + lane, a.nf - 1)];
         zero_bins(buf, c.nb, lane, 32);
         __syncwarp();
-        fold_tile<PTS_SMEM>(c, f, buf, pts_sa, pts_g, lane, 0, 1, n_canon);
+        fold_tile<PTS_SMEM, 2>(c, f, buf, pts_sa, pts_g, lane, 0, 1, n_canon);
         __syncwarp();
         convert_rows(c, buf, lane, 0, 1);
         __syncwarp();
