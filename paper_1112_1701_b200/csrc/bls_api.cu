@@ -16,6 +16,7 @@ struct bls_plan {
     int device = 0;
     int sm_count = 0;
     int max_smem_optin = 0;
+    int max_smem_sm = 0;
     int64_t nf = 0;
     int nb = 0, kmin = 0, kmax = 0, max_top_k = 0;
     uint32_t flags = 0;
@@ -160,6 +161,7 @@ int bls_plan_create(const bls_config *cfg, bls_plan **out_plan)
     cudaError_t e = cudaSetDevice(p->device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&p->max_smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, p->device);
     if (e == cudaSuccess) e = search_configure(p->max_smem_optin);
     if (e == cudaSuccess) e = cudaMalloc(&p->d_freqs, (size_t)p->nf * sizeof(double));
     if (e == cudaSuccess) e = cudaMemcpy(p->d_freqs, grid.data(), (size_t)p->nf * sizeof(double), cudaMemcpyHostToDevice);
@@ -305,19 +307,21 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
 
     // ---- launch geometry of the search ---------------------------------------------------------
     const int ntiles = (int)((p->nf + kTileFreqs - 1) / kTileFreqs);
+    const size_t optin = (size_t)p->max_smem_optin;
+    const size_t sm_smem = (size_t)p->max_smem_sm;
+    const int warps_flag = (int)((p->flags >> 8) & 0xffu);
+    const int fold_flag = (int)((p->flags >> 16) & 0xffu);
     // Kernel 2 (warp-specialised, two bin buffers) whenever its buffers fit shared memory, with the
     // curve staged in shared memory if that fits too; otherwise kernel 1 (one buffer, two CTAs per SM).
-    const size_t optin = (size_t)p->max_smem_optin;
+    int ws_search = kWsSearchWarps;
+    if (warps_flag >= 1 && warps_flag <= kWsMaxWarps - 1) ws_search = warps_flag;
+    int ws_fold = kWsMaxWarps - ws_search;
+    if (fold_flag >= 1 && fold_flag < ws_fold) ws_fold = fold_flag;
     const bool ws = !(p->flags & BLS_FLAG_SINGLE_BUFFER) &&
-                    search_smem_bytes(p->nb, p->kmax, kMaxSearchWarps, 2, 0) <= optin;
-    int starts = 4, warps = 8;
-    // kernel 2 runs 8 box-search warps beside 12 fold warps (measured best at C1: the fold side is
-    // latency bound and wants the warps); kernel 1 uses up to 10 warps for everything
-    search_geometry(p->nb, ws ? 8 : kMaxSearchWarps, &starts, &warps);
-    const int warps_flag = (int)((p->flags >> 8) & 0xffu);
-    if (warps_flag >= 1 && warps_flag <= kMaxSearchWarps) warps = warps_flag;
-    int fold_warps = (int)((p->flags >> 16) & 0xffu);
-    if (fold_warps < 1 || warps + fold_warps > kWsMaxWarps) fold_warps = kWsMaxWarps - warps;
+                    search_smem_bytes(p->nb, p->kmax, ws_search, 2, 0) <= optin;
+    int k1_warps = kMaxSearchWarps;
+    if (warps_flag >= 1 && warps_flag <= kMaxSearchWarps) k1_warps = warps_flag;
+    const int warps = ws ? ws_search : k1_warps;            // warps that walk the boxes
     const int buffers = ws ? 2 : 1;
     int pts_in_smem = 1;
     size_t smem = search_smem_bytes(p->nb, p->kmax, warps, buffers, max_n);
@@ -325,18 +329,20 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
         pts_in_smem = 0;
         smem = search_smem_bytes(p->nb, p->kmax, warps, buffers, 0);
     }
-    int threads = (ws ? warps + fold_warps : warps) * 32;
+    if (smem > optin) return BLS_ERR_UNSUPPORTED;
+    int threads = (ws ? ws_search + ws_fold : k1_warps) * 32;
     int kernel = ws ? 2 : 1;
+    int nrows = search_rows_for(p->nb, p->kmax, 2 * warps);
     // Kernel 3 (one warp per tile, warp-private bins) for small shapes: when two CTAs of kWtWarps
     // warps, each with the curve staged, fit an SM.  There a tile is too little work to pay for the
     // hand-offs of kernels 1 and 2 (C4: 200 epochs, 64 bins).
-    const size_t wt_smem = (size_t)kWtWarps * ((size_t)search_rows(p->nb, p->kmax) * kTileFreqs * 8 + 256) +
-                           (size_t)max_n * sizeof(PointRec);
-    const bool wt_fits = 2 * (wt_smem + 1024) <= (size_t)228 * 1024;
+    const int wt_rows = search_rows_for(p->nb, p->kmax, 2);
+    const size_t wt_smem = (size_t)kWtWarps * ((size_t)wt_rows * kTileFreqs * 8 + 256) + (size_t)max_n * sizeof(PointRec);
+    const bool wt_fits = 2 * (wt_smem + 1024) <= sm_smem;
     if (!(p->flags & (BLS_FLAG_SINGLE_BUFFER | BLS_FLAG_NO_WARP_PER_TILE)) && wt_fits) {
-        kernel = 3; smem = wt_smem; pts_in_smem = 1; threads = kWtWarps * 32;
+        kernel = 3; smem = wt_smem; pts_in_smem = 1; threads = kWtWarps * 32; nrows = wt_rows;
     }
-    int ctas_per_sm = (int)((size_t)(228 * 1024) / (smem + 1024));
+    int ctas_per_sm = (int)(sm_smem / (smem + 1024));
     if (ctas_per_sm < 1) ctas_per_sm = 1;
     const int max_ctas = kernel == 2 ? 1 : 2;                       // register-limited (launch bounds)
     if (ctas_per_sm > max_ctas) ctas_per_sm = max_ctas;
@@ -355,8 +361,8 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     a.nf = (int)p->nf; a.nb = p->nb; a.kmin = p->kmin; a.kmax = p->kmax;
     a.tiles_per_item = tiles_per_item; a.items_per_curve = (int)items;
     a.pts_in_smem = pts_in_smem;
-    a.starts_per_thread = starts;
-    a.search_warps = kernel == 2 ? warps : 0;
+    a.nrows = nrows;
+    a.search_warps = kernel == 2 ? ws_search : 0;
     a.kernel = kernel;
     a.threads = threads;
     a.force_canonical = (p->flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0;
@@ -366,6 +372,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     a.u_width = out ? out->best_width : nullptr;
     a.u_depth = out ? out->depth : nullptr;
     a.canon_count = p->d_canon;
+    a.debug = (int)(p->flags >> 24);
 
     // ---- per chunk of curves: search -> peak candidates ------------------------------------------
     p->last_search_ctas = 0;
@@ -400,7 +407,9 @@ int bls_debug_fold_bins(int32_t device, const double *f, const double *t, int64_
     unsigned long long *d_cnt = nullptr, h_cnt = 0;
     if (cudaMalloc(&d_cnt, sizeof(h_cnt)) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
     cudaError_t e = cudaMemset(d_cnt, 0, sizeof(h_cnt));
-    if (e == cudaSuccess) e = launch_debug_bins(f, t, n, n_bins, (flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0, bins, d_cnt, nullptr);
+    int sm_count = 1;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess) e = launch_debug_bins(f, t, n, n_bins, (flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0, bins, d_cnt, sm_count, nullptr);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e == cudaSuccess) e = cudaMemcpy(&h_cnt, d_cnt, sizeof(h_cnt), cudaMemcpyDeviceToHost);
     cudaFree(d_cnt);

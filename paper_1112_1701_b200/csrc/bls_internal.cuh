@@ -16,13 +16,18 @@ struct __align__(16) PointRec {
     int32_t qy;    // rint(w_i * x_i * SY)      fixed-point weighted residual
 };
 
-// Per-curve constants written by the prep kernel.
+// Per-curve constants written by the prep kernel.  The bins hold exact integer sums of qw / qy;
+// with SWT = sum_i qw_i (exact) a box of integer sums (R, S) has r = R/SWT, 1-r = (SWT-R)/SWT and
+//   SR = S^2/(R (SWT-R)) * sr_scale ,  depth = S/(R (SWT-R)) * dp_scale
 struct CurveMeta {
-    float cw;          // 1/SW : bin integer -> weight fraction r
+    float ncw;         // -1/SWT : the box search accumulates n = -r (one FFMA2 per box pair)
     float cy;          // 1/SY : bin integer -> weighted residual s (0 for a constant curve)
     int32_t status;    // BLS_CURVE_*
-    int32_t force_canonical;  // 1: |f t| may reach 2^19 cycles, the fast phase is not valid
-    double tabs_max;   // max |t|
+    int32_t force_canonical;  // 1: |f t| may reach 2^18 cycles, the fast phase is not valid
+    uint32_t swt;      // sum_i qw_i (exact; < 2^32)
+    uint32_t pad_;
+    double sr_scale;   // SWT^2 / SY^2   (0 for a constant curve)
+    double dp_scale;   // SWT^2 / SY
     double wx2;        // sum_i w_i x_i^2  (upper bound of SR)
 };
 
@@ -35,13 +40,13 @@ struct PeakCand {
 };
 
 constexpr int kTileFreqs = 32;        // frequencies per tile = lanes of a warp
-constexpr int kSearchThreads = 256;   // default: 8 warps per CTA
-constexpr int kMaxSearchWarps = 10;   // upper bound (BLS_FLAG_WARPS override); 2 CTAs x 10 warps x 96 registers fill an SM
+constexpr int kMaxSearchWarps = 10;   // kernel 1 upper bound (BLS_FLAG_WARPS override); 2 CTAs x 10 warps x 96 registers fill an SM
 constexpr int kWsMaxWarps = 20;       // warp-specialised kernel: search warps + fold warps
+constexpr int kWsSearchWarps = 8;     // its default split: 8 search (two per SM sub-partition) + 12 fold; 20 warps = 5 per sub-partition leave 96 registers per thread
+constexpr int kMergeWarps = 8;        // warps of a group that share the exact merge of a tile (one start each, S <= 8)
 constexpr int kWtWarps = 5;           // warp-per-tile kernel: warps per CTA (two CTAs per SM)
 constexpr int kPrepThreads = 256;
 constexpr int kPeakThreads = 256;
-constexpr int kStartsPerThread = 4;   // register tile of the box search (A)
 
 struct SearchArgs {
     const PointRec *pts;        // [n_points] prepared points of the whole batch
@@ -53,10 +58,11 @@ struct SearchArgs {
     int64_t curve_base;         // first curve of this chunk
     int threads;                // CTA size of the search kernel (multiple of 32, <= 32*kMaxSearchWarps)
     int pts_in_smem;            // 1: stage the curve in shared memory, 0: read it through L1
-    int starts_per_thread;      // S of the box search (4 or 5)
-    int search_warps;           // kernel 2: this many search warps (the rest fold)
+    int nrows;                  // bin rows per buffer: nb + cyclic extension (search_rows_for)
+    int search_warps;           // kernel 2: this many search warps (then the fold warps)
     int kernel;                 // 1 single buffer, 2 warp-specialised double buffer, 3 one warp per tile
     int force_canonical;        // BLS_FLAG_CANONICAL_PHASE
+    int debug;                  // DEV ONLY
     float *sr;                  // chunk scratch, [chunk_curves][nf]
     uint32_t *ak;
     float *depth;
@@ -108,13 +114,12 @@ __device__ __forceinline__ int fold_bin(double f, double t, int nb, uint32_t G, 
 }
 #endif
 
-// Bin rows a search CTA holds: the nb bins plus the cyclic extension the widest box of the last
-// start tile reaches (kmax rounded up to whole width blocks, plus the window's slack).
-__host__ __device__ inline int search_rows(int nb, int kmax) { return nb + ((kmax + 3) & ~3) + 4; }
+// Bin rows a search buffer holds when the start bins are dealt to `slots` half-warps: the nb bins
+// plus the cyclic extension the widest box of the last start reaches (bls_search.cu).
+int search_rows_for(int nb, int kmax, int slots);
 size_t search_smem_bytes(int nb, int kmax, int warps, int buffers, int64_t n_points_in_smem);
-void search_geometry(int nb, int max_warps, int *starts_per_thread, int *warps);
 cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int nb, int force_canon,
-                              int32_t *bins, unsigned long long *n_canon, cudaStream_t st);
+                              int32_t *bins, unsigned long long *n_canon, int sm_count, cudaStream_t st);
 cudaError_t search_configure(int max_smem_optin);
 cudaError_t launch_prep(const float *t, const float *mag, const float *sigma, const int64_t *offsets,
                         int64_t n_curves, double fmax, PointRec *pts, CurveMeta *meta, int32_t *u_status,

@@ -78,8 +78,8 @@ prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const fl
             pts[i] = r;
         }
         if (threadIdx.x == 0) {
-            CurveMeta m; m.cw = 0.f; m.cy = 0.f; m.status = status; m.force_canonical = 0;
-            m.tabs_max = 0.0; m.wx2 = 0.0;
+            CurveMeta m; m.ncw = 0.f; m.cy = 0.f; m.status = status; m.force_canonical = 0;
+            m.swt = 0u; m.pad_ = 0u; m.sr_scale = 0.0; m.dp_scale = 0.0; m.wx2 = 0.0;
             meta[c] = m;
             if (u_status) u_status[c] = status;
         }
@@ -109,6 +109,7 @@ prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const fl
     const double SY = (sigw > 0.0 && isfinite(sigw))
                           ? (2147483648.0 - (double)n - 2.0) / (0.5 * sigw * (1.0 + 1e-12)) : 0.0;
 
+    double qsum = 0.0;                                  // integers < 2^32: exact in fp64, any order
     for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
         double s = (double)sigma[i];
         double w = (1.0 / (s * s)) / sw;
@@ -117,16 +118,21 @@ prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const fl
         r.t = (double)t[i];
         r.qw = (uint32_t)__double2ll_rn(w * SW);
         r.qy = (int32_t)__double2ll_rn(w * x * SY);
+        qsum += (double)r.qw;
         pts[i] = r;
     }
+    const double swt = block_sum(qsum, sh);             // SWT = sum_i qw_i <= SW + N/2 < 2^32
     if (threadIdx.x == 0) {
         CurveMeta m;
-        m.cw = (float)(1.0 / SW);
+        m.ncw = (float)(-1.0 / swt);
         m.cy = SY > 0.0 ? (float)(1.0 / SY) : 0.f;
         m.status = BLS_CURVE_OK;
-        // the fast phase needs |f t| < 2^19 cycles
+        // the fast phase needs |f t| < 2^18 cycles
         m.force_canonical = (fmax_grid * tmax < 262144.0) ? 0 : 1;
-        m.tabs_max = tmax;
+        m.swt = (uint32_t)swt;
+        m.pad_ = 0u;
+        m.sr_scale = SY > 0.0 ? (swt / SY) * (swt / SY) : 0.0;
+        m.dp_scale = SY > 0.0 ? swt * (swt / SY) : 0.0;
         m.wx2 = wx2;
         meta[c] = m;
         if (u_status) u_status[c] = BLS_CURVE_OK;

@@ -1,58 +1,55 @@
 // a1 Load, a2 Fold, a3/a4 box search, per-frequency argmax (DESIGN.md
-// "Kernels / search").  PAPER.md L145: "the light curve data is read into fast shared memory by each
+// section 6.3).  PAPER.md L145: "the light curve data is read into fast shared memory by each
 // thread block (with memory accesses coalesced for speed), then each thread picks an untested
 // period, phases the light curve at that period and then tests a range of durations and phases."
 //
 // What is kept from that design: the curve is resident in shared memory across a block of trial
-// frequencies, and a LANE owns a trial frequency.  What differs (Fermi -> sm_100a):
-//   * a CTA owns one curve and a tile of 32 consecutive frequencies at a time; ALL its warps fold
-//     the curve into the tile's bins (each warp takes every NW-th point, every lane its own
-//     frequency), so the bins of a frequency are private to a lane column: bins[bin][lane] puts
-//     lane l in bank l -> the native 32-bit ATOMS.ADD is conflict-free by construction;
-//   * bins accumulate int32 fixed point (exact, order independent, bitwise reproducible);
+// frequencies, and a LANE owns a trial frequency while folding.  What differs (Fermi -> sm_100a):
+//   * a CTA owns one curve and a tile of 32 consecutive frequencies at a time; the fold warps fold
+//     the curve into the tile's bins (each warp takes every NW-th group of points, every lane its
+//     own frequency): bins[bin][{W,Y}][lane] puts lane l in bank l -> the native 32-bit ATOMS.ADD
+//     is conflict-free by construction;
+//   * bins are int32 fixed point and STAY integers for the whole life of a tile: sums are exact,
+//     order independent and bitwise reproducible, and the statistic reported for a box is a
+//     function of the box's point set alone (exact plateaus between adjacent frequencies);
 //   * the phase is one DFMA with a magic constant whose low mantissa word is frac(f t) * 2^32;
 //     one IMAD.WIDE gives (bin, position inside the bin); positions inside a guard band of a bin
 //     edge fall back to the canonical 3-rounding fp64 rule, so bin indices equal the oracle's
 //     bit for bit (DESIGN.md "Fold / fast phase" has the error bound);
-//   * the box search is register tiled: a thread owns 4 consecutive start bins of its lane's
-//     frequency and slides an 8-row window over the bins, so one shared load feeds 4 boxes; sums
-//     are direct running sums in bin order (no prefix differences), so boxes holding the same
-//     point set tie bitwise;
-//   * boxes are ranked by |s| * rsqrt(r(1-r)) (one MUFU.RSQ + one FMUL; monotone in SR); a thread
-//     keeps only the maximum per block of 16 boxes (FMNMX3 tree) and the block's id, re-walks its
-//     winning block once at the end to find the box, and the merge step canonicalises exact ties
-//     (trim empty edge bins -> smallest width, then smallest start: reading R12).
+//   * the box search ranks boxes in packed fp32 (add/fma/mul.f32x2): a thread owns TWO adjacent
+//     frequencies and S consecutive start bins; it walks the bin rows once, converting each row
+//     (one LDS.64 per plane, I2FP) as it arrives, so a row feeds 2S boxes.  Per pair of boxes:
+//     FFMA2 (n -= W/SWT), FADD2 (s += Y), FFMA2 (n^2 + n = -r(1-r)), 2 MUFU.RSQ, FMUL2, FMNMX3.
+//     Running sums are direct (no prefix differences).  Only the maximum of |s| rsqrt(r(1-r)) per
+//     group of 4 rows is tracked; the group id goes to the merge step;
+//   * the merge step (one warp, lane = frequency) re-walks the winning group in EXACT integer
+//     arithmetic, applies the canonical tie-break (reading R12) and writes SR and depth from the
+//     integer box sums (R, S) in fp64, rounded once to fp32.
 #include "bls_internal.cuh"
 
 namespace bls {
 
-// `buffers` = 1 (search_kernel) or 2 (search_ws_kernel); `warps` = warps that write partial results
-size_t search_smem_bytes(int nb, int kmax, int warps, int buffers, int64_t n_points_in_smem)
+// Box-search geometry (host and device agree on it through these functions).
+// The nb start bins are dealt to `slots` half-warps, P = ceil(nb/slots) consecutive starts each;
+// a slot walks its starts as n = ceil(P/8) start tiles of S = base or base+1 starts, 4 <= S <= 8.
+__host__ __device__ inline int slot_starts(int nb, int slots) { int p = (nb + slots - 1) / slots; return p < 4 ? 4 : p; }
+
+// bin rows a search buffer holds: every start a0+u < slots*P (and < nb+8) reaches a0+u+kmax-1
+int search_rows_for(int nb, int kmax, int slots)
 {
-    size_t bins = (size_t)search_rows(nb, kmax) * kTileFreqs * 8;
-    size_t red = (size_t)2 * warps * kTileFreqs * 4;
-    return (size_t)buffers * (bins + red) + (size_t)n_points_in_smem * sizeof(PointRec);
+    const int P = slot_starts(nb, slots);
+    long long max_start = (long long)slots * P;
+    if (max_start > nb + 7) max_start = nb + 7;      // tiles starting at a0 >= nb are skipped; S <= 8
+    return (int)max_start + kmax;
 }
 
-// Geometry of the box search: a thread owns S consecutive start bins (S = 4 or 5), the
-// ceil(nb/S) start tiles of a column are dealt to the warps.  Pick (S, warps in [6,10]) that wastes
-// the fewest thread-tiles; ties go to S = 5 (fewer loads per box), then to more warps.
-void search_geometry(int nb, int max_warps, int *starts_per_thread, int *warps)
+// `buffers` = 1 (search_kernel) or 2 (search_ws_kernel); `warps` = box-search warps
+size_t search_smem_bytes(int nb, int kmax, int warps, int buffers, int64_t n_points_in_smem)
 {
-    int best_s = 4, best_w = 8;
-    double best_cost = 1e30;
-    for (int s = 4; s <= 5; ++s) {
-        const int nst = (nb + s - 1) / s;
-        for (int w = 6; w <= max_warps; ++w) {
-            const int per = (nst + w - 1) / w;
-            const double cost = (double)per * w * s / nb;      // thread-starts issued per useful start
-            if (cost < best_cost - 1e-9 || (cost < best_cost + 1e-9 && (s > best_s || (s == best_s && w > best_w)))) {
-                best_cost = cost; best_s = s; best_w = w;
-            }
-        }
-    }
-    *starts_per_thread = best_s;
-    *warps = best_w;
+    const size_t bins = (size_t)search_rows_for(nb, kmax, 2 * warps) * kTileFreqs * 8;
+    // candidates (rank, code) per buffer; merge posts: kernel 2 kMergeWarps, kernel 1 all its warps
+    const size_t cand = (size_t)buffers * warps * kTileFreqs * 8 + (size_t)(buffers == 2 ? kMergeWarps : warps) * kTileFreqs * 8;
+    return (size_t)buffers * bins + cand + (size_t)n_points_in_smem * sizeof(PointRec);
 }
 
 __device__ __noinline__ int canonical_bin(double f, double t, int nb)
@@ -81,62 +78,23 @@ __device__ __forceinline__ PointRec load_point(const PointRec *p)
     return r;
 }
 
-// Bins of one frequency column after the convert pass: row b holds the pair (W, Y) at col[b*32].
-struct Column {
-    const float2 *col;
-    int nb;
-    __device__ __forceinline__ float W(int b) const { return col[b * 32].x; }
-    __device__ __forceinline__ float Y(int b) const { return col[b * 32].y; }
-};
-
-// Scalar, guarded re-search of one frequency column in canonical order; only used when the fast
-// search produced a non-finite or impossible value (a box holding the entire weight, r == 1.0f).
-__device__ __noinline__ void careful_search(Column c, int kmin, int kmax, float &bv, uint32_t &bkey)
-{
-    bv = 0.f; bkey = ((uint32_t)kmin << 16);
-    for (int a = 0; a < c.nb; ++a) {
-        float r = 0.f, s = 0.f;
-        for (int k = 1; k <= kmax; ++k) {
-            int j = a + k - 1; if (j >= c.nb) j -= c.nb;
-            r += c.W(j); s += c.Y(j);
-            if (k < kmin) continue;
-            float den = fmaf(-r, r, r);
-            if (!(den > 0.f) || !(r < 1.f)) continue;
-            float v = s * s / den;
-            uint32_t key = ((uint32_t)k << 16) | (uint32_t)a;
-            if (v > bv || (v == bv && v > 0.f && key < bkey)) { bv = v; bkey = key; }
-        }
-    }
-}
-
-// Reading R12: among boxes holding the same point set take the smallest width, then the smallest
-// start.  Given any box of that family: drop empty bins at both ends; if that falls below kmin,
-// re-grow to kmin over empty bins, as far left as the numeric start index allows.
-__device__ __forceinline__ void canonicalise(Column c, int kmin, int &a, int &k)
-{
-    const int nb = c.nb;
-    auto empty = [&](int b) { return c.W(b) == 0.f && c.Y(b) == 0.f; };
-    while (k > 1 && empty(a)) { a = a + 1 == nb ? 0 : a + 1; --k; }
-    while (k > 1) { int e = a + k - 1; if (e >= nb) e -= nb; if (!empty(e)) break; --k; }
-    if (k < kmin) {
-        const int need = kmin - k;
-        int L = 0, R = 0;
-        while (L < need) { int b = a - 1 - L; if (b < 0) b += nb; if (!empty(b)) break; ++L; }
-        while (R < need) { int b = a + k + R; if (b >= nb) b -= nb; if (!empty(b)) break; ++R; }
-        const int d_hi = L, d_lo = need - R;          // feasible left shifts: d_lo <= d <= d_hi
-        const int d = (d_lo <= a) ? min(d_hi, a) : d_hi;
-        a -= d; if (a < 0) a += nb;
-        k = kmin;
-    }
-}
-
-// ---- packed fp32 pairs -------------------------------------------------------------------------
-// After the fold a bin row holds, per frequency column, the pair (W, Y) as one 64-bit word, so a
-// box's running sums (r, s) advance with ONE packed add (FADD2) fed by ONE LDS.64.
+// ---- packed fp32 pairs (sm_100a add/mul/fma.f32x2: one issue slot, two results) ---------------------
 __device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b)
 {
     uint64_t c;
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(c) : "l"(a), "l"(b));
+    return c;
+}
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b)
+{
+    uint64_t c;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(c) : "l"(a), "l"(b));
+    return c;
+}
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t d)
+{
+    uint64_t c;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(c) : "l"(a), "l"(b), "l"(d));
     return c;
 }
 __device__ __forceinline__ void unpack2(uint64_t v, float &lo, float &hi)
@@ -150,15 +108,15 @@ __device__ __forceinline__ uint64_t pack2(float lo, float hi)
     return v;
 }
 
-constexpr int kRowBytes = kTileFreqs * 8;   // one bin row: 32 columns x (W, Y)
+constexpr int kRowBytes = kTileFreqs * 8;   // one bin row: W plane [32 x u32] | Y plane [32 x i32]
 
 // Shared memory is addressed by 32-bit shared-window addresses with immediate offsets in the hot
 // loops (one address register per stream, no generic-pointer arithmetic).
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ uint64_t lds64(uint32_t addr)
+__device__ __forceinline__ uint2 lds64(uint32_t addr)
 {
-    uint64_t v;
-    asm volatile("ld.shared.b64 %0, [%1];" : "=l"(v) : "r"(addr));
+    uint2 v;
+    asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
     return v;
 }
 __device__ __forceinline__ uint32_t lds32(uint32_t addr)
@@ -173,9 +131,9 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr)
     asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
     return v;
 }
-__device__ __forceinline__ void sts64(uint32_t addr, uint64_t v)
+__device__ __forceinline__ void sts128(uint32_t addr, uint4 v)
 {
-    asm volatile("st.shared.b64 [%0], %1;" ::"r"(addr), "l"(v) : "memory");
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 __device__ __forceinline__ void red_add(uint32_t addr, uint32_t v)      // ATOMS.ADD, no return value
 {
@@ -192,150 +150,6 @@ __device__ __forceinline__ uint32_t row_addr(uint32_t base, uint32_t row)
 }
 static_assert(kRowBytes == 256, "row_addr hard-codes the row pitch");
 
-// rows g .. g+3 of this thread's column; `p` is the shared address of row g of the column
-__device__ __forceinline__ void load4(uint32_t p, uint64_t (&v)[4])
-{
-#pragma unroll
-    for (int i = 0; i < 4; ++i) v[i] = lds64(p + i * kRowBytes);
-}
-
-// 16 boxes: starts u = 0..3 (rows of the window), widths k0+1 .. k0+4.  Running sums advance by one
-// row per width; returns the largest |s| * rsqrt(r(1-r)).  NaN (empty box: 0 * inf, or r > 1 by
-// rounding: rsqrt of a negative, or an invalid start seeded with NaN) never wins an FMNMX.
-// The 8-row window is two halves (cur = rows g..g+3, nxt = rows g+4..g+7) so the caller can
-// ping-pong them instead of shifting registers.
-#define WIN(cur, nxt, i) ((i) < 4 ? cur[(i) & 3] : nxt[(i) & 3])
-
-template <int S, bool CHECK>
-__device__ __forceinline__ float block_max(uint64_t (&rs)[S], const uint64_t (&cur)[4], const uint64_t (&nxt)[4],
-                                           int k0, int kmin, int kmax)
-{
-    float mj[4] = {0.f, 0.f, 0.f, 0.f};           // one short FMNMX chain per width, joined at the end
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-#pragma unroll
-        for (int u = 0; u < S; ++u) rs[u] = add2(rs[u], WIN(cur, nxt, u + j));
-        if (!CHECK || (k0 + j + 1 >= kmin && k0 + j + 1 <= kmax)) {
-#pragma unroll
-            for (int u = 0; u < S; ++u) {
-                float r, s;
-                unpack2(rs[u], r, s);
-                const float den = fmaf(-r, r, r);       // r (1 - r)
-                const float t = s * fast_rsqrt(den);
-                mj[j] = fmaxf(mj[j], fabsf(t));
-            }
-        }
-    }
-    return fmaxf(fmaxf(mj[0], mj[1]), fmaxf(mj[2], mj[3]));
-}
-
-// Box search of one frequency column by one thread: start tiles tl = first, first+stride, ... of
-// S consecutive start bins each (S = 4 or 5: S + 3 rows fit the 8-row window).
-// `col` is the shared address of row 0 of the column; rows nb .. are copies of rows 0 .. (cyclic
-// boxes without index arithmetic).  Returns the best |t| (t^2 = SR) and its (width << 16 | start)
-// key; ties in any order.
-template <int S>
-__device__ __forceinline__ void search_column(uint32_t col, int nb, int kmin, int kmax, int first, int stride,
-                                              float &out_t, uint32_t &out_key)
-{
-    static_assert(S == 4 || S == 5, "the 8-row window holds S + 3 rows");
-    const int nst = (nb + S - 1) / S;
-    const int nkb = (kmax + 3) >> 2;
-    const int kb_full_lo = (kmin + 2) >> 2;          // blocks kb in [kb_full_lo, kb_full_hi) need no width check
-    const int kb_full_hi = kmax >> 2;
-    const uint64_t nan2 = pack2(__int_as_float(0x7fc00000), 0.f);
-    float best = 0.f;
-    int bcode = -1;
-    for (int tl = first; tl < nst; tl += stride) {
-        uint32_t p = col + tl * (S * kRowBytes);
-        const int tcode = tl << 10;
-        uint64_t rs[S], wa[4], wb[4];
-#pragma unroll
-        for (int u = 0; u < S; ++u) rs[u] = (tl * S + u < nb) ? 0ull : nan2;
-        load4(p, wa);
-        int kb = 0;
-        // head blocks below kmin (only when kmin > 4), one at a time, window shifted through registers
-        for (; kb < kb_full_lo && kb < nkb; ++kb) {
-            p += 4 * kRowBytes;
-            load4(p, wb);
-            const float m = block_max<S, true>(rs, wa, wb, kb * 4, kmin, kmax);
-            if (m > best) { best = m; bcode = tcode | kb; }
-#pragma unroll
-            for (int i = 0; i < 4; ++i) wa[i] = wb[i];
-        }
-        // two full blocks per iteration, the window halves ping-pong
-        for (; kb + 2 <= kb_full_hi; kb += 2) {
-            load4(p + 4 * kRowBytes, wb);
-            float m = block_max<S, false>(rs, wa, wb, 0, 0, 0);
-            if (m > best) { best = m; bcode = tcode | kb; }
-            load4(p + 8 * kRowBytes, wa);
-            m = block_max<S, false>(rs, wb, wa, 0, 0, 0);
-            if (m > best) { best = m; bcode = tcode | (kb + 1); }
-            p += 8 * kRowBytes;
-        }
-        // tail: at most one full block and the block that holds kmax
-        if (kb + 2 <= nkb) {
-            load4(p + 4 * kRowBytes, wb);
-            float m = block_max<S, true>(rs, wa, wb, kb * 4, kmin, kmax);
-            if (m > best) { best = m; bcode = tcode | kb; }
-            load4(p + 8 * kRowBytes, wa);
-            m = block_max<S, true>(rs, wb, wa, kb * 4 + 4, kmin, kmax);
-            if (m > best) { best = m; bcode = tcode | (kb + 1); }
-        } else if (kb < nkb) {
-            load4(p + 4 * kRowBytes, wb);
-            const float m = block_max<S, true>(rs, wa, wb, kb * 4, kmin, kmax);
-            if (m > best) { best = m; bcode = tcode | kb; }
-        }
-    }
-    out_t = 0.f;
-    out_key = (uint32_t)kmin << 16;
-    if (bcode < 0) return;
-    // Re-walk to the winning block: first only the running sums (lanes differ in how far they
-    // go, so this loop holds nothing else), then that block's boxes once, with the argmax.
-    // Identical operations in identical order, so identical values.
-    const int tl = bcode >> 10, kbs = bcode & 1023;
-    uint32_t p = col + tl * (S * kRowBytes);
-    uint64_t rs[S], w[8];
-#pragma unroll
-    for (int u = 0; u < S; ++u) rs[u] = (tl * S + u < nb) ? 0ull : nan2;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) w[i] = lds64(p + i * kRowBytes);
-    for (int kb = 0; kb < kbs; ++kb) {
-        p += 4 * kRowBytes;
-#pragma unroll
-        for (int i = 0; i < 4; ++i) w[4 + i] = lds64(p + i * kRowBytes);
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-#pragma unroll
-            for (int u = 0; u < S; ++u) rs[u] = add2(rs[u], w[u + j]);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) w[i] = w[i + 4];
-    }
-    p += 4 * kRowBytes;
-#pragma unroll
-    for (int i = 0; i < 4; ++i) w[4 + i] = lds64(p + i * kRowBytes);
-    float bt = 0.f;
-    int bk = kmin, bu = 0;
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-#pragma unroll
-        for (int u = 0; u < S; ++u) rs[u] = add2(rs[u], w[u + j]);
-        const int k = kbs * 4 + j + 1;
-        if (k >= kmin && k <= kmax) {
-#pragma unroll
-            for (int u = 0; u < S; ++u) {
-                float r, s;
-                unpack2(rs[u], r, s);
-                const float den = fmaf(-r, r, r);
-                const float t = fabsf(s * fast_rsqrt(den));
-                if (t > bt) { bt = t; bk = k; bu = u; }
-            }
-        }
-    }
-    out_t = bt;
-    out_key = ((uint32_t)bk << 16) | (uint32_t)(tl * S + bu);
-}
-
 // ---- the phases of one tile (32 trial frequencies, one per lane), written for a GROUP of warps:
 //      `gw` = this warp's index in the group, `gnw` = warps in the group -------------------------
 
@@ -343,8 +157,19 @@ struct TileCtx {
     int nb, nrows, kmin, kmax, n;
     uint32_t G;
     bool force_canon;
-    float cw, cy, wx2;
+    float ncw, cy, wx2;       // -1/SWT, 1/SY, sum w x^2
+    uint32_t swt;             // exact total of the integer weights
+    double sr_scale, dp_scale;
 };
+
+__device__ __forceinline__ void load_ctx(TileCtx &c, const SearchArgs &a, const CurveMeta &meta, int nrows)
+{
+    c.nb = a.nb; c.kmin = a.kmin; c.kmax = a.kmax; c.nrows = nrows;
+    c.force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
+    c.ncw = meta.ncw; c.cy = meta.cy; c.wx2 = (float)meta.wx2;
+    c.swt = meta.swt; c.sr_scale = meta.sr_scale; c.dp_scale = meta.dp_scale;
+    c.G = (uint32_t)a.nb + 8u;                    // guard band, units of 2^-32 bin
+}
 
 __device__ __forceinline__ void zero_bins(uint32_t bins_s, int nb, int gtid, int gthreads)
 {
@@ -452,50 +277,211 @@ __device__ __forceinline__ void fold_tile(const TileCtx &c, double f, uint32_t b
     }
 }
 
-// fixed point -> fp32 pairs (weight fraction, weighted residual), in place, plus the cyclic
-// extension rows nb .. nrows-1.  A warp owns whole rows, so reading both int planes before
-// writing the pairs needs only a warp sync.
-__device__ __forceinline__ void convert_rows(const TileCtx &c, uint32_t bins_s, int lane, int gw, int gnw)
+// Cyclic extension: rows nb .. nrows-1 repeat rows 0 .., so a box that crosses phase 1 needs no
+// index arithmetic in the search (reading R11).  16-byte chunks dealt to the group's threads.
+__device__ __forceinline__ void extend_rows(const TileCtx &c, uint32_t bins_s, int gtid, int gthreads)
 {
-    const int nb = c.nb;
-    const int next = c.nrows - nb;                // extension rows
-    uint32_t ra = bins_s + gw * kRowBytes + lane * 4;
-    if (next <= nb) {                             // every shape but tiny nb with wide boxes
-        int j = gw;
-        for (; j + gnw < nb; j += 2 * gnw, ra += 2 * gnw * kRowBytes) {     // two rows in flight
-            const uint32_t rb = ra + gnw * kRowBytes;
-            const uint32_t qw0 = lds32(ra), qw1 = lds32(rb);
-            const int32_t qy0 = (int32_t)lds32(ra + 128), qy1 = (int32_t)lds32(rb + 128);
-            __syncwarp();
-            const uint64_t v0 = pack2((float)qw0 * c.cw, (float)qy0 * c.cy);
-            const uint64_t v1 = pack2((float)qw1 * c.cw, (float)qy1 * c.cy);
-            const uint32_t wa = ra + lane * 4, wb = rb + lane * 4;
-            sts64(wa, v0);
-            sts64(wb, v1);
-            if (j < next) sts64(wa + nb * kRowBytes, v0);
-            if (j + gnw < next) sts64(wb + nb * kRowBytes, v1);
-        }
-        for (; j < nb; j += gnw, ra += gnw * kRowBytes) {
-            const uint32_t qw = lds32(ra);
-            const int32_t qy = (int32_t)lds32(ra + 128);
-            __syncwarp();
-            const uint64_t v = pack2((float)qw * c.cw, (float)qy * c.cy);
-            const uint32_t wa = ra + lane * 4;
-            sts64(wa, v);
-            if (j < next) sts64(wa + nb * kRowBytes, v);
-        }
-    } else {
-        for (int j = gw; j < nb; j += gnw, ra += gnw * kRowBytes) {
-            const uint32_t qw = lds32(ra);
-            const int32_t qy = (int32_t)lds32(ra + 128);
-            __syncwarp();
-            const uint64_t v = pack2((float)qw * c.cw, (float)qy * c.cy);
-            uint32_t wa = ra + lane * 4;
-            sts64(wa, v);
-            for (int x = j + nb; x < c.nrows; x += nb) { wa += nb * kRowBytes; sts64(wa, v); }
-        }
+    const int nvec = (c.nrows - c.nb) * (kRowBytes / 16);
+    for (int i = gtid; i < nvec; i += gthreads) {
+        const int row = i >> 4, col = i & 15;
+        const int src = row % c.nb;
+        sts128(bins_s + (c.nb + row) * kRowBytes + col * 16, lds128(bins_s + src * kRowBytes + col * 16));
     }
 }
+
+// ---- a3/a4 box search ------------------------------------------------------------------------------
+// A start tile is S consecutive start bins a0 .. a0+S-1 walked over the rows x = 0 .. kmax+S-2 of the
+// column (row x = bin a0+x; rows >= nb are the cyclic extension); box (u, k) = start a0+u, width k
+// ends at row x = u+k-1.  Only the maximum rank per GROUP of rows is tracked:
+//   fast geometry (kmin == 1 and kmax >= S-1): group 0 = head rows [0, S-1); group g in 1..nfull =
+//     rows [S-1+4(g-1), S-1+4g), nfull = (kmax-S+1)/4; group nfull+1 = the rest (incl. the tail);
+//   general geometry: group g = rows [4g, 4g+4).
+// A candidate code is  g | S << 10 | a0 << 14  (bit 31: the column needs the exact full search).
+__host__ __device__ __forceinline__ bool fast_geometry(int S, int kmin, int kmax) { return kmin == 1 && kmax >= S - 1; }
+
+__device__ __forceinline__ void group_rows(int S, int kmin, int kmax, int g, int &x0, int &x1)
+{
+    const int xend = kmax + S - 1;
+    if (fast_geometry(S, kmin, kmax)) {
+        const int nfull = (kmax - S + 1) >> 2;
+        if (g == 0) { x0 = 0; x1 = S - 1; }
+        else if (g <= nfull) { x0 = S - 1 + 4 * (g - 1); x1 = x0 + 4; }
+        else { x0 = S - 1 + 4 * nfull; x1 = xend; }
+    } else {
+        x0 = 4 * g; x1 = min(x0 + 4, xend);
+    }
+}
+
+struct Best {               // per thread: its two frequencies
+    float t0, t1;           // best |s| rsqrt(r(1-r)) seen (units of 1/SY)
+    uint32_t c0, c1;        // candidate codes
+    float nmin0, nmin1;     // min over starts of n = -r at width kmax
+};
+
+struct RowI { uint2 w, y; };
+__device__ __forceinline__ RowI ld_row(uint32_t p)
+{
+    RowI r;
+    r.w = lds64(p);             // W plane: (qW[f0], qW[f1])
+    r.y = lds64(p + 128);       // Y plane
+    return r;
+}
+__device__ __forceinline__ void cvt_row(const RowI &r, uint64_t &W, uint64_t &Y)
+{
+    W = pack2(__uint2float_rn(r.w.x), __uint2float_rn(r.w.y));
+    Y = pack2(__int2float_rn((int)r.y.x), __int2float_rn((int)r.y.y));
+}
+__device__ __forceinline__ void box_acc(uint64_t &n, uint64_t &s, uint64_t W, uint64_t Y, uint64_t ncw2)
+{
+    n = fma2(W, ncw2, n);       // n = -r
+    s = add2(s, Y);
+}
+// rank |s| rsqrt(r(1-r)); n^2 + n = -r(1-r).  An empty box gives 0 * inf = NaN, which never wins an
+// FMNMX; r == 1 gives inf, which the merge step recognises as impossible.
+__device__ __forceinline__ void box_eval(uint64_t n, uint64_t s, float &m0, float &m1)
+{
+    const uint64_t d = fma2(n, n, n);
+    float d0, d1;
+    unpack2(d, d0, d1);
+#ifdef BLS_DEV_NOMUFU
+    const uint64_t t = mul2(s, pack2(fabsf(d0) * 1.0001f, fabsf(d1) * 1.0001f));
+#else
+    const uint64_t t = mul2(s, pack2(fast_rsqrt(fabsf(d0)), fast_rsqrt(fabsf(d1))));
+#endif
+    float t0, t1;
+    unpack2(t, t0, t1);
+    m0 = fmaxf(m0, fabsf(t0));
+    m1 = fmaxf(m1, fabsf(t1));
+}
+
+template <int S>
+__device__ __forceinline__ void search_tile(uint32_t p, int kmin, int kmax, uint64_t ncw2, uint32_t tcode, Best &b)
+{
+    uint64_t rn[S], rs[S];
+#pragma unroll
+    for (int u = 0; u < S; ++u) { rn[u] = 0ull; rs[u] = 0ull; }
+    float m0 = 0.f, m1 = 0.f;
+    auto close_group = [&](uint32_t g) {
+        if (m0 > b.t0) { b.t0 = m0; b.c0 = tcode | g; }
+        if (m1 > b.t1) { b.t1 = m1; b.c1 = tcode | g; }
+        m0 = 0.f; m1 = 0.f;
+    };
+    RowI nx = ld_row(p);
+    uint64_t W, Y;
+    if (fast_geometry(S, kmin, kmax)) {
+#pragma unroll
+        for (int x = 0; x < S - 1; ++x) {                    // head: row x closes starts u <= x
+            const RowI cur = nx;
+            p += kRowBytes; nx = ld_row(p);
+            cvt_row(cur, W, Y);
+#pragma unroll
+            for (int u = 0; u <= x; ++u) { box_acc(rn[u], rs[u], W, Y, ncw2); box_eval(rn[u], rs[u], m0, m1); }
+        }
+        close_group(0u);
+        int x = S - 1;
+        uint32_t g = 1u;
+        for (; x + 4 <= kmax; x += 4, ++g) {                 // full rows: every start, no checks
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const RowI cur = nx;
+                p += kRowBytes; nx = ld_row(p);
+                cvt_row(cur, W, Y);
+#pragma unroll
+                for (int u = 0; u < S; ++u) { box_acc(rn[u], rs[u], W, Y, ncw2); box_eval(rn[u], rs[u], m0, m1); }
+            }
+            close_group(g);
+        }
+        for (; x < kmax; ++x) {
+            const RowI cur = nx;
+            p += kRowBytes; nx = ld_row(p);
+            cvt_row(cur, W, Y);
+#pragma unroll
+            for (int u = 0; u < S; ++u) { box_acc(rn[u], rs[u], W, Y, ncw2); box_eval(rn[u], rs[u], m0, m1); }
+        }
+#pragma unroll
+        for (int d = 0; d < S - 1; ++d) {                    // tail: row kmax+d serves starts u > d
+            const RowI cur = nx;
+            if (d < S - 2) { p += kRowBytes; nx = ld_row(p); }
+            cvt_row(cur, W, Y);
+#pragma unroll
+            for (int u = d + 1; u < S; ++u) { box_acc(rn[u], rs[u], W, Y, ncw2); box_eval(rn[u], rs[u], m0, m1); }
+        }
+        close_group(g);
+    } else {
+        const int xend = kmax + S - 1;
+        for (int x = 0; x < xend; ++x) {
+            const RowI cur = nx;
+            p += kRowBytes; nx = ld_row(p);                  // the last one reads one row too far (unused)
+            cvt_row(cur, W, Y);
+#pragma unroll
+            for (int u = 0; u < S; ++u) {
+                const int k = x - u + 1;
+                if (k >= 1 && k <= kmax) {
+                    box_acc(rn[u], rs[u], W, Y, ncw2);
+                    if (k >= kmin) box_eval(rn[u], rs[u], m0, m1);
+                }
+            }
+            if ((x & 3) == 3 || x == xend - 1) close_group((uint32_t)(x >> 2));
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < S; ++u) {                            // rn[u] = -r(start u, width kmax)
+        float a0, a1;
+        unpack2(rn[u], a0, a1);
+        b.nmin0 = fminf(b.nmin0, a0);
+        b.nmin1 = fminf(b.nmin1, a1);
+    }
+}
+
+// The starts of slot `slot` of `nslots` (half-warps), as start tiles of 4..8 starts.  `col` is the
+// shared address of row 0 of this thread's frequency pair (W plane).
+__device__ __forceinline__ void search_slot(uint32_t col, const TileCtx &c, int slot, int nslots, Best &b)
+{
+    const int P = slot_starts(c.nb, nslots);
+    int a0 = slot * P;
+    if (a0 >= c.nb) return;
+    const int n = (P + 7) >> 3, base = P / n, extra = P - base * n;
+    const uint64_t ncw2 = pack2(c.ncw, c.ncw);
+    for (int i = 0; i < n && a0 < c.nb; ++i) {
+        const int S = base + (i < extra ? 1 : 0);
+        const uint32_t tcode = ((uint32_t)a0 << 14) | ((uint32_t)S << 10);
+        const uint32_t p = col + a0 * kRowBytes;
+        switch (S) {
+            case 4: search_tile<4>(p, c.kmin, c.kmax, ncw2, tcode, b); break;
+            case 5: search_tile<5>(p, c.kmin, c.kmax, ncw2, tcode, b); break;
+            case 6: search_tile<6>(p, c.kmin, c.kmax, ncw2, tcode, b); break;
+            case 7: search_tile<7>(p, c.kmin, c.kmax, ncw2, tcode, b); break;
+            default: search_tile<8>(p, c.kmin, c.kmax, ncw2, tcode, b); break;
+        }
+        a0 += S;
+    }
+}
+
+// Box search of one tile by one warp: lanes l and l+16 own the frequency pair (2l', 2l'+1),
+// l' = l & 15, and different slots.  Writes the warp's 32 candidates (rank, code) to cand_t/cand_c.
+__device__ __forceinline__ void search_warp(uint32_t bins_s, const TileCtx &c, int lane, int sw, int nsw,
+                                            float *cand_t, uint32_t *cand_c)
+{
+    Best b;
+    b.t0 = 0.f; b.t1 = 0.f; b.c0 = 0u; b.c1 = 0u; b.nmin0 = 0.f; b.nmin1 = 0.f;
+    const int half = lane >> 4, lp = lane & 15;
+    search_slot(bins_s + lp * 8, c, 2 * sw + half, 2 * nsw, b);
+    __syncwarp();
+    const float ot0 = __shfl_xor_sync(0xffffffffu, b.t0, 16), ot1 = __shfl_xor_sync(0xffffffffu, b.t1, 16);
+    const uint32_t oc0 = __shfl_xor_sync(0xffffffffu, b.c0, 16), oc1 = __shfl_xor_sync(0xffffffffu, b.c1, 16);
+    const float on0 = __shfl_xor_sync(0xffffffffu, b.nmin0, 16), on1 = __shfl_xor_sync(0xffffffffu, b.nmin1, 16);
+    if (ot0 > b.t0) { b.t0 = ot0; b.c0 = oc0; }
+    if (ot1 > b.t1) { b.t1 = ot1; b.c1 = oc1; }
+    // a box holding more than 0.9 of the weight: r(1-r) loses precision in fp32 -> exact full search
+    if (fminf(b.nmin0, on0) < -0.9f) b.c0 |= 0x80000000u;
+    if (fminf(b.nmin1, on1) < -0.9f) b.c1 |= 0x80000000u;
+    if (half == 0) {
+        *reinterpret_cast<float2 *>(cand_t + sw * 32 + 2 * lp) = make_float2(b.t0, b.t1);
+        *reinterpret_cast<uint2 *>(cand_c + sw * 32 + 2 * lp) = make_uint2(b.c0, b.c1);
+    }
+}
+
+// ---- merge: exact integer re-evaluation of the winning group, canonical ties, outputs -----------------
 
 // Outputs of one (curve, frequency).
 struct OutPtrs {
@@ -503,45 +489,195 @@ struct OutPtrs {
     float *u_sr; uint16_t *u_start; uint16_t *u_width; float *u_depth;   // user rows or NULL
 };
 
-// Merge the per-warp partial results of column `lane`, canonicalise exact ties (R12), recompute
-// (r, s) of the chosen box by direct summation and write SR = s^2/den, depth = s/den (IEEE
-// division).  The chains below are serial per column, so callers spread the 32 columns over
-// several warps.
-__device__ __forceinline__ void merge_column(const TileCtx &c, const float2 *rows2, const float *red_v,
-                                             const uint32_t *red_key, int nparts, int lane, int q, int nf,
-                                             const OutPtrs &o)
+// One integer column of a bin buffer: row b holds qW at colw + b*256 and qY 128 bytes later.
+struct IntColumn {
+    uint32_t colw;
+    int nb;
+    __device__ __forceinline__ uint32_t W(int b) const { return lds32(colw + b * kRowBytes); }
+    __device__ __forceinline__ int32_t Y(int b) const { return (int32_t)lds32(colw + b * kRowBytes + 128); }
+    __device__ __forceinline__ bool empty(int b) const { return W(b) == 0u && Y(b) == 0; }
+};
+
+struct ExactBest {
+    float v;            // S^2 / (R (SWT - R)) evaluated in fp32 from the exact integers: ranking only
+    int a, k;
+    uint32_t R;
+    int32_t S;
+};
+
+// Reading R10: a box is valid iff r(1-r) > 0, decided exactly on the integers.  Reading R12: among
+// equal values the smallest width wins, then the smallest start.  v is a deterministic function of
+// (R, S), so boxes holding the same point set tie exactly.
+__device__ __forceinline__ void exact_eval(uint32_t R, int32_t S, uint32_t swt, int a, int k, ExactBest &e)
 {
-    const int nb = c.nb, kmin = c.kmin, kmax = c.kmax;
-    float bt = red_v[lane];
-    uint32_t bkey = red_key[lane];
-#pragma unroll 4
-    for (int w = 1; w < nparts; ++w) {
-        const float v = red_v[w * 32 + lane];
-        const uint32_t key = red_key[w * 32 + lane];
-        if (v > bt) { bt = v; bkey = key; }
+    if (R == 0u || R >= swt) return;
+    const float Sf = (float)S;
+    const float v = __fdividef(Sf * Sf, (float)R * (float)(swt - R));   // deterministic in (R, S)
+    if (v > e.v || (v == e.v && v > 0.f && (k < e.k || (k == e.k && a < e.a)))) {
+        e.v = v; e.a = a; e.k = k; e.R = R; e.S = S;
     }
-    const Column col{rows2 + lane, nb};
-    float bv = bt * bt;
-    if (!(bv <= 1.001f * c.wx2 + 1e-30f)) {   // inf / impossible: r == 1.0f box
-        careful_search(col, kmin, kmax, bv, bkey);
-        bt = bv;
+}
+
+// Boxes (a0+u, k) that end in rows [x0, x1) of a start tile, from exact integer sums: one pass over
+// the rows keeps the prefix sum (PW, PY) of rows a0 .. a0+x; box (u, k = x-u+1) is that prefix minus
+// the prefix before row u, rebuilt per row from the first 8 rows held in registers (S <= 8).
+__device__ __forceinline__ void exact_group(const IntColumn &c, int kmin, int kmax, uint32_t swt, int a0, int S,
+                                            int x0, int x1, ExactBest &e)
+{
+    const uint32_t p = c.colw + a0 * kRowBytes;
+    uint32_t hw[8];
+    int32_t hy[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { hw[u] = lds32(p + u * kRowBytes); hy[u] = (int32_t)lds32(p + u * kRowBytes + 128); }
+    uint32_t PW = 0u;
+    int32_t PY = 0;
+    int x = 0;
+    uint32_t q = p;
+    for (; x + 4 <= x0; x += 4, q += 4 * kRowBytes) {        // rows before the group: sums only
+        const uint32_t w0 = lds32(q), w1 = lds32(q + kRowBytes), w2 = lds32(q + 2 * kRowBytes), w3 = lds32(q + 3 * kRowBytes);
+        const uint32_t y0 = lds32(q + 128), y1 = lds32(q + kRowBytes + 128), y2 = lds32(q + 2 * kRowBytes + 128),
+                       y3 = lds32(q + 3 * kRowBytes + 128);
+        PW += (w0 + w1) + (w2 + w3);
+        PY += (int32_t)((y0 + y1) + (y2 + y3));
     }
-    int bk = (int)(bkey >> 16), ba = (int)(bkey & 0xffffu);
-    if (bt > 0.f) canonicalise(col, kmin, ba, bk);
-    else { bk = kmin; ba = 0; }
-    float r = 0.f, s = 0.f;
-    {   // bins in order (as the oracle sums them); rows nb .. repeat rows 0 .., so no wrap; loads 4 ahead
-        const float2 *pr = col.col + ba * 32;
-        int j = 0;
-        for (; j + 4 <= bk; j += 4, pr += 128) {
-            const float2 v0 = pr[0], v1 = pr[32], v2 = pr[64], v3 = pr[96];
-            r += v0.x; s += v0.y; r += v1.x; s += v1.y; r += v2.x; s += v2.y; r += v3.x; s += v3.y;
+    for (; x < x1; ++x, q += kRowBytes) {
+        PW += lds32(q);
+        PY += (int32_t)lds32(q + 128);
+        if (x < x0) continue;
+        uint32_t bw = 0u;                                    // prefix before row u
+        int32_t by = 0;
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int k = x - u + 1;
+            if (u < S && k >= kmin && k <= kmax) {
+                const int a = a0 + u;
+                exact_eval(PW - bw, PY - by, swt, a >= c.nb ? a - c.nb : a, k, e);
+            }
+            bw += hw[u]; by += hy[u];
         }
-        for (; j < bk; ++j, pr += 32) { r += pr[0].x; s += pr[0].y; }
     }
-    const float den = fmaf(-r, r, r);
+}
+
+// every box of the column, in the oracle's order (guarded path: degenerate columns only)
+__device__ __noinline__ void exact_full(IntColumn c, int kmin, int kmax, uint32_t swt, ExactBest &e)
+{
+    for (int a = 0; a < c.nb; ++a) {
+        uint32_t R = 0u;
+        int32_t Sy = 0;
+        for (int k = 1; k <= kmax; ++k) {
+            int j = a + k - 1; if (j >= c.nb) j -= c.nb;
+            R += c.W(j); Sy += c.Y(j);
+            if (k >= kmin) exact_eval(R, Sy, swt, a, k, e);
+        }
+    }
+}
+
+// Reading R12: among boxes holding the same point set take the smallest width, then the smallest
+// start.  Given any box of that family: drop empty bins at both ends; if that falls below kmin,
+// re-grow to kmin over empty bins, as far left as the numeric start index allows.
+__device__ __forceinline__ void canonicalise(const IntColumn &c, int kmin, int &a, int &k)
+{
+    const int nb = c.nb;
+    while (k > 1 && c.empty(a)) { a = a + 1 == nb ? 0 : a + 1; --k; }
+    while (k > 1) { int e = a + k - 1; if (e >= nb) e -= nb; if (!c.empty(e)) break; --k; }
+    if (k < kmin) {
+        const int need = kmin - k;
+        int L = 0, R = 0;
+        while (L < need) { int b = a - 1 - L; if (b < 0) b += nb; if (!c.empty(b)) break; ++L; }
+        while (R < need) { int b = a + k + R; if (b >= nb) b -= nb; if (!c.empty(b)) break; ++R; }
+        const int d_hi = L, d_lo = need - R;          // feasible left shifts: d_lo <= d <= d_hi
+        const int d = (d_lo <= a) ? min(d_hi, a) : d_hi;
+        a -= d; if (a < 0) a += nb;
+        k = kmin;
+    }
+}
+
+// boxes (a0+u, k) of ONE start that end in rows [x0, x1): exact integer running sums in bin order
+__device__ __forceinline__ void exact_start(const IntColumn &c, int kmin, int kmax, uint32_t swt, int a0, int u,
+                                            int x0, int x1, ExactBest &e)
+{
+    const int klo = max(kmin, x0 - u + 1), khi = min(kmax, x1 - u);
+    if (khi < klo) return;
+    const int a = a0 + u;
+    const int an = a >= c.nb ? a - c.nb : a;              // starts in the cyclic extension
+    uint32_t R = 0u;
+    int32_t Sy = 0;
+    uint32_t p = c.colw + a * kRowBytes;
+    int k = 1;
+    for (; k + 3 < klo; k += 4, p += 4 * kRowBytes) {      // below klo: sums only, four rows in flight
+        const uint32_t w0 = lds32(p), w1 = lds32(p + kRowBytes), w2 = lds32(p + 2 * kRowBytes), w3 = lds32(p + 3 * kRowBytes);
+        const uint32_t y0 = lds32(p + 128), y1 = lds32(p + kRowBytes + 128), y2 = lds32(p + 2 * kRowBytes + 128),
+                       y3 = lds32(p + 3 * kRowBytes + 128);
+        R += (w0 + w1) + (w2 + w3);
+        Sy += (int32_t)((y0 + y1) + (y2 + y3));
+    }
+    for (; k <= khi; ++k, p += kRowBytes) {
+        R += lds32(p); Sy += (int32_t)lds32(p + 128);
+        if (k >= klo) exact_eval(R, Sy, swt, an, k, e);
+    }
+}
+
+// Merge of one tile by `mw` warps (warp `w` of them, lane = frequency column):
+//   A  best of the `ncand` candidates (rank, code) of the column -> winning start tile and group;
+//   B  warp w re-evaluates starts u = w, w+mw, .. of that group in exact integer arithmetic
+//      (one warp: the whole group in one pass) and posts its best (value, width << 16 | start);
+//   C  after `sync`, the warp that holds the column's best box (value, then smallest width, then
+//      smallest start: reading R12) canonicalises it and writes
+//      SR = S^2/(R(SWT-R)) * sr_scale, depth = S/(R(SWT-R)) * dp_scale   (fp64, rounded once).
+// cand_t/cand_c: [ncand][32] written by search_warp (and made visible by the caller's barrier);
+// post_v/post_k: [mw][32] scratch.  Warps w >= mw of the group only take part in `sync`.
+template <typename Sync>
+__device__ __forceinline__ void merge_tile(const TileCtx &c, uint32_t bins_s, const float *cand_t, const uint32_t *cand_c,
+                                           float *post_v, uint32_t *post_k, int ncand, int mw, int w, int lane, int q,
+                                           int nf, const OutPtrs &o, Sync sync)
+{
+    if (w >= mw) { if (mw > 1) sync(); return; }
+    float bt = 0.f;
+    uint32_t bc = 0u, flag = 0u;
+    for (int p = 0; p < ncand; ++p) {
+        const float t = cand_t[p * 32 + lane];
+        const uint32_t cc = cand_c[p * 32 + lane];
+        flag |= cc;
+        if (t > bt) { bt = t; bc = cc; }
+    }
+    const IntColumn col{bins_s + (uint32_t)lane * 4u, c.nb};
+    ExactBest e;
+    e.v = 0.f; e.a = 0; e.k = c.kmin; e.R = 0u; e.S = 0;
+    const float tv = bt * c.cy;
+    if ((flag >> 31) || !(tv * tv <= 1.001f * c.wx2 + 1e-30f)) {     // a box near r = 1, or inf / NaN
+        if (w == 0) exact_full(col, c.kmin, c.kmax, c.swt, e);
+    } else if (bt > 0.f) {
+        const int g = (int)(bc & 1023u), S = (int)((bc >> 10) & 15u), a0 = (int)((bc >> 14) & 0x1fffu);
+        int x0, x1;
+        group_rows(S, c.kmin, c.kmax, g, x0, x1);
+        if (mw == 1) exact_group(col, c.kmin, c.kmax, c.swt, a0, S, x0, x1, e);
+        else for (int u = w; u < S; u += mw) exact_start(col, c.kmin, c.kmax, c.swt, a0, u, x0, x1, e);
+    }
+    int win = 0;
+    if (mw > 1) {
+        post_v[w * 32 + lane] = e.v;
+        post_k[w * 32 + lane] = ((uint32_t)e.k << 16) | (uint32_t)e.a;
+        sync();
+        float bv = 0.f;
+        uint32_t bkey = 0xffffffffu;
+        for (int p = 0; p < mw; ++p) {
+            const float v = post_v[p * 32 + lane];
+            const uint32_t key = post_k[p * 32 + lane];
+            if (v > bv || (v == bv && v > 0.f && key < bkey)) { bv = v; bkey = key; win = p; }
+        }
+        if (!(bv > 0.f)) { win = 0; e.v = 0.f; }
+    }
+    if (win != w) return;
     float sr = 0.f, dp = 0.f;
-    if (bt > 0.f && den > 0.f) { sr = (s * s) / den; dp = s / den; }
+    int ba = 0, bk = c.kmin;
+    if (e.v > 0.f) {
+        ba = e.a; bk = e.k;
+        canonicalise(col, c.kmin, ba, bk);
+        const double Rd = (double)e.R, Cd = (double)(c.swt - e.R), Sd = (double)e.S;
+        const double inv = 1.0 / (Rd * Cd);
+        sr = (float)(Sd * Sd * inv * c.sr_scale);
+        dp = (float)(Sd * inv * c.dp_scale);
+    }
     if (q < nf) {
         o.sr[q] = sr; o.ak[q] = ((uint32_t)bk << 16) | (uint32_t)ba; o.depth[q] = dp;
         if (o.u_sr) o.u_sr[q] = sr;
@@ -583,10 +719,44 @@ __device__ __forceinline__ void count_canonical(const SearchArgs &a, unsigned in
     }
 }
 
+// ---- common prologue: which curve / tiles this CTA owns; stage the curve (a1 Load) -------------------
+struct WorkItem {
+    int64_t curve_local, cv, beg;
+    int tile0, tile1;
+    CurveMeta meta;
+    OutPtrs out;
+};
+
+__device__ __forceinline__ WorkItem work_item(const SearchArgs &a, TileCtx &c)
+{
+    WorkItem w;
+    w.curve_local = blockIdx.x / a.items_per_curve;
+    const int item = blockIdx.x % a.items_per_curve;
+    w.cv = a.curve_base + w.curve_local;
+    w.beg = a.offsets[w.cv];
+    c.n = (int)(a.offsets[w.cv + 1] - w.beg);
+    w.meta = a.meta[w.cv];
+    const int ntiles = (a.nf + kTileFreqs - 1) / kTileFreqs;
+    w.tile0 = item * a.tiles_per_item;
+    w.tile1 = min(w.tile0 + a.tiles_per_item, ntiles);
+    w.out = out_rows(a, w.curve_local, w.cv);
+    load_ctx(c, a, w.meta, a.nrows);
+    return w;
+}
+
+template <bool PTS_SMEM>
+__device__ __forceinline__ void stage_curve(const PointRec *pts_g, PointRec *pts_s, int n, int tid, int nthr)
+{
+    if (PTS_SMEM) {                               // coalesced LDG.128 -> STS.128, once per work item
+        const uint4 *src = reinterpret_cast<const uint4 *>(pts_g);
+        uint4 *dst = reinterpret_cast<uint4 *>(pts_s);
+        for (int i = tid; i < n; i += nthr) dst[i] = __ldg(src + i);
+    }
+}
+
 // ---- kernel 1: every warp does every phase, phases separated by CTA barriers.  Used where the
-//      double-buffered bins of kernel 2 do not fit shared memory (e.g. nb = 400).  Two CTAs per
-//      SM overlap each other's LSU-bound fold and XU-bound box search only by chance. -----------
-template <bool PTS_SMEM, int S>
+//      double-buffered bins of kernel 2 do not fit shared memory (nb above ~420 at wide boxes). ------
+template <bool PTS_SMEM>
 __global__ void __launch_bounds__(kMaxSearchWarps * 32, 2)
 search_kernel(const SearchArgs a)
 {
@@ -594,73 +764,47 @@ search_kernel(const SearchArgs a)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nthr = blockDim.x, nw = nthr >> 5;
     TileCtx c;
-    c.nb = a.nb; c.kmin = a.kmin; c.kmax = a.kmax;
-    c.nrows = search_rows(a.nb, a.kmax);
-    // smem: bins [nrows][256 B] | red_v [nw][32] | red_key [nw][32] | points [n] (if PTS_SMEM)
-    float *red_v = reinterpret_cast<float *>(smem_raw + (size_t)c.nrows * kRowBytes);
-    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + nw * 32);
-    PointRec *pts_s = reinterpret_cast<PointRec *>(red_key + nw * 32);
-    const float2 *rows2 = reinterpret_cast<const float2 *>(smem_raw);
+    const WorkItem w = work_item(a, c);
+    // smem: bins [nrows][256 B] | cand_t, cand_c, post_v, post_k [nw][32] each | points [n] (if PTS_SMEM)
+    float *cand_t = reinterpret_cast<float *>(smem_raw + (size_t)c.nrows * kRowBytes);
+    uint32_t *cand_c = reinterpret_cast<uint32_t *>(cand_t + nw * 32);
+    float *post_v = reinterpret_cast<float *>(cand_c + nw * 32);
+    uint32_t *post_k = reinterpret_cast<uint32_t *>(post_v + nw * 32);
+    PointRec *pts_s = reinterpret_cast<PointRec *>(post_k + nw * 32);
 
-    const int64_t curve_local = blockIdx.x / a.items_per_curve;
-    const int item = blockIdx.x % a.items_per_curve;
-    const int64_t cv = a.curve_base + curve_local;
-    const int64_t beg = a.offsets[cv];
-    c.n = (int)(a.offsets[cv + 1] - beg);
-    const CurveMeta meta = a.meta[cv];
-    const int ntiles = (a.nf + kTileFreqs - 1) / kTileFreqs;
-    const int tile0 = item * a.tiles_per_item;
-    const int tile1 = min(tile0 + a.tiles_per_item, ntiles);
-    const OutPtrs out = out_rows(a, curve_local, cv);
-
-    if (meta.status != BLS_CURVE_OK) {
-        zero_fill_outputs(out, tile0 * kTileFreqs, min(tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
+    if (w.meta.status != BLS_CURVE_OK) {
+        zero_fill_outputs(w.out, w.tile0 * kTileFreqs, min(w.tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
         return;
     }
-
-    // ---- a1 Load: the curve becomes resident for every tile of this work item -------------------
-    const PointRec *pts_g = a.pts + beg;
-    if (PTS_SMEM) {
-        const uint4 *src = reinterpret_cast<const uint4 *>(pts_g);
-        uint4 *dst = reinterpret_cast<uint4 *>(pts_s);
-        for (int i = tid; i < c.n; i += nthr) dst[i] = __ldg(src + i);
-    }
+    const PointRec *pts_g = a.pts + w.beg;
+    stage_curve<PTS_SMEM>(pts_g, pts_s, c.n, tid, nthr);
     const uint32_t bins_s = smem_u32(smem_raw), pts_sa = smem_u32(pts_s);
-    c.force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
-    c.cw = meta.cw; c.cy = meta.cy; c.wx2 = (float)meta.wx2;
-    c.G = (uint32_t)a.nb + 8u;                    // guard band, units of 2^-32 bin
     unsigned int n_canon = 0;
 
-    for (int tile = tile0; tile < tile1; ++tile) {
+    for (int tile = w.tile0; tile < w.tile1; ++tile) {
         const int q0 = tile * kTileFreqs;
         const double f = a.freqs[min(q0 + lane, a.nf - 1)];   // ragged last tile: surplus lanes repeat the last f
         zero_bins(bins_s, c.nb, tid, nthr);
         __syncthreads();
         fold_tile<PTS_SMEM>(c, f, bins_s, pts_sa, pts_g, lane, warp, nw, n_canon);
         __syncthreads();
-        convert_rows(c, bins_s, lane, warp, nw);
+        extend_rows(c, bins_s, tid, nthr);
         __syncthreads();
-        // ---- a3/a4 box search: this thread owns start tiles warp, warp+nw, ... of column `lane` --
-        {
-            float t_best; uint32_t key_best;
-            search_column<S>(bins_s + lane * 8, c.nb, c.kmin, c.kmax, warp, nw, t_best, key_best);
-            red_v[warp * 32 + lane] = t_best;
-            red_key[warp * 32 + lane] = key_best;
-        }
+        search_warp(bins_s, c, lane, warp, nw, cand_t, cand_c);
         __syncthreads();
-        if (warp < 4 && (lane >> 3) == warp)      // 4 warps x 8 columns
-            merge_column(c, rows2, red_v, red_key, nw, lane, q0 + lane, a.nf, out);
+        merge_tile(c, bins_s, cand_t, cand_c, post_v, post_k, nw, nw, warp, lane, q0 + lane, a.nf, w.out,
+                   [] { __syncthreads(); });
         __syncthreads();
     }
     count_canonical(a, n_canon, lane);
 }
 
-// ---- kernel 2: warp-specialised, double-buffered.  The fold is bound by the LSU pipe (shared
-//      atomics + point broadcasts), the box search by the XU pipe (one MUFU.RSQ per box): run
-//      them CONCURRENTLY on different warps so the SM is busy for max(fold, search), not their
-//      sum.  "Fold warps" zero / fold / convert tile i+1 (and merge tile i-1) into one bin buffer
-//      while "search warps" walk the boxes of tile i in the other.  Hand-off by named barriers
-//      (bar.arrive by the producer side, bar.sync by the consumer side). --------------------------
+// ---- kernel 2: warp-specialised, double-buffered.  The fold is bound by the shared-memory pipe
+//      (atomics + point broadcasts), the box search by the XU pipe (one MUFU.RSQ per box): they run
+//      CONCURRENTLY on different warps.  "Search warps" rank the boxes of tile i in one bin buffer
+//      while "fold warps" merge tile i-1 out of the other buffer and then zero / fold / extend tile
+//      i+1 into it.  Hand-off by named barriers (bar.arrive on the producing side, bar.sync on the
+//      consuming side): FULL[b] fold -> search, DONE[b] search -> fold; one barrier for the fold group.
 __device__ __forceinline__ void named_sync(int id, int count)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
@@ -672,105 +816,78 @@ __device__ __forceinline__ void named_arrive(int id, int count)
 }
 enum { kBarFull0 = 1, kBarFull1 = 2, kBarDone0 = 3, kBarDone1 = 4, kBarFoldGroup = 5 };
 
-template <bool PTS_SMEM, int S>
+template <bool PTS_SMEM>
 __global__ void __launch_bounds__(kWsMaxWarps * 32, 1)
 search_ws_kernel(const SearchArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nthr = blockDim.x;
-    const int nsw = a.search_warps, nfw = (nthr >> 5) - nsw;      // search warps come first
+    const int nsw = a.search_warps, nfw = (nthr >> 5) - nsw;      // search warps come first, then the fold warps
+    const int mw = min(nfw, kMergeWarps);
     TileCtx c;
-    c.nb = a.nb; c.kmin = a.kmin; c.kmax = a.kmax;
-    c.nrows = search_rows(a.nb, a.kmax);
-    // smem: bins[2] [nrows][256 B] | red_v[2] [nsw][32] | red_key[2] [nsw][32] | points [n]
+    const WorkItem w = work_item(a, c);
+    // smem: bins[2] [nrows][256 B] | cand_t[2], cand_c[2] [nsw][32] | post_v, post_k [kMergeWarps][32] | points [n]
     const size_t buf_bytes = (size_t)c.nrows * kRowBytes;
-    float *red_v = reinterpret_cast<float *>(smem_raw + 2 * buf_bytes);
-    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + 2 * nsw * 32);
-    PointRec *pts_s = reinterpret_cast<PointRec *>(red_key + 2 * nsw * 32);
+    float *cand_t = reinterpret_cast<float *>(smem_raw + 2 * buf_bytes);
+    uint32_t *cand_c = reinterpret_cast<uint32_t *>(cand_t + 2 * nsw * 32);
+    float *post_v = reinterpret_cast<float *>(cand_c + 2 * nsw * 32);
+    uint32_t *post_k = reinterpret_cast<uint32_t *>(post_v + kMergeWarps * 32);
+    PointRec *pts_s = reinterpret_cast<PointRec *>(post_k + kMergeWarps * 32);
 
-    const int64_t curve_local = blockIdx.x / a.items_per_curve;
-    const int item = blockIdx.x % a.items_per_curve;
-    const int64_t cv = a.curve_base + curve_local;
-    const int64_t beg = a.offsets[cv];
-    c.n = (int)(a.offsets[cv + 1] - beg);
-    const CurveMeta meta = a.meta[cv];
-    const int ntiles = (a.nf + kTileFreqs - 1) / kTileFreqs;
-    const int tile0 = item * a.tiles_per_item;
-    const int tile1 = min(tile0 + a.tiles_per_item, ntiles);
-    const OutPtrs out = out_rows(a, curve_local, cv);
-
-    if (meta.status != BLS_CURVE_OK) {
-        zero_fill_outputs(out, tile0 * kTileFreqs, min(tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
+    if (w.meta.status != BLS_CURVE_OK) {
+        zero_fill_outputs(w.out, w.tile0 * kTileFreqs, min(w.tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
         return;
     }
-
-    const PointRec *pts_g = a.pts + beg;
-    if (PTS_SMEM) {                               // a1 Load, by all warps
-        const uint4 *src = reinterpret_cast<const uint4 *>(pts_g);
-        uint4 *dst = reinterpret_cast<uint4 *>(pts_s);
-        for (int i = tid; i < c.n; i += nthr) dst[i] = __ldg(src + i);
-    }
+    const PointRec *pts_g = a.pts + w.beg;
+    stage_curve<PTS_SMEM>(pts_g, pts_s, c.n, tid, nthr);        // a1 Load, by all warps
     __syncthreads();
     const uint32_t bins_s = smem_u32(smem_raw), pts_sa = smem_u32(pts_s);
-    c.force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
-    c.cw = meta.cw; c.cy = meta.cy; c.wx2 = (float)meta.wx2;
-    c.G = (uint32_t)a.nb + 8u;
+    const int nt = w.tile1 - w.tile0;
 
     if (warp < nsw) {
-        // ================= search warps: a3/a4 only =================
-        for (int tile = tile0, it = 0; tile < tile1; ++tile, ++it) {
+        // ================= search warps: a3/a4 ranking only =================
+        for (int it = 0; it < nt; ++it) {
             const int b = it & 1;
-            named_sync(kBarFull0 + b, nthr);                      // buffer b holds tile's fp32 rows
-            float t_best; uint32_t key_best;
-            search_column<S>(bins_s + b * (uint32_t)buf_bytes + lane * 8, c.nb, c.kmin, c.kmax, warp, nsw, t_best, key_best);
-            red_v[(b * nsw + warp) * 32 + lane] = t_best;
-            red_key[(b * nsw + warp) * 32 + lane] = key_best;
-            named_arrive(kBarDone0 + b, nthr);                    // done with buffer b
+            named_sync(kBarFull0 + b, nthr);                      // buffer b holds the tile's integer rows
+            if (!(a.debug & 1)) search_warp(bins_s + b * (uint32_t)buf_bytes, c, lane, warp, nsw, cand_t + b * nsw * 32, cand_c + b * nsw * 32);
+            named_arrive(kBarDone0 + b, nthr);                    // candidates posted, done reading buffer b
         }
     } else {
-        // ================= fold warps: zero, a2 fold, convert, merge =================
+        // ================= fold warps: exact merge of tile i-2, then zero, a2 fold, cyclic extension =================
         const int gw = warp - nsw, gtid = tid - nsw * 32, gthreads = nfw * 32;
         unsigned int n_canon = 0;
-        auto merge = [&](int tile, int b) {
-            const int mw = min(nfw, 4), per = (32 + mw - 1) / mw;  // mw warps x ceil(32/mw) columns
-            if (gw < mw && lane / per == gw)
-                merge_column(c, reinterpret_cast<const float2 *>(smem_raw + b * buf_bytes), red_v + b * nsw * 32,
-                             red_key + b * nsw * 32, nsw, lane, tile * kTileFreqs + lane, a.nf, out);
-        };
-        for (int tile = tile0, it = 0; tile < tile1; ++tile, ++it) {
+        auto merge = [&](int it) {
             const int b = it & 1;
+            named_sync(kBarDone0 + b, nthr);
+            if (!(a.debug & 4)) merge_tile(c, bins_s + b * (uint32_t)buf_bytes, cand_t + b * nsw * 32, cand_c + b * nsw * 32, post_v, post_k, nsw, mw,
+                       gw, lane, (w.tile0 + it) * kTileFreqs + lane, a.nf, w.out,
+                       [gthreads] { named_sync(kBarFoldGroup, gthreads); });
+            named_sync(kBarFoldGroup, gthreads);                  // every column has left the buffer
+        };
+        for (int it = 0; it < nt; ++it) {
+            const int b = it & 1, tile = w.tile0 + it;
             const uint32_t buf = bins_s + b * (uint32_t)buf_bytes;
-            if (it >= 2) {                                        // tile-2 used this buffer: wait, then merge it
-                named_sync(kBarDone0 + b, nthr);
-                merge(tile - 2, b);
-                named_sync(kBarFoldGroup, gthreads);
-            }
+            if (it >= 2) merge(it - 2);
             const double f = a.freqs[min(tile * kTileFreqs + lane, a.nf - 1)];
             zero_bins(buf, c.nb, gtid, gthreads);
             named_sync(kBarFoldGroup, gthreads);
-            fold_tile<PTS_SMEM>(c, f, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
+            if (!(a.debug & 2)) fold_tile<PTS_SMEM>(c, f, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
             named_sync(kBarFoldGroup, gthreads);
-            convert_rows(c, buf, lane, gw, nfw);
+            extend_rows(c, buf, gtid, gthreads);
             named_arrive(kBarFull0 + b, nthr);
         }
-        // drain: the last (up to) two tiles
-        const int nt = tile1 - tile0;
-        for (int it = max(nt - 2, 0); it < nt; ++it) {
-            const int b = it & 1;
-            named_sync(kBarDone0 + b, nthr);
-            merge(tile0 + it, b);
-        }
+        for (int it = max(nt - 2, 0); it < nt; ++it) merge(it);   // drain
         count_canonical(a, n_canon, lane);
     }
 }
 
 // ---- kernel 3: one warp per tile.  For small shapes (C4: 200 epochs, 64 bins) a tile is a few
 //      thousand instructions and the hand-offs of kernels 1/2 cost more than the work.  Here every
-//      warp owns private bins and runs zero / fold / convert / search / merge of its own tiles with
+//      warp owns private bins and runs zero / fold / extend / search / merge of its own tiles with
 //      warp syncs only; warps of an SM sit in different phases, so the LSU-bound fold of one overlaps
 //      the XU-bound search of another without any CTA-level barrier. ------------------------------
-template <bool PTS_SMEM, int S>
+template <bool PTS_SMEM>
 __global__ void __launch_bounds__(kWtWarps * 32, 2)
 search_wt_kernel(const SearchArgs a)
 {
@@ -778,58 +895,36 @@ search_wt_kernel(const SearchArgs a)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nthr = blockDim.x, nw = nthr >> 5;
     TileCtx c;
-    c.nb = a.nb; c.kmin = a.kmin; c.kmax = a.kmax;
-    c.nrows = search_rows(a.nb, a.kmax);
-    // smem: per warp { bins [nrows][256 B] | red_v [32] | red_key [32] } ... | points [n]
+    const WorkItem w = work_item(a, c);
+    // smem: per warp { bins [nrows][256 B] | cand_t [32] | cand_c [32] } ... | points [n]
     const size_t per_warp = (size_t)c.nrows * kRowBytes + 256;
     unsigned char *mine = smem_raw + warp * per_warp;
-    float *red_v = reinterpret_cast<float *>(mine + (size_t)c.nrows * kRowBytes);
-    uint32_t *red_key = reinterpret_cast<uint32_t *>(red_v + 32);
+    float *cand_t = reinterpret_cast<float *>(mine + (size_t)c.nrows * kRowBytes);
+    uint32_t *cand_c = reinterpret_cast<uint32_t *>(cand_t + 32);
     PointRec *pts_s = reinterpret_cast<PointRec *>(smem_raw + nw * per_warp);
 
-    const int64_t curve_local = blockIdx.x / a.items_per_curve;
-    const int item = blockIdx.x % a.items_per_curve;
-    const int64_t cv = a.curve_base + curve_local;
-    const int64_t beg = a.offsets[cv];
-    c.n = (int)(a.offsets[cv + 1] - beg);
-    const CurveMeta meta = a.meta[cv];
-    const int ntiles = (a.nf + kTileFreqs - 1) / kTileFreqs;
-    const int tile0 = item * a.tiles_per_item;
-    const int tile1 = min(tile0 + a.tiles_per_item, ntiles);
-    const OutPtrs out = out_rows(a, curve_local, cv);
-
-    if (meta.status != BLS_CURVE_OK) {
-        zero_fill_outputs(out, tile0 * kTileFreqs, min(tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
+    if (w.meta.status != BLS_CURVE_OK) {
+        zero_fill_outputs(w.out, w.tile0 * kTileFreqs, min(w.tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
         return;
     }
-    const PointRec *pts_g = a.pts + beg;
-    if (PTS_SMEM) {
-        const uint4 *src = reinterpret_cast<const uint4 *>(pts_g);
-        uint4 *dst = reinterpret_cast<uint4 *>(pts_s);
-        for (int i = tid; i < c.n; i += nthr) dst[i] = __ldg(src + i);
-    }
+    const PointRec *pts_g = a.pts + w.beg;
+    stage_curve<PTS_SMEM>(pts_g, pts_s, c.n, tid, nthr);
     __syncthreads();                              // the only CTA barrier
     const uint32_t buf = smem_u32(mine), pts_sa = smem_u32(pts_s);
-    c.force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
-    c.cw = meta.cw; c.cy = meta.cy; c.wx2 = (float)meta.wx2;
-    c.G = (uint32_t)a.nb + 8u;
     unsigned int n_canon = 0;
 
-    for (int tile = tile0 + warp; tile < tile1; tile += nw) {
+    for (int tile = w.tile0 + warp; tile < w.tile1; tile += nw) {
         const int q0 = tile * kTileFreqs;
         const double f = a.freqs[min(q0 + lane, a.nf - 1)];
         zero_bins(buf, c.nb, lane, 32);
         __syncwarp();
         fold_tile<PTS_SMEM, 2>(c, f, buf, pts_sa, pts_g, lane, 0, 1, n_canon);
         __syncwarp();
-        convert_rows(c, buf, lane, 0, 1);
+        extend_rows(c, buf, lane, 32);
         __syncwarp();
-        float t_best; uint32_t key_best;
-        search_column<S>(buf + lane * 8, c.nb, c.kmin, c.kmax, 0, 1, t_best, key_best);
-        red_v[lane] = t_best;
-        red_key[lane] = key_best;
+        search_warp(buf, c, lane, 0, 1, cand_t, cand_c);
         __syncwarp();
-        merge_column(c, reinterpret_cast<const float2 *>(mine), red_v, red_key, 1, lane, q0 + lane, a.nf, out);
+        merge_tile(c, buf, cand_t, cand_c, nullptr, nullptr, 1, 1, 0, lane, q0 + lane, a.nf, w.out, [] {});
         __syncwarp();
     }
     count_canonical(a, n_canon, lane);
@@ -849,23 +944,20 @@ __global__ void debug_bins_kernel(const double *__restrict__ f, const double *__
 }
 
 cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int nb, int force_canon,
-                              int32_t *bins, unsigned long long *n_canon, cudaStream_t st)
+                              int32_t *bins, unsigned long long *n_canon, int sm_count, cudaStream_t st)
 {
     if (n <= 0) return cudaSuccess;
     int64_t blocks = (n + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > (int64_t)sm_count * 16) blocks = (int64_t)sm_count * 16;
     debug_bins_kernel<<<(unsigned)blocks, 256, 0, st>>>(f, t, n, nb, force_canon, bins, n_canon);
     return cudaGetLastError();
 }
 
 cudaError_t search_configure(int max_smem_optin)
 {
-    const void *fns[] = {(const void *)search_kernel<true, 4>,    (const void *)search_kernel<false, 4>,
-                         (const void *)search_kernel<true, 5>,    (const void *)search_kernel<false, 5>,
-                         (const void *)search_ws_kernel<true, 4>, (const void *)search_ws_kernel<false, 4>,
-                         (const void *)search_ws_kernel<true, 5>, (const void *)search_ws_kernel<false, 5>,
-                         (const void *)search_wt_kernel<true, 4>, (const void *)search_wt_kernel<false, 4>,
-                         (const void *)search_wt_kernel<true, 5>, (const void *)search_wt_kernel<false, 5>};
+    const void *fns[] = {(const void *)search_kernel<true>,    (const void *)search_kernel<false>,
+                         (const void *)search_ws_kernel<true>, (const void *)search_ws_kernel<false>,
+                         (const void *)search_wt_kernel<true>, (const void *)search_wt_kernel<false>};
     for (const void *f : fns) {
         cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
         if (e != cudaSuccess) return e;
@@ -879,15 +971,10 @@ cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem
     if (grid <= 0) return cudaSuccess;
     if (grid > 2147483647LL) return cudaErrorInvalidConfiguration;
     const unsigned g = (unsigned)grid;
-#define BLS_LAUNCH(K)                                                                   \
-    do {                                                                                \
-        if (a.starts_per_thread == 5) {                                                 \
-            if (a.pts_in_smem) K<true, 5><<<g, a.threads, smem, st>>>(a);               \
-            else K<false, 5><<<g, a.threads, smem, st>>>(a);                            \
-        } else {                                                                        \
-            if (a.pts_in_smem) K<true, 4><<<g, a.threads, smem, st>>>(a);               \
-            else K<false, 4><<<g, a.threads, smem, st>>>(a);                            \
-        }                                                                               \
+#define BLS_LAUNCH(K)                                                  \
+    do {                                                               \
+        if (a.pts_in_smem) K<true><<<g, a.threads, smem, st>>>(a);     \
+        else K<false><<<g, a.threads, smem, st>>>(a);                  \
     } while (0)
     if (a.kernel == 3) BLS_LAUNCH(search_wt_kernel);
     else if (a.kernel == 2) BLS_LAUNCH(search_ws_kernel);

@@ -33,22 +33,31 @@ constexpr int kThreads = 1024;
 constexpr int kIters = 2048;
 
 enum Test { ATOMS_CF, ATOMS_RAND, LDS128_BCAST, LDS32_CF, MUFU_RSQ, FADD, FADD2, FFMA, FFMA2, FMNMX3, DFMA, IMAD_WIDE,
-            FOLD_MIX, BOX_MIX, BOX_MIX2, ATOMS_CF2, LDS64_BCAST, LDS32_BCAST, LDS64_CF, N_TESTS };
+            FOLD_MIX, BOX_MIX, BOX_MIX2, ATOMS_CF2, LDS64_BCAST, LDS32_BCAST, LDS64_CF, I2FP, MUFU_I2FP, FMUL2, BOX_PACKED, BOX_PACKED_CVT, N_TESTS };
 static const char *kNames[N_TESTS] = {"atoms_add_cf", "atoms_add_rand", "lds128_bcast", "lds32_cf", "mufu_rsq", "fadd",
                                       "fadd2", "ffma", "ffma2", "fmnmx3", "dfma", "imad_wide", "fold_mix", "box_mix",
-                                      "box_mix_fadd2", "atoms_add_cf_min", "lds64_bcast", "lds32_bcast", "lds64_cf"};
+                                      "box_mix_fadd2", "atoms_add_cf_min", "lds64_bcast", "lds32_bcast", "lds64_cf", "i2fp",
+                                      "mufu_plus_i2fp", "fmul2", "box_packed", "box_packed_cvt"};
 // lane-operations each thread performs per inner iteration (what the rate is quoted in)
-static const double kOpsPerIter[N_TESTS] = {8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 4, 8, 8, 8, 8, 8, 8};
+static const double kOpsPerIter[N_TESTS] = {8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 4, 8, 8, 8, 8, 8, 8, 8, 8, 8, 14, 14};
 static const char *kUnit[N_TESTS] = {"ATOMS lane-ops", "ATOMS lane-ops", "LDS.128 lane-loads", "LDS.32 lane-loads",
                                      "MUFU lane-ops", "FADD lane-ops", "FADD2 lane-instr (2 adds each)", "FFMA lane-ops",
                                      "FFMA2 lane-instr (2 fmas each)", "FMNMX3 lane-ops (+1/8 FADD)", "DFMA lane-ops",
-                                     "IMAD.WIDE lane-ops", "point-folds", "boxes", "boxes", "ATOMS lane-ops", "LDS.64 lane-loads", "LDS.32 lane-loads", "LDS.64 lane-loads"};
+                                     "IMAD.WIDE lane-ops", "point-folds", "boxes", "boxes", "ATOMS lane-ops", "LDS.64 lane-loads", "LDS.32 lane-loads", "LDS.64 lane-loads",
+                                     "I2FP lane-ops", "MUFU lane-ops (each with one I2FP beside it)", "FMUL2 lane-instr (2 muls each)",
+                                     "boxes (packed f32x2 search mix, rows already fp32)", "boxes (packed f32x2 search mix, int rows converted on the fly)"};
 
 __device__ __forceinline__ float rsq(float x) { float y; asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ unsigned long long add2(unsigned long long a, unsigned long long b)
 { unsigned long long c; asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(c) : "l"(a), "l"(b)); return c; }
 __device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c)
 { unsigned long long d; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ unsigned long long mul2(unsigned long long a, unsigned long long b)
+{ unsigned long long c; asm volatile("mul.rn.f32x2 %0, %1, %2;" : "=l"(c) : "l"(a), "l"(b)); return c; }
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
+{ unsigned long long v; asm("mov.b64 %0, {%1, %2};" : "=l"(v) : "f"(lo), "f"(hi)); return v; }
+__device__ __forceinline__ void unpack2(unsigned long long v, float &lo, float &hi)
+{ asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
 __device__ __forceinline__ float fmax3(float a, float b, float c) { return fmaxf(fmaxf(a, b), c); }
 
 template <int T>
@@ -156,6 +165,44 @@ __global__ void __launch_bounds__(kThreads, 1) bench(long long *cycles, float *s
             p0 = add2(p0, p1); p0 = add2(p0, p1);   // stand-ins for the 4th start: keeps the mix at 8 boxes
             { float r = __uint_as_float((uint32_t)p0), s = __uint_as_float((uint32_t)(p0 >> 32));
               float t = fabsf(s) * rsq(fmaf(-r, r, r)); float t2 = fabsf(s + y) * rsq(fmaf(-(r + w), r + w, r + w)); f6 = fmax3(f6, t, t2); }
+        } else if (T == I2FP) {
+            f0 = __int2float_rn(__float_as_int(f0)); f1 = __int2float_rn(__float_as_int(f1)); f2 = __int2float_rn(__float_as_int(f2));
+            f3 = __int2float_rn(__float_as_int(f3)); f4 = __int2float_rn(__float_as_int(f4)); f5 = __int2float_rn(__float_as_int(f5));
+            f6 = __int2float_rn(__float_as_int(f6)); f7 = __int2float_rn(__float_as_int(f7));
+        } else if (T == MUFU_I2FP) {
+            f0 = rsq(__int2float_rn(__float_as_int(f0))); f1 = rsq(__int2float_rn(__float_as_int(f1)));
+            f2 = rsq(__int2float_rn(__float_as_int(f2))); f3 = rsq(__int2float_rn(__float_as_int(f3)));
+            f4 = rsq(__int2float_rn(__float_as_int(f4))); f5 = rsq(__int2float_rn(__float_as_int(f5)));
+            f6 = rsq(__int2float_rn(__float_as_int(f6))); f7 = rsq(__int2float_rn(__float_as_int(f7)));
+        } else if (T == FMUL2) {
+            p0 = mul2(p0, pm); p1 = mul2(p1, pm); p2 = mul2(p2, pm); p3 = mul2(p3, pm);
+            p4 = mul2(p4, pm); p5 = mul2(p5, pm); p6 = mul2(p6, pm); p7 = mul2(p7, pm);
+        } else if (T == BOX_PACKED || T == BOX_PACKED_CVT) {
+            // one bin row -> 7 starts x 2 frequencies = 14 boxes: per box pair FFMA2 (n -= W c), FADD2, FFMA2 (n^2 + n),
+            // 2 MUFU.RSQ, FMUL2, and one FMNMX3 per two box pairs and frequency
+            const uint2 wi = *reinterpret_cast<const uint2 *>(sm + (it % nb) * 64 + (lane & 15) * 2);
+            const uint2 yi = *reinterpret_cast<const uint2 *>(sm + (it % nb) * 64 + 32 + (lane & 15) * 2);
+            unsigned long long W, Y;
+            if (T == BOX_PACKED_CVT) {
+                W = pack2(__uint2float_rn(wi.x), __uint2float_rn(wi.y));
+                Y = pack2(__int2float_rn((int)yi.x), __int2float_rn((int)yi.y));
+            } else {
+                W = ((unsigned long long)(wi.y & 0x3fffffffu) << 32) | (wi.x & 0x3fffffffu);
+                Y = ((unsigned long long)(yi.y & 0x3fffffffu) << 32) | (yi.x & 0x3fffffffu);
+            }
+            unsigned long long *rn = q;                 // q[0..6] = n, p0..p6 = s
+            unsigned long long rs[7] = {p0, p1, p2, p3, p4, p5, p6};
+#pragma unroll
+            for (int u = 0; u < 7; ++u) {
+                rn[u] = fma2(W, pm, rn[u]);
+                rs[u] = add2(rs[u], Y);
+                const unsigned long long d = fma2(rn[u], rn[u], rn[u]);
+                float d0, d1; unpack2(d, d0, d1);
+                const unsigned long long t = mul2(rs[u], pack2(rsq(fabsf(d0)), rsq(fabsf(d1))));
+                float t0, t1; unpack2(t, t0, t1);
+                f6 = fmaxf(f6, fabsf(t0)); f7 = fmaxf(f7, fabsf(t1));
+            }
+            p0 = rs[0]; p1 = rs[1]; p2 = rs[2]; p3 = rs[3]; p4 = rs[4]; p5 = rs[5]; p6 = rs[6];
         } else if (T == BOX_MIX2) {
             // 8 boxes with packed (r, s) running sums: FADD2, FFMA, MUFU, FMUL, 1/2 FMNMX3 per box
             const unsigned long long wy = ((unsigned long long)sm[(it % nb) * 64 + lane] << 32) | 0x2b8cbccbu;
@@ -233,5 +280,10 @@ int main()
     run<LDS64_BCAST>(n_sm, nb, d_cyc, d_sink);
     run<LDS32_BCAST>(n_sm, nb, d_cyc, d_sink);
     run<LDS64_CF>(n_sm, nb, d_cyc, d_sink);
+    run<I2FP>(n_sm, nb, d_cyc, d_sink);
+    run<MUFU_I2FP>(n_sm, nb, d_cyc, d_sink);
+    run<FMUL2>(n_sm, nb, d_cyc, d_sink);
+    run<BOX_PACKED>(n_sm, nb, d_cyc, d_sink);
+    run<BOX_PACKED_CVT>(n_sm, nb, d_cyc, d_sink);
     return 0;
 }
