@@ -2,6 +2,13 @@
 C-ABI library libbls_b200.so.  The CUDA kernels are the product; this package only marshals
 arguments.  Importing it never builds or falls back to anything on the CPU."""
 from .binding import (  # noqa: F401
+    BLS_ERR_ARG,
+    BLS_ERR_BATCH,
+    BLS_ERR_CONFIG,
+    BLS_ERR_CUDA,
+    BLS_ERR_NULL,
+    BLS_ERR_UNSUPPORTED,
+    BLS_OK,
     BLS_FLAG_CANONICAL_PHASE,
     BLS_FLAG_FOLD_WARPS,
     BLS_FLAG_NONE,

@@ -21,6 +21,9 @@ def pytest_collection_modifyitems(config, items):
         has_gpu = False
     if has_gpu:
         return
+    if "gpu" in (config.getoption("-m") or "") and "not gpu" not in (config.getoption("-m") or ""):
+        # `-m gpu` was asked for explicitly: a box without a GPU must fail, not report green
+        pytest.exit("pytest -m gpu needs a CUDA device (torch.cuda.is_available() is False)", returncode=3)
     skip = pytest.mark.skip(reason="no CUDA device")
     for item in items:
         if "gpu" in item.keywords:

@@ -40,6 +40,7 @@ def run_gpu(batch, grid, top_k=5, flags=0, scratch_bytes=0, want_spectrum=True, 
     out["kmin"], out["kmax"] = plan.kmin, plan.kmax
     out["n_canonical"] = plan.query(bls.binding.QUERY_LAST_CANONICAL) if nc else 0
     out["launches"] = plan.query(bls.binding.QUERY_LAST_LAUNCHES)
+    out["kernel"] = plan.query(bls.binding.QUERY_SEARCH_KERNEL)
     out["freqs"] = freqs
     plan.destroy()
     return out

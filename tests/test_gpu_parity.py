@@ -9,13 +9,25 @@ import pytest
 
 import oracle
 import synth
-from comparator import compare_peaks, compare_spectrum
+from comparator import compare_peaks, compare_spectrum, exact_tie_runs
 from gpu_common import run_gpu
 
 pytestmark = pytest.mark.gpu
 
 
-def check_config(name, curve_ids=None, flags=0, scratch_bytes=0):
+def check_curve_peaks(t, freqs, nb, orc, pk, k, g_sr_row, label):
+    """Peak list of one curve against the oracle: first against R14 on the oracle's raw spectrum; if
+    that differs, the exact ties around it are PROVEN from the member sets and the list must equal R14
+    on the tie-collapsed spectrum (tests/comparator.py)."""
+    _, o_sr, o_a, o_k, _ = orc
+    if np.array_equal(oracle.peaks(o_sr, k), pk["freq_index"]):
+        compare_peaks(o_sr, pk["freq_index"], pk["sr"], k, label=label, g_spectrum=g_sr_row)
+        return dict(exact_tie_slots=0, near_tie_slots=0)
+    ties, _ = exact_tie_runs(t, freqs, nb, o_sr, o_a, o_k)
+    return compare_peaks(o_sr, pk["freq_index"], pk["sr"], k, label=label, g_spectrum=g_sr_row, ties=ties)
+
+
+def check_config(name, curve_ids=None, flags=0, scratch_bytes=0, max_near_tie_frac=0.01):
     cfg = synth.config(name)
     grid = cfg["grid"]
     batch = synth.make_batch(cfg, curve_ids)
@@ -24,14 +36,15 @@ def check_config(name, curve_ids=None, flags=0, scratch_bytes=0):
     assert (g["kmin"], g["kmax"]) == oracle.widths(grid.nb, grid.qmin, grid.qmax)
     assert (g["status"] == 0).all()
     freqs = g["freqs"]
-    rep = dict(max_rel_err=0.0, box_near_ties=0, peak_near_ties=0, worst_tie_gap=0.0, n=0)
+    orcs, _ = oracle.spectrum_batch(batch.offsets, batch.t, batch.mag, batch.sigma, freqs, grid.nb, g["kmin"], g["kmax"])
+    rep = dict(max_rel_err=0.0, box_near_ties=0, exact_tie_slots=0, near_tie_slots=0, worst_tie_gap=0.0, n=0, slots=0)
     for c in range(batch.n_curves):
         t, mag, sig = batch.curve(c)
+        label = "%s curve %d" % (name, int(batch.curve_ids[c]))
         r = compare_spectrum(t, mag, sig, freqs, grid.nb, g["kmin"], g["kmax"],
-                             g["sr"][c], g["a"][c], g["k"][c], g["depth"][c], label="%s curve %d" % (name, c))
-        o_sr = r["oracle"][1]
+                             g["sr"][c], g["a"][c], g["k"][c], g["depth"][c], orc=orcs[c], label=label)
         pk = g["peaks"][c]
-        pr = compare_peaks(o_sr, pk["freq_index"], pk["sr"], k, label="%s curve %d" % (name, c), g_spectrum=g["sr"][c])
+        pr = check_curve_peaks(t, freqs, grid.nb, orcs[c], pk, k, g["sr"][c], label)
         # the peak records repeat the spectrum's values at their index
         for p in pk:
             if p["freq_index"] >= 0:
@@ -44,13 +57,18 @@ def check_config(name, curve_ids=None, flags=0, scratch_bytes=0):
         rep["max_rel_err"] = max(rep["max_rel_err"], r["max_rel_err"])
         rep["worst_tie_gap"] = max(rep["worst_tie_gap"], r["worst_tie_gap"])
         rep["box_near_ties"] += r["box_near_ties"]
-        rep["peak_near_ties"] += pr["peak_near_ties"]
+        rep["exact_tie_slots"] += pr["exact_tie_slots"]
+        rep["near_tie_slots"] += pr["near_tie_slots"]
         rep["n"] += len(freqs)
-    print("\n[parity %s] %d (curve,freq) pairs: max SR rel err %.3g, box near-ties %d (worst gap %.3g), "
-          "peak near-ties %d, canonical-rule point-folds %d" % (name, rep["n"], rep["max_rel_err"],
-          rep["box_near_ties"], rep["worst_tie_gap"], rep["peak_near_ties"], g["n_canonical"]))
-    # near-ties must stay rare (exact same-point-set ties resolve canonically on both sides)
-    assert rep["box_near_ties"] <= max(3, 0.01 * rep["n"])
+        rep["slots"] += k
+    print("\n[parity %s] %d curves, %d (curve,freq) pairs: max SR rel err %.3g; box near-ties %d (worst gap %.3g); "
+          "peak slots %d: %d explained by a proven exact tie, %d near-ties inside 2e-6, 0 unexplained; "
+          "canonical-rule point-folds %d" % (name, batch.n_curves, rep["n"], rep["max_rel_err"], rep["box_near_ties"],
+          rep["worst_tie_gap"], rep["slots"], rep["exact_tie_slots"], rep["near_tie_slots"], g["n_canonical"]))
+    # near-ties (different point sets whose SR differ by < 1e-6: the fp32 ranking may take either) must stay
+    # rare; a near-tie that persists along a plateau can move a peak slot, so those are rare as well
+    assert rep["box_near_ties"] <= max(3, 1e-4 * rep["n"])
+    assert rep["near_tie_slots"] <= max(2, max_near_tie_frac * rep["slots"])
     return g, rep
 
 
@@ -76,22 +94,87 @@ def test_small_shapes_without_the_warp_per_tile_kernel(name):
 
 
 def test_kernel_variants_give_identical_results():
-    """Warp counts and kernel choice are tuning only.  Bins are exact integers and every box is scored by
-    the same instructions, so spectra agree to rounding; they are not bitwise equal because boxes whose
-    approximate rank (MUFU.RSQ) ties exactly are merged in warp order."""
+    """Warp counts and kernel choice are tuning only.  Bins are exact integers and the reported SR /
+    depth are computed from the integer sums of the chosen box, so wherever two variants choose the
+    same box the outputs are bitwise equal; they may choose different boxes only where the approximate
+    ranks of two boxes tie (different grouping of the starts), i.e. at near-ties."""
     import paper_1112_1701_b200 as bls
     cfg = synth.config("T1")
     batch = synth.make_batch(cfg)
     ref = run_gpu(batch, cfg["grid"], top_k=5)
-    for flags in (bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_NO_WARP_PER_TILE,
-                  bls.BLS_FLAG_NO_WARP_PER_TILE | bls.BLS_FLAG_WARPS(6) | bls.BLS_FLAG_FOLD_WARPS(3),
-                  bls.BLS_FLAG_WARPS(7) | bls.BLS_FLAG_SINGLE_BUFFER,
-                  bls.BLS_FLAG_NO_WARP_PER_TILE | bls.BLS_FLAG_WARPS(10) | bls.BLS_FLAG_FOLD_WARPS(1)):
+    variants = [bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_NO_WARP_PER_TILE,
+                bls.BLS_FLAG_NO_WARP_PER_TILE | bls.BLS_FLAG_WARPS(6) | bls.BLS_FLAG_FOLD_WARPS(3),
+                bls.BLS_FLAG_WARPS(7) | bls.BLS_FLAG_SINGLE_BUFFER,
+                bls.BLS_FLAG_NO_WARP_PER_TILE | bls.BLS_FLAG_WARPS(10) | bls.BLS_FLAG_FOLD_WARPS(1),
+                bls.BLS_FLAG_NO_WARP_PER_TILE | bls.BLS_FLAG_WARPS(1) | bls.BLS_FLAG_FOLD_WARPS(2)]
+    variants += [bls.BLS_FLAG_WARPS(n) | bls.BLS_FLAG_SINGLE_BUFFER for n in (1, 2, 3)]   # ADVICE r1: fewer than 4 warps
+    for flags in variants:
         g = run_gpu(batch, cfg["grid"], top_k=5, flags=flags)
         np.testing.assert_allclose(g["sr"], ref["sr"], rtol=2e-6, atol=0)
         same = (g["a"] == ref["a"]) & (g["k"] == ref["k"])
         assert same.mean() > 0.999
         assert (g["sr"] == ref["sr"])[same].all() and (g["depth"] == ref["depth"])[same].all()
+
+
+def test_kernel_selection_per_configuration_and_shape_limit():
+    """Which search kernel bls_run picks by itself (BLS_QUERY_SEARCH_KERNEL): the warp-specialised one for
+    C0-C3 shapes, one warp per tile for C4, the single-buffer one where two bin buffers do not fit
+    (nb = 512, q_max = 0.1) -- checked against the oracle there -- and BLS_ERR_UNSUPPORTED beyond the
+    shared-memory limit bls.h states."""
+    import torch
+    import paper_1112_1701_b200 as bls
+    from paper_1112_1701_b200 import binding as B
+    dev = torch.device("cuda", 0)
+    want = {"C0": 2, "C1": 2, "C2": 2, "C3": 2, "C4": 3, "T0": 2, "T1": 3, "T2": 2}
+    for name, kern in want.items():
+        cfg = synth.config(name)
+        grid = cfg["grid"]
+        batch = synth.make_batch(cfg, [0])
+        with bls.Plan(n_bins=grid.nb, q_min=grid.qmin, q_max=grid.qmax, freqs=synth.freq_grid(grid)[:64], max_top_k=2) as plan:
+            plan.run(batch.offsets, torch.from_numpy(batch.t).to(dev), torch.from_numpy(batch.mag).to(dev),
+                     torch.from_numpy(batch.sigma).to(dev))
+            torch.cuda.synchronize()
+            assert plan.query(B.QUERY_SEARCH_KERNEL) == kern, name
+    # nb = 512, widths 1..52: two buffers need 2 * 571 rows * 256 B > 227 KB -> kernel 1 on its own
+    rng = np.random.default_rng(31)
+    n = 900
+    t = np.sort(rng.integers(0, 50, n) + rng.uniform(0, 0.3, n))
+    mag = 15 + rng.normal(0, 0.02, n) + 0.06 * ((((t - 0.1) / 1.37) % 1.0) < 0.05)
+    b = _batch([(t, mag, rng.uniform(0.01, 0.03, n))])
+    grid = synth.Grid(70, 0.3, 1.2, 512, 0.004, 0.1)
+    g = run_gpu(b, grid, top_k=3)
+    assert g["kernel"] == 1 and (g["kmin"], g["kmax"]) == (2, 52)
+    tt, mm, ss = b.curve(0)
+    r = compare_spectrum(tt, mm, ss, g["freqs"], grid.nb, g["kmin"], g["kmax"], g["sr"][0], g["a"][0], g["k"][0], g["depth"][0])
+    compare_peaks(r["oracle"][1], g["peaks"][0]["freq_index"], g["peaks"][0]["sr"], 3, g_spectrum=g["sr"][0])
+    # the limit: (nb + kmax + 7) rows of 256 B plus the candidate area must fit 227 KB
+    f = np.array([0.5, 0.6])
+    with bls.Plan(n_bins=800, q_min=0.01, q_max=0.1, freqs=f) as plan:       # 800 + 80 + 7 rows: fits
+        assert plan.kmax == 80
+    with pytest.raises(bls.BlsError) as ei:
+        bls.Plan(n_bins=1024, q_min=0.01, q_max=0.1, freqs=f)
+    assert ei.value.code == bls.BLS_ERR_UNSUPPORTED
+
+
+def test_low_weight_outlier_and_boxes_holding_almost_all_the_weight():
+    """one point with a very large sigma (tiny weight) outside a box that holds everything
+    else: r = 1 - 1e-7.  fp32 r(1-r) is useless there; the exact integer merge must give the oracle's
+    value (the complement's SR).  Clustered phases at low frequency make such boxes reachable."""
+    rng = np.random.default_rng(77)
+    n = 80
+    t = np.sort(rng.uniform(0.0, 0.12, n))                 # one short night: everything within a few bins
+    t[-1] = 0.7                                            # the outlier, half a cycle away at f ~ 0.7
+    mag = 15 + rng.normal(0, 0.02, n)
+    mag[-1] += 0.5
+    sig = np.full(n, 0.02)
+    sig[-1] = 20.0                                         # weight 1e-6 of the others
+    b = _batch([(t, mag, sig)])
+    grid = synth.Grid(41, 0.3, 0.9, 32, 0.05, 0.5)
+    g = run_gpu(b, grid, top_k=2)
+    assert np.isfinite(g["sr"]).all() and np.isfinite(g["depth"]).all()
+    tt, mm, ss = b.curve(0)
+    r = compare_spectrum(tt, mm, ss, g["freqs"], grid.nb, g["kmin"], g["kmax"], g["sr"][0], g["a"][0], g["k"][0], g["depth"][0])
+    assert (r["oracle"][1] > 0).any()
 
 
 def test_c0_whole():
@@ -104,9 +187,13 @@ def test_c0_whole():
     assert top["depth"] == pytest.approx(0.05, rel=0.25)
 
 
-def test_c1_subset_all_frequencies():
-    """configs[1] shapes (1,500 epochs, 20,000 frequencies, 200 bins, widths 1..30) on 3 curves."""
-    check_config("C1", curve_ids=[0, 7, 500])
+def test_c1_128_curves_all_frequencies():
+    """configs[1] (1,500 epochs, 20,000 frequencies, 200 bins, widths 1..30): 128 curves spread over the
+    1,000 (">= 128"), every injected one among the first 600 included, at every frequency."""
+    cfg = synth.config("C1")
+    inj = [c for c in range(600) if synth.make_curve(cfg, c)[4] is not None]
+    ids = sorted(set(list(range(0, 1000, 8))[:128 - len(inj)] + inj))
+    check_config("C1", curve_ids=ids)
 
 
 def test_chunked_scratch_gives_identical_results():
@@ -312,77 +399,59 @@ def test_bin_indices_equal_the_oracles_on_many_pairs():
 # ---- BASELINE.json configs[2..4] at full size: the launch configuration bench.py times (full
 #      frequency grid, the library's own geometry), on sampled curves / sampled outputs ------------
 
-def _first_injected(cfg, limit):
-    for cid in range(limit):
-        if synth.make_curve(cfg, cid)[4] is not None:
-            return cid
-    return None
+def _injected(cfg, ids):
+    return [c for c in ids if synth.make_curve(cfg, int(c))[4] is not None]
 
 
-def check_peak_properties(g_sr, pk, k, label=""):
-    """Properties that hold at any size: peaks are local maxima of the spectrum they come from (R14),
-    ranked by SR then index, and no better local maximum was left out."""
-    idx = pk["freq_index"]
-    n = int((idx >= 0).sum())
-    assert np.all(idx[n:] == -1)
-    v = g_sr
-    nf = len(v)
-    is_pk = (v > 0) & np.concatenate(([True], v[1:] > v[:-1])) & np.concatenate((v[:-1] >= v[1:], [True]))
-    assert is_pk[idx[:n]].all(), label + " a reported peak is not a local maximum"
-    srs = v[idx[:n]]
-    assert np.array_equal(srs, pk["sr"][:n])
-    order = np.lexsort((idx[:n], -srs))
-    assert np.array_equal(order, np.arange(n)), label + " peaks not ranked"
-    rest = is_pk.copy()
-    rest[idx[:n]] = False
-    if n == k and rest.any():
-        assert v[rest].max() <= srs[-1], label + " a better local maximum was left out"
-    else:
-        assert n == min(k, int(is_pk.sum()))
-
-
-def test_c2_shape_ragged_lengths_all_frequencies():
-    """configs[2]: N in 500..4000, 50,000 frequencies, 200 bins, widths 1..30, top-5; three curves
-    (one of them injected) against the oracle at every frequency."""
+def test_c2_64_curves_stratified_over_length_all_frequencies():
+    """configs[2]: N in 500..4000, 50,000 frequencies, 200 bins, widths 1..30, top-5.  64 curves of the
+    first 2,000: every injected one among them, the rest stratified over N (8 strata),
+    against the oracle at every frequency."""
     cfg = synth.config("C2")
-    inj = _first_injected(cfg, 600)
-    ids = [0, 1] + ([inj] if inj is not None else [2])
+    pool = np.arange(2000)
+    inj = _injected(cfg, pool)
+    n = synth.curve_lengths(cfg, pool)
+    order = pool[np.argsort(n, kind="stable")]
+    strata = np.array_split(order, 8)
+    rest = []
+    j = 0
+    while len(rest) + len(inj) < 64:
+        for st in strata:
+            c = int(st[(j * 37) % len(st)])
+            if c not in inj and c not in rest and len(rest) + len(inj) < 64:
+                rest.append(c)
+        j += 1
+    ids = sorted(inj + rest)
+    lens = synth.curve_lengths(cfg, ids)
+    assert len(ids) == 64 and lens.min() < 1000 and lens.max() > 3500
     g, rep = check_config("C2", curve_ids=ids)
-    if inj is not None:
-        tr = synth.make_curve(cfg, inj)[4]
-        top = g["peaks"][2][0]
-        ratio = top["freq"] * tr["P"]
-        if tr["depth"] > 0.05:      # a deep eclipse: the top peak is the period or a harmonic of it
+    for c, cid in enumerate(ids):
+        tr = synth.make_curve(cfg, cid)[4]
+        if tr is not None and tr["depth"] > 0.05:      # a deep eclipse: the top peak is the period or a harmonic of it
+            ratio = g["peaks"][c][0]["freq"] * tr["P"]
             assert min(abs(ratio * m - round(ratio * m)) for m in (1, 2, 3, 4)) < 0.02
 
 
-def test_c3_shape_full_grid_sampled_frequencies():
-    """configs[3]: 5,000 epochs over two seasons, 500,000 frequencies, 400 bins, widths 1..40.  The
-    CUDA path runs the full grid (its launch configuration); the oracle scores every 193rd
-    frequency, element by element; the peak list is checked by its properties."""
+def test_c3_8_curves_full_grid_all_frequencies():
+    """configs[3]: 5,000 epochs over two seasons, 500,000 frequencies, 400 bins, widths 1..40.  Eight
+    curves (four injected, four not) against the oracle at ALL 500,000 frequencies."""
     cfg = synth.config("C3")
-    grid = cfg["grid"]
-    batch = synth.make_batch(cfg, [3])
-    g = run_gpu(batch, grid, top_k=cfg["top_k"])
-    assert (g["kmin"], g["kmax"]) == oracle.widths(grid.nb, grid.qmin, grid.qmax) == (1, 40)
-    assert g["status"][0] == 0
-    idx = np.arange(7, grid.nf, 193)
-    t, mag, sig = batch.curve(0)
-    r = compare_spectrum(t, mag, sig, g["freqs"][idx], grid.nb, g["kmin"], g["kmax"], g["sr"][0][idx],
-                         g["a"][0][idx], g["k"][0][idx], g["depth"][0][idx], label="C3 curve 3")
-    print("\n[parity C3] %d sampled frequencies of %d: max SR rel err %.3g, box near-ties %d" % (
-        len(idx), grid.nf, r["max_rel_err"], r["box_near_ties"]))
-    check_peak_properties(g["sr"][0], g["peaks"][0], cfg["top_k"], "C3")
-    assert np.isfinite(g["sr"]).all() and (g["sr"] >= 0).all()
-    assert (g["a"] < grid.nb).all() and (g["k"] >= 1).all() and (g["k"] <= 40).all()
+    inj = []
+    cid = 0
+    while len(inj) < 4:
+        if synth.make_curve(cfg, cid)[4] is not None:
+            inj.append(cid)
+        cid += 1
+    plain = [c for c in range(3, 200) if c not in inj][:4]
+    g, rep = check_config("C3", curve_ids=sorted(inj + plain))
+    assert (g["kmin"], g["kmax"]) == (1, 40)
 
 
-def test_c4_shape_many_short_curves():
-    """configs[4]: 200 epochs, 5,000 frequencies, 64 bins, widths 1..10; 96 curves at every frequency."""
-    cfg = synth.config("C4")
-    inj = _first_injected(cfg, 400)
-    ids = list(range(95)) + [inj if inj is not None else 95]
-    check_config("C4", curve_ids=ids)
+def test_c4_4096_short_curves():
+    """configs[4]: 200 epochs, 5,000 frequencies, 64 bins, widths 1..10; 4,096 curves at
+    every frequency.  This is the shape where exact plateaus are common (200 epochs in 64 bins)."""
+    g, rep = check_config("C4", curve_ids=list(range(4096)))
+    assert rep["exact_tie_slots"] > 0       # the tie proofs were exercised
 
 
 def test_handoff_stress_bitwise_repeatable_and_kernels_agree():
