@@ -1,18 +1,21 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the BLS hot path on B200 (BASELINE.json metric: point-folds/s, curves/s,
-fraction of the stated roofline), with the fp64 oracle timed beside it.
+fraction of the stated roofline), with the fp64 oracle timed beside it and compared with it.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C1] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2] [--impl ours|reference]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
-A "step" is one pass of the whole hot path (prep -> fold/search -> peaks -> top-k) over one batch of
-synthetic light curves of the chosen configuration (default C1 = BASELINE.json configs[1]: 1,000
-curves x 1,500 epochs, 20,000 frequencies, 200 bins).  Prints ONE JSON line (rank 0).
+A "step" is one pass of the whole hot path (prep -> fold/search/merge -> peaks -> top-k) over one batch
+of synthetic light curves of the chosen configuration.  The default is C2 = BASELINE.json configs[2]
+at FULL size (100,000 curves of 500-4,000 epochs, 50,000 frequencies, 200 bins, top-5): the largest
+configuration whose 20 timed steps fit the driver's bench arm.  Prints ONE JSON line (rank 0).
 
-  value      whole-job point-folds/s, inputs resident in HBM (CUDA events around bls_run + bls_topk)
-  e2e        the same metric through bls_search_host with pinned HOST buffers (H2D + D2H inside)
-  roofline   the search kernel against the issue-rate roofline stated in DESIGN.md
-  cpu_baseline  the oracle as it stands on the host cores, bounded sample
+  value        whole-job point-folds/s, inputs resident in HBM (CUDA events around bls_run + bls_topk)
+  e2e          the same metric through bls_search_host with pinned HOST buffers (H2D + D2H inside)
+  roofline     the search kernel against the issue-rate roofline stated in DESIGN.md section 7
+  cpu_baseline the oracle as it stands on the host cores, bounded sample, and the parity of the timed
+               step's peaks against it
+  per_config   C1, C3 (full) and C4 (full): one timed step each (after warm-up), same fields in short
 With --impl reference the oracle itself is the timed arm (rank 0 only).
 """
 from __future__ import annotations
@@ -35,12 +38,13 @@ METRIC = "bls_point_folds_per_sec"
 UNIT = "point-folds/s"
 
 # Roofline constants, measured on B200 by paper_1112_1701_b200/microbench/issue_rates.cu
-# (profiles/r01a_microbench.md): lane-operations per clock per SM.
-LSU_LANE_OPS_PER_CLK_SM = 32.0       # shared wavefront pipe: conflict-free ATOMS.ADD 31.96
+# (profiles/r02_microbench.md): lane-operations per clock per SM.
+LSU_LANE_OPS_PER_CLK_SM = 32.0       # shared wavefront pipe: conflict-free ATOMS.ADD 31.97
 XU_LANE_OPS_PER_CLK_SM = 16.0        # MUFU.RSQ 16.00: one per box
 ISSUE_LANE_INSTR_PER_CLK_SM = 128.0  # 4 schedulers x 32 lanes
-FOLD_MIN_INSTR, BOX_MIN_INSTR = 5.0, 4.5
-N_SM = 148
+# fewest instructions the method needs: fold = point load, DFMA, IMAD.WIDE, 2 ATOMS; box = 1/2 (FFMA2 + FADD2 +
+# FFMA2 + FMUL2 + FMNMX3) + MUFU with packed f32x2 arithmetic
+FOLD_MIN_INSTR, BOX_MIN_INSTR = 5.0, 3.5
 
 
 def pair_clocks(n_mean, nb, kmax, nk):
@@ -49,12 +53,8 @@ def pair_clocks(n_mean, nb, kmax, nk):
     t_xu = nb * nk / XU_LANE_OPS_PER_CLK_SM
     t_issue = (FOLD_MIN_INSTR * n_mean + BOX_MIN_INSTR * nb * nk) / ISSUE_LANE_INSTR_PER_CLK_SM
     t_sum = 2.0 * n_mean / LSU_LANE_OPS_PER_CLK_SM + nb * nk / XU_LANE_OPS_PER_CLK_SM   # SURVEY 8(d) sum form
-    return {"lsu": t_lsu, "xu": t_xu, "issue": t_issue, "min": max(t_lsu, t_xu, t_issue), "sum_form": t_sum}
-
-
-def stated_peak_pf_per_s(n_mean, nb, kmax, nk, clk_hz, n_sm=N_SM, which="min"):
-    """Whole-path ceiling n_SM * f * N / t_min, t_min = max over pipes."""
-    return n_sm * clk_hz * n_mean / pair_clocks(n_mean, nb, kmax, nk)[which]
+    return {"lsu": t_lsu, "xu": t_xu, "issue": t_issue, "min": max(t_lsu, t_xu, t_issue),
+            "method": max(t_lsu, t_issue), "sum_form": t_sum}
 
 
 class ClockSampler:
@@ -114,15 +114,15 @@ class ClockSampler:
 
 
 def oracle_rate(cfg, batch, freqs, kmin, kmax, curves, threads=None):
-    """Time the oracle as it stands on `curves` of the batch at all frequencies."""
+    """Time the oracle as it stands on `curves` of the batch at all frequencies; returns the spectra too."""
     import oracle
     oracle.lib()
     t0 = time.perf_counter()
-    _, used = oracle.spectrum_batch(batch.offsets, batch.t, batch.mag, batch.sigma, freqs,
-                                    cfg["grid"].nb, kmin, kmax, curves=curves, threads=threads)
+    res, used = oracle.spectrum_batch(batch.offsets, batch.t, batch.mag, batch.sigma, freqs,
+                                      cfg["grid"].nb, kmin, kmax, curves=curves, threads=threads)
     dt = time.perf_counter() - t0
     pts = sum(int(batch.offsets[c + 1] - batch.offsets[c]) for c in curves)
-    return pts * len(freqs) / dt, len(curves) / dt, used, dt
+    return pts * len(freqs) / dt, len(curves) / dt, used, dt, res
 
 
 def run_reference(args, cfg, rank, world):
@@ -134,14 +134,14 @@ def run_reference(args, cfg, rank, world):
     freqs = synth.freq_grid(grid)
     kmin, kmax = oracle.widths(grid.nb, grid.qmin, grid.qmax)
     cores = oracle.host_cores()
-    n_sample = max(cores, 8)           # curves per step: about 0.5 s/curve/core at C1
+    n_sample = max(cores, 8)           # curves per step: about 0.5 s/curve/core at C1, 1.2 at C2
     batch = synth.make_batch(cfg, range(min(n_sample, cfg["n_curves"])))
     curves = list(range(batch.n_curves))
     for _ in range(min(args.warmup, 1)):
         oracle_rate(cfg, batch, freqs, kmin, kmax, curves[:cores])
     tot_pf, tot_t, used = 0.0, 0.0, cores
     for _ in range(args.steps):
-        pf_s, _, used, dt = oracle_rate(cfg, batch, freqs, kmin, kmax, curves)
+        pf_s, _, used, dt, _ = oracle_rate(cfg, batch, freqs, kmin, kmax, curves)
         tot_pf += pf_s * dt
         tot_t += dt
     value = tot_pf / tot_t
@@ -180,16 +180,230 @@ def workload_name(name, cfg):
         g.nf, g.fmin, g.fmax, g.nb, g.qmin, g.qmax, cfg["top_k"])
 
 
+def profile_facts(name):
+    """Per-launch DRAM bytes and shared wavefronts per (curve, frequency) pair of the search kernel from the
+    committed `ncu --set full` captures (profiles/search_kernel_ncu_facts.json); None where not captured."""
+    p = os.path.join(ROOT, "profiles", "search_kernel_ncu_facts.json")
+    try:
+        return json.load(open(p)).get(name) or {}
+    except Exception:
+        return {}
+
+
+def parity_of_sample(batch, grid, freqs, kmin, kmax, k, curves, spectra, peaks):
+    """The timed step's peak lists (and their SR values) against the oracle spectra of the cpu_baseline
+    sample: tests/comparator.py, the same checks `pytest -m gpu` runs (peaks-only: the timed step writes no
+    spectrum, so SR is compared at the reported peaks)."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import oracle
+    from comparator import SR_RTOL, compare_peaks, exact_tie_runs
+    rep = {"curves": len(curves), "peak_slots": 0, "max_rel_err_at_peaks": 0.0, "exact_tie_slots": 0,
+           "near_tie_slots": 0, "unexplained": 0, "tolerance": "SR 1e-4 rel; peak lists = R14 on the tie-collapsed "
+           "oracle spectrum, near-ties inside 2e-6 counted (tests/comparator.py)"}
+    for c, orc in zip(curves, spectra):
+        st, o_sr, o_a, o_k, _ = orc
+        pk = peaks[c]
+        t = batch.curve(c)[0]
+        try:
+            if np.array_equal(oracle.peaks(o_sr, k), pk["freq_index"]):
+                r = compare_peaks(o_sr, pk["freq_index"], pk["sr"], k)
+            else:
+                ties, _ = exact_tie_runs(t, freqs, grid.nb, o_sr, o_a, o_k)
+                r = compare_peaks(o_sr, pk["freq_index"], pk["sr"], k, ties=ties)
+            rep["exact_tie_slots"] += r["exact_tie_slots"]
+            rep["near_tie_slots"] += r["near_tie_slots"]
+            idx = pk["freq_index"][pk["freq_index"] >= 0]
+            if idx.size:
+                rel = np.abs(pk["sr"][:idx.size].astype(np.float64) - o_sr[idx]) / o_sr[idx]
+                rep["max_rel_err_at_peaks"] = max(rep["max_rel_err_at_peaks"], float(rel.max()))
+                if rel.max() > SR_RTOL:
+                    rep["unexplained"] += 1
+        except AssertionError as e:
+            rep["unexplained"] += 1
+            rep.setdefault("first_failure", str(e)[:200])
+        rep["peak_slots"] += k
+    return rep
+
+
+def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_rank=0, flags=0, do_e2e=True,
+                do_cpu=True, workers=1, prefix_warmup=0):
+    """Time `steps` passes of the hot path over the configuration (this rank's replica).  Returns the
+    fields of the bench line for it.  prefix_warmup > 0: the warm-up runs on that many curves, then one
+    full untimed step grows the plan's scratch (long configurations in per_config)."""
+    import torch
+    import paper_1112_1701_b200 as bls
+    from paper_1112_1701_b200 import binding as B
+
+    dev = torch.device("cuda", local_rank)
+    props = torch.cuda.get_device_properties(dev)
+    n_sm = props.multi_processor_count
+    grid = cfg["grid"]
+    freqs = synth.freq_grid(grid)
+    t_gen = time.perf_counter()
+    batch = synth.make_batch(cfg, rank_curve_ids(cfg["n_curves"], rank), workers=workers)
+    t_gen = time.perf_counter() - t_gen
+    k = cfg["top_k"]
+    n_pts, n_curves = batch.n_points, batch.n_curves
+    pf_per_step = float(n_pts) * grid.nf
+
+    plan = bls.Plan(n_bins=grid.nb, q_min=grid.qmin, q_max=grid.qmax, freqs=freqs, max_top_k=k, device=local_rank, flags=flags)
+    kmin, kmax = plan.kmin, plan.kmax
+    t_d = torch.from_numpy(batch.t).to(dev)
+    m_d = torch.from_numpy(batch.mag).to(dev)
+    s_d = torch.from_numpy(batch.sigma).to(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+
+    def step():
+        plan.run(batch.offsets, t_d, m_d, s_d, batch.t_origin)
+        return plan.topk(k)
+
+    if prefix_warmup and prefix_warmup < n_curves:
+        npre = int(batch.offsets[prefix_warmup])
+        for _ in range(max(warmup, 3)):
+            plan.run(batch.offsets[:prefix_warmup + 1], t_d[:npre], m_d[:npre], s_d[:npre], batch.t_origin[:prefix_warmup])
+            plan.topk(k)
+        step()
+    else:
+        for _ in range(max(warmup, 3)):
+            step()
+    torch.cuda.synchronize()
+    launches_per_step = plan.query(B.QUERY_LAST_LAUNCHES)
+
+    sampler = ClockSampler(local_rank)
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    search_ns = 0
+    wall0 = time.perf_counter()
+    for i in range(steps):
+        flush.zero_()                       # L2 flush between timed iterations (outside the events)
+        ev[i][0].record()
+        raw = step()
+        ev[i][1].record()
+        search_ns += plan.query(B.QUERY_LAST_SEARCH_NS)   # synchronises; outside the event pair
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    t_ms = sum(a.elapsed_time(b) for a, b in ev)
+    t_ms = max_over_ranks(t_ms, dist, dev)
+    if dist:
+        dist.barrier()
+    ms_per_step = t_ms / steps
+    value = world * pf_per_step / (ms_per_step * 1e-3)
+    curves_s = world * n_curves / (ms_per_step * 1e-3)
+    peaks = plan.peaks_to_numpy(raw, k)
+    del flush
+
+    # ---- end to end: host buffers in, peaks out, through bls_search_host -------------------------
+    e2e = None
+    if do_e2e:
+        pin = lambda a: torch.from_numpy(a).pin_memory().numpy()
+        ht, hm, hs = pin(batch.t), pin(batch.mag), pin(batch.sigma)
+        long_step = ms_per_step > 1000.0
+        for _ in range(1 if long_step else 2):
+            plan.search_host(batch.offsets, ht, hm, hs, batch.t_origin, k)
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        n_e2e = 3 if long_step else max(3, min(steps, 10))
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            hp, hst = plan.search_host(batch.offsets, ht, hm, hs, batch.t_origin, k)
+        e2e_s = (time.perf_counter() - t0) / n_e2e
+        e2e_s = max_over_ranks(e2e_s, dist, dev)
+        assert np.array_equal(hp["freq_index"], peaks["freq_index"])
+        e2e = {"value": world * pf_per_step / e2e_s, "unit": UNIT,
+               "h2d_bytes_per_step": int(3 * 4 * n_pts + 8 * (n_curves + 1) + 8 * n_curves),
+               "d2h_bytes_per_step": int(n_curves * k * B.PEAK_DTYPE.itemsize + 4 * n_curves),
+               "ms_per_step": 1e3 * e2e_s, "steps": n_e2e, "api": "bls_search_host (pinned host buffers)"}
+        del ht, hm, hs
+
+    out = {"value": value, "ms_per_step": ms_per_step, "curves_per_sec": curves_s, "e2e": e2e, "clocks": clocks,
+           "gpu_launches": int(launches_per_step * steps), "wall_s_timed_region": wall, "steps": steps,
+           "config": {"workload": workload_name(name, cfg), "curves_per_gpu": n_curves, "points_per_gpu": n_pts,
+                      "l2": "flushed between timed iterations (256 MB memset)",
+                      "timing": "CUDA events per step on the launching stream, max over ranks",
+                      "generation_s": round(t_gen, 1)},
+           "canonical_rule_point_folds_per_step": plan.query(B.QUERY_LAST_CANONICAL)}
+    if rank != 0:
+        plan.destroy()
+        return out
+
+    # ---- roofline of the dominant kernel (search) -----------------------------------------------
+    nk = kmax - kmin + 1
+    n_mean = n_pts / n_curves
+    kernel_name = {1: "search_kernel", 2: "search_ws_kernel", 3: "search_wt_kernel"}.get(plan.query(B.QUERY_SEARCH_KERNEL), "?")
+    search_s = search_ns * 1e-9 / steps
+    achieved = pf_per_step / search_s
+    max_hz = (clocks.get("sm_max_mhz") or props.clock_rate / 1e3) * 1e6
+    pc = pair_clocks(n_mean, grid.nb, kmax, nk)
+    clk_per_pair = n_sm * max_hz * search_s / (n_curves * grid.nf)
+    peak = n_sm * max_hz * n_mean / pc["min"]
+    facts = profile_facts(name)
+    out["roofline"] = {
+        "bound": "alu", "kernel": kernel_name, "achieved": achieved, "peak": peak, "unit": UNIT, "frac": achieved / peak,
+        "traffic": facts.get("dram_bytes_per_launch"),
+        "peak_def": "n_SM*f_max*N/t_min per (curve,frequency) pair, t_min = max(LSU (2N+2(nb+kmax))/32, XU nb*nk/16, "
+                    "issue (5N+3.5 nb nk)/128) clk = max(%.0f, %.0f, %.0f); rates measured by microbench/issue_rates.cu "
+                    "(profiles/r02_microbench.md); f_max=%d MHz, n_SM=%d (DESIGN.md section 7)" % (
+                        pc["lsu"], pc["xu"], pc["issue"], max_hz / 1e6, n_sm),
+        "clk_per_pair": clk_per_pair,
+        "frac_method_floor": pc["method"] / clk_per_pair,
+        "method_floor_def": "max(LSU, issue) only: the XU term (one MUFU.RSQ per box) is a property of the instruction mix "
+                            "chosen for the division, not of the method; the >= 50 %% target is claimed against `frac`",
+        "frac_sum_form": pc["sum_form"] / clk_per_pair,
+        "fold_stage_peak": n_sm * max_hz * LSU_LANE_OPS_PER_CLK_SM / 2.0,
+        "frac_of_fold_stage_peak": achieved / (n_sm * max_hz * LSU_LANE_OPS_PER_CLK_SM / 2.0),
+        "lsu_wavefronts_per_pair": {"measured": facts.get("shared_wavefronts_per_pair"),
+                                    "algorithmic": (2.0 * n_mean + 2.0 * (grid.nb + kmax)) / 32.0},
+        "kernel_ms": 1e3 * search_s, "kernel_share_of_step": search_s / (ms_per_step * 1e-3),
+        "box_evals_per_s": n_curves * grid.nf * grid.nb * nk / search_s,
+        "peak_source": "derived from measured issue rates (no HBM/tensor bound applies); "
+                       "MEASURED_PEAKS.json hbm_gbs is not the bound of this kernel"}
+
+    # ---- the oracle beside it (bounded sample) and the parity of the timed step against it -------
+    if do_cpu and world == 1:                              # rank 0 at N = 1 only
+        import oracle
+        cores = oracle.host_cores()
+        # bounded sample: a short probe sizes the sample to about 15 s of wall time on this box's cores
+        probe = list(range(min(n_curves, cores)))
+        _, cv_probe, _, _, _ = oracle_rate(cfg, batch, freqs, kmin, kmax, probe)
+        n_s = int(min(n_curves, max(len(probe), 15.0 * cv_probe)))
+        curves = list(range(n_s))
+        pf_s, cv_s, used, dt, spectra = oracle_rate(cfg, batch, freqs, kmin, kmax, curves)
+        out["cpu_baseline"] = {"value": pf_s, "unit": UNIT, "cores": used, "kind": "oracle", "curves_per_sec": cv_s,
+                               "sample": "first %d curves x all %d frequencies of %s, %.1f s wall" % (n_s, grid.nf, name, dt),
+                               "parity": parity_of_sample(batch, grid, freqs, kmin, kmax, k, curves, spectra, peaks)}
+    plan.destroy()
+    return out
+
+
+PER_CONFIG = [("C1", 0), ("C3", 100), ("C4", 20000)]     # (name, curves of the warm-up prefix; 0 = whole batch)
+
+
+def short(r):
+    """The per_config entry of one configuration."""
+    rf = r.get("roofline") or {}
+    return {"workload": r["config"]["workload"], "steps": r["steps"], "ms_per_step": r["ms_per_step"],
+            "point_folds_per_sec": r["value"], "curves_per_sec": r["curves_per_sec"], "kernel": rf.get("kernel"),
+            "clk_per_pair": rf.get("clk_per_pair"), "roofline_frac": rf.get("frac"),
+            "frac_method_floor": rf.get("frac_method_floor"), "kernel_share_of_step": rf.get("kernel_share_of_step"),
+            "clocks": r["clocks"], "generation_s": r["config"]["generation_s"]}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C1")
+    ap.add_argument("--config", default="C2")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--max-curves", type=int, default=0, help="run only a prefix of the configuration")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (C1, C3, C4)")
     ap.add_argument("--flags", type=lambda v: int(v, 0), default=0, help="bls_config.flags (tuning only)")
     args = ap.parse_args()
 
@@ -205,9 +419,6 @@ def main():
         return
 
     import torch
-    import paper_1112_1701_b200 as bls
-    from paper_1112_1701_b200 import binding as B
-
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the BLS library has no CPU fallback")
     torch.cuda.set_device(local_rank)
@@ -216,144 +427,42 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=dev)
+    try:
+        workers = max(1, len(os.sched_getaffinity(0)) // max(world, 1))
+    except AttributeError:  # pragma: no cover
+        workers = os.cpu_count() or 1
 
     # weak scaling: every rank searches its own n_curves curves (curve ids offset by rank)
-    grid = cfg["grid"]
-    freqs = synth.freq_grid(grid)
-    ids = rank_curve_ids(cfg["n_curves"], rank)
-    batch = synth.make_batch(cfg, ids)
-    k = cfg["top_k"]
-    n_pts, n_curves = batch.n_points, batch.n_curves
-    pf_per_step = float(n_pts) * grid.nf
-
-    plan = bls.Plan(n_bins=grid.nb, q_min=grid.qmin, q_max=grid.qmax, freqs=freqs, max_top_k=k, device=local_rank, flags=args.flags)
-    kmin, kmax = plan.kmin, plan.kmax
-    t_d = torch.from_numpy(batch.t).to(dev)
-    m_d = torch.from_numpy(batch.mag).to(dev)
-    s_d = torch.from_numpy(batch.sigma).to(dev)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
-
-    def step():
-        plan.run(batch.offsets, t_d, m_d, s_d, batch.t_origin)
-        return plan.topk(k)
-
-    for _ in range(max(args.warmup, 3)):
-        step()
-    torch.cuda.synchronize()
-    launches_per_step = plan.query(B.QUERY_LAST_LAUNCHES)
-
-    sampler = ClockSampler(local_rank)
-    if dist:
-        dist.barrier()
-    torch.cuda.synchronize()
-    sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    search_ns = 0
-    wall0 = time.perf_counter()
-    for i in range(args.steps):
-        flush.zero_()                       # L2 flush between timed iterations (outside the events)
-        ev[i][0].record()
-        raw = step()
-        ev[i][1].record()
-        search_ns += plan.query(B.QUERY_LAST_SEARCH_NS)   # synchronises; outside the event pair
-    torch.cuda.synchronize()
-    wall = time.perf_counter() - wall0
-    clocks = sampler.stop()
-    t_ms = sum(a.elapsed_time(b) for a, b in ev)
-    t_ms = max_over_ranks(t_ms, dist, dev)
-    if dist:
-        dist.barrier()
-    ms_per_step = t_ms / args.steps
-    value = world * pf_per_step / (ms_per_step * 1e-3)
-    curves_s = world * n_curves / (ms_per_step * 1e-3)
-    peaks = plan.peaks_to_numpy(raw, k)
-
-    # ---- end to end: host buffers in, peaks out, through bls_search_host -------------------------
-    e2e = None
-    if not args.no_e2e:
-        pin = lambda a: torch.from_numpy(a).pin_memory().numpy()
-        ht, hm, hs = pin(batch.t), pin(batch.mag), pin(batch.sigma)
-        for _ in range(2):
-            plan.search_host(batch.offsets, ht, hm, hs, batch.t_origin, k)
-        torch.cuda.synchronize()
-        if dist:
-            dist.barrier()
-        n_e2e = max(3, min(args.steps, 10))
-        t0 = time.perf_counter()
-        for _ in range(n_e2e):
-            hp, hst = plan.search_host(batch.offsets, ht, hm, hs, batch.t_origin, k)
-        e2e_s = (time.perf_counter() - t0) / n_e2e
-        e2e_s = max_over_ranks(e2e_s, dist, dev)
-        assert np.array_equal(hp["freq_index"], peaks["freq_index"])
-        e2e = {"value": world * pf_per_step / e2e_s, "unit": UNIT,
-               "h2d_bytes_per_step": int(3 * 4 * n_pts + 8 * (n_curves + 1) + 8 * n_curves),
-               "d2h_bytes_per_step": int(n_curves * k * B.PEAK_DTYPE.itemsize + 4 * n_curves),
-               "ms_per_step": 1e3 * e2e_s, "api": "bls_search_host (pinned host buffers)"}
-
+    r = time_config(args.config, cfg, args.steps, args.warmup, rank=rank, world=world, dist=dist, local_rank=local_rank,
+                    flags=args.flags, do_e2e=not args.no_e2e, do_cpu=not args.no_cpu_baseline, workers=workers)
     if rank != 0:
-        plan.destroy()
         if dist:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (search) -----------------------------------------------
-    nk = kmax - kmin + 1
-    n_mean = n_pts / n_curves
-    plan_kernel_name = {1: "search_kernel", 2: "search_ws_kernel", 3: "search_wt_kernel"}.get(plan.query(B.QUERY_SEARCH_KERNEL), "?")
-    search_s = search_ns * 1e-9 / args.steps
-    achieved = pf_per_step / search_s
-    max_hz = (clocks.get("sm_max_mhz") or 1965) * 1e6
-    peak = stated_peak_pf_per_s(n_mean, grid.nb, kmax, nk, max_hz)
-    peak_sum = stated_peak_pf_per_s(n_mean, grid.nb, kmax, nk, max_hz, which="sum_form")
-    pc = pair_clocks(n_mean, grid.nb, kmax, nk)
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "search_kernel_dram_bytes.json")
-    if os.path.exists(tp):
-        try:
-            traffic = json.load(open(tp)).get(args.config)
-        except Exception:
-            traffic = None
-    roofline = {"bound": "alu", "kernel": plan_kernel_name, "achieved": achieved, "peak": peak,
-                "unit": UNIT, "frac": achieved / peak, "traffic": traffic,
-                "peak_def": "n_SM*f_max*N/t_min per (curve,frequency) pair, t_min = max(LSU (2N+2(nb+kmax))/32, XU nb*nk/16, "
-                            "issue (5N+4.5 nb nk)/128) clk = max(%.0f, %.0f, %.0f); rates measured by microbench/issue_rates.cu "
-                            "(profiles/r01a_microbench.md); f_max=%d MHz, n_SM=%d (DESIGN.md section 7)" % (
-                                pc["lsu"], pc["xu"], pc["issue"], max_hz / 1e6, N_SM),
-                "clk_per_pair": N_SM * max_hz * search_s / (n_curves * grid.nf),
-                "frac_sum_form": achieved / peak_sum,
-                "fold_stage_peak": N_SM * max_hz * LSU_LANE_OPS_PER_CLK_SM / 2.0,
-                "frac_of_fold_stage_peak": achieved / (N_SM * max_hz * LSU_LANE_OPS_PER_CLK_SM / 2.0),
-                "kernel_ms": 1e3 * search_s, "kernel_share_of_step": search_s / (ms_per_step * 1e-3),
-                "box_evals_per_s": n_curves * grid.nf * grid.nb * nk / search_s,
-                "peak_source": "derived from measured issue rates (no HBM/tensor bound applies); "
-                               "MEASURED_PEAKS.json hbm_gbs is not the bound of this kernel"}
+    per_config = None
+    if not args.no_per_config and world == 1 and not args.max_curves:
+        per_config = {}
+        for name, prefix in PER_CONFIG:
+            if name == args.config:
+                continue
+            try:
+                rc = time_config(name, dict(synth.config(name)), 3 if prefix == 0 else 1, 3, local_rank=local_rank, flags=args.flags,
+                                 do_e2e=False, do_cpu=False, workers=workers, prefix_warmup=prefix)
+                per_config[name] = short(rc)
+            except Exception as e:  # a secondary line must not sink the headline
+                per_config[name] = {"error": repr(e)[:300]}
+        per_config[args.config] = short(r)
 
-    # ---- the oracle beside it (bounded sample; also a parity spot check of the timed result) -----
-    cpu = None
-    if not args.no_cpu_baseline and world == 1:           # rank 0 at N = 1 only
-        import oracle
-        cores = oracle.host_cores()
-        # bounded sample: a short probe sizes the sample to about 15 s of wall time on this box's cores
-        probe = list(range(min(n_curves, cores)))
-        _, cv_probe, _, _ = oracle_rate(cfg, batch, freqs, kmin, kmax, probe)
-        n_s = int(min(n_curves, max(len(probe), 15.0 * cv_probe)))
-        curves = list(range(n_s))
-        pf_s, cv_s, used, dt = oracle_rate(cfg, batch, freqs, kmin, kmax, curves)
-        cpu = {"value": pf_s, "unit": UNIT, "cores": used, "kind": "oracle", "curves_per_sec": cv_s,
-               "sample": "first %d curves x all %d frequencies of %s, %.1f s wall" % (n_s, grid.nf, args.config, dt)}
-
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "int32 fixed-point bins, fp64 phase, fp32 box statistic",
-            "data": "synthetic", "curves_per_sec": curves_s,
-            "config": {"workload": workload_name(args.config, cfg), "curves_per_gpu": n_curves,
-                       "points_per_gpu": n_pts, "l2": "flushed between timed iterations (256 MB memset)",
-                       "timing": "CUDA events per step on the launching stream, max over ranks"},
-            "e2e": e2e, "gpu_launches": int(launches_per_step * args.steps), "clocks": clocks,
-            "roofline": roofline, "cpu_baseline": cpu, "wall_s_timed_region": wall,
-            "canonical_rule_point_folds_per_step": plan.query(B.QUERY_LAST_CANONICAL)}
+    line = {"metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32 fixed-point bins, fp64 phase, fp32 box ranking, fp64 SR from integer box sums",
+            "data": "synthetic", "curves_per_sec": r["curves_per_sec"], "config": r["config"],
+            "e2e": r["e2e"], "gpu_launches": r["gpu_launches"], "clocks": r["clocks"],
+            "roofline": r.get("roofline"), "cpu_baseline": r.get("cpu_baseline"), "per_config": per_config,
+            "wall_s_timed_region": r["wall_s_timed_region"],
+            "canonical_rule_point_folds_per_step": r["canonical_rule_point_folds_per_step"]}
     print(json.dumps(line), flush=True)
-    plan.destroy()
     if dist:
         dist.destroy_process_group()
 

@@ -204,18 +204,32 @@ def make_curve(cfg: dict, curve_id: int):
     return t_rel, mag.astype(np.float32), sig.astype(np.float32), t_origin, truth
 
 
-def make_batch(cfg: dict, curve_ids: Optional[Sequence[int]] = None) -> Batch:
-    """CSR batch of the requested curves (all curves of the configuration by default)."""
+def _make_chunk(args):
+    """Curves `ids` of `cfg` as one packed piece: (lengths, t, mag, sigma, origins, truths)."""
+    cfg, ids = args
+    curves = [make_curve(cfg, int(c)) for c in ids]
+    cat = (lambda j: np.concatenate([cv[j] for cv in curves]) if curves else np.empty(0, np.float32))
+    return (np.asarray([cv[0].size for cv in curves], dtype=np.int64), cat(0), cat(1), cat(2),
+            np.asarray([cv[3] for cv in curves], dtype=np.float64), [cv[4] for cv in curves])
+
+
+def make_batch(cfg: dict, curve_ids: Optional[Sequence[int]] = None, workers: int = 1) -> Batch:
+    """CSR batch of the requested curves (all curves of the configuration by default).  Every curve
+    has its own counter-based stream, so the result does not depend on `workers` (processes used to
+    generate large batches; 1 = in this process)."""
     if curve_ids is None:
         curve_ids = range(cfg["n_curves"])
     curve_ids = np.asarray(list(curve_ids), dtype=np.int64)
-    ts, ms, ss, origins, truth = [], [], [], [], []
+    if workers > 1 and len(curve_ids) >= 64 * workers:
+        import multiprocessing as mp
+        chunks = np.array_split(curve_ids, workers * 8)
+        with mp.get_context("spawn").Pool(workers) as pool:     # spawn: safe after CUDA has been initialised
+            parts = pool.map(_make_chunk, [(cfg, ch) for ch in chunks])
+    else:
+        parts = [_make_chunk((cfg, curve_ids))]
+    lengths = np.concatenate([p[0] for p in parts]) if parts else np.zeros(0, np.int64)
     offsets = np.zeros(len(curve_ids) + 1, dtype=np.int64)
-    for j, cid in enumerate(curve_ids):
-        t, m, s, o, tr = make_curve(cfg, int(cid))
-        ts.append(t); ms.append(m); ss.append(s); origins.append(o); truth.append(tr)
-        offsets[j + 1] = offsets[j] + t.size
-    cat = (lambda xs, dt: np.concatenate(xs).astype(dt) if xs else np.empty(0, dt))
-    return Batch(offsets=offsets, t=cat(ts, np.float32), mag=cat(ms, np.float32),
-                 sigma=cat(ss, np.float32), t_origin=np.asarray(origins, dtype=np.float64),
-                 curve_ids=curve_ids, truth=truth)
+    np.cumsum(lengths, out=offsets[1:])
+    cat = (lambda j, dt: np.concatenate([p[j] for p in parts]).astype(dt, copy=False))
+    return Batch(offsets=offsets, t=cat(1, np.float32), mag=cat(2, np.float32), sigma=cat(3, np.float32),
+                 t_origin=cat(4, np.float64), curve_ids=curve_ids, truth=[tr for p in parts for tr in p[5]])
