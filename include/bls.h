@@ -170,6 +170,49 @@ int bls_search_host(bls_plan *plan, const bls_batch *host_batch, int32_t k, bls_
 int bls_debug_fold_bins(int32_t device, const double *f, const double *t, int64_t n, int32_t n_bins,
                         uint32_t flags, int32_t *bins, int64_t *n_canonical);
 
+/* ---- f3: high-variability pre-filter (section 2.2.1) --------------------------------
+ * "We estimate the value and scatter of the locally expected photometric stability as a function of
+ * stellar magnitude in 0.1-mag bins, using a sigma-clipped average of the stars detected on each chip.
+ * Objects that show a more than 2 sigma increased variability compared to the ensemble expectation are
+ * flagged for further review."  Readings V1-V5:
+ *   per star   mu = weighted mean magnitude, rms = sqrt(sum_i w_i (mag_i - mu)^2), w as in bls_run;
+ *   cell       (group[c], floor((mu - mag_lo)/mag_bin)); stars with a data fault, a group outside
+ *              [0, n_groups) or a magnitude outside the n_mag_bins bins belong to no cell (cell = -1);
+ *   per cell   sigma clip of the members' rms: E = mean, S = population standard deviation, drop
+ *              |rms - E| > clip*S, at most max_iter rounds, stop when nothing is dropped;
+ *   flag       1 iff the cell kept >= min_members stars and rms > E + nsig*S.                        */
+typedef struct {
+    int32_t struct_size;   /* = sizeof(bls_variability_config)                                      */
+    int32_t n_groups;      /* >= 1: number of groups (chips)                                        */
+    double mag_lo;         /* lower edge of the first magnitude bin                                 */
+    double mag_bin;        /* bin width in magnitudes (the paper: 0.1), > 0                         */
+    int32_t n_mag_bins;    /* >= 1; n_groups * n_mag_bins <= 2^24                                   */
+    int32_t max_iter;      /* clip rounds, 0..100                                                   */
+    double clip;           /* clip threshold in sigma (> 0), e.g. 3                                 */
+    double nsig;           /* flag threshold in sigma (the paper: 2)                                */
+    int32_t min_members;   /* cells that keep fewer stars flag nothing                              */
+    int32_t reserved;
+} bls_variability_config;
+
+/* All DEVICE, [n_curves] each; any pointer may be NULL = "do not write". */
+typedef struct {
+    int32_t *status;    /* BLS_CURVE_*                                                               */
+    double *mean_mag;   /* mu                                                                        */
+    double *rms;        /* weighted RMS about mu                                                     */
+    int32_t *cell;      /* group * n_mag_bins + bin, or -1                                           */
+    double *expected;   /* E of the star's cell (0 if none)                                          */
+    double *scatter;    /* S of the star's cell                                                      */
+    int32_t *kept;      /* stars the clip kept in the cell                                           */
+    int32_t *flag;      /* 1 = more than nsig sigma above the ensemble expectation                   */
+} bls_variability_outputs;
+
+/* Runs the pre-filter on `batch` (same layout as bls_run: offsets HOST, t/mag/sigma DEVICE; t is only
+ * checked for finiteness).  group: DEVICE int32 [n_curves] or NULL (= one group).  Enqueues on
+ * cuda_stream; scratch is stream-ordered (cudaMallocAsync) and freed before returning control of the
+ * stream.  Needs no plan.  Errors: BLS_ERR_NULL / BLS_ERR_CONFIG / BLS_ERR_BATCH / BLS_ERR_CUDA. */
+int bls_variability(int32_t device, const bls_variability_config *cfg, const bls_batch *batch,
+                    const int32_t *group, const bls_variability_outputs *out, void *cuda_stream);
+
 /* NULL is a no-op. */
 int bls_plan_destroy(bls_plan *plan);
 

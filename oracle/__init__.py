@@ -60,6 +60,15 @@ def lib():
         L.oracle_peaks.argtypes = [C.c_int64, _f64p, C.c_int, _i64p]
         L.oracle_bins_many.restype = None
         L.oracle_bins_many.argtypes = [C.c_int64, _f64p, _f64p, C.c_int, _i32p]
+        L.oracle_sde.restype = C.c_double
+        L.oracle_sde.argtypes = [C.c_int64, _f64p, C.c_int64]
+        L.oracle_bin_shift.restype = C.c_int
+        L.oracle_bin_shift.argtypes = [C.c_double, C.c_double, C.c_int, C.c_double]
+        L.oracle_refine_spectrum.restype = C.c_int
+        L.oracle_refine_spectrum.argtypes = [C.c_int64, _f32p, _f32p, _f32p, C.c_double, C.c_double, C.c_int, C.c_int,
+                                             C.c_int, C.c_int, C.c_int, _f64p, _f64p, _i32p, _i32p, _f64p]
+        L.oracle_refine_pick.restype = C.c_int64
+        L.oracle_refine_pick.argtypes = [C.c_int64, _f64p]
         _lib = L
     return _lib
 
@@ -122,6 +131,37 @@ def peaks(sr, kpk: int) -> np.ndarray:
     idx = np.full(kpk, -1, dtype=np.int64)
     lib().oracle_peaks(sr.size, sr, kpk, idx)
     return idx
+
+
+def sde(sr, q: int) -> float:
+    sr = np.ascontiguousarray(sr, dtype=np.float64)
+    return lib().oracle_sde(sr.size, sr, int(q))
+
+
+def bin_index_shift(f: float, t: float, nb: int, shift: float) -> int:
+    return lib().oracle_bin_shift(float(f), float(t), int(nb), float(shift))
+
+
+def refine_spectrum(t, mag, sigma, f_lo: float, f_hi: float, n_fine: int, n_shift: int, nb: int, kmin: int, kmax: int):
+    """Fine spectrum around one peak -> (status, freq[m], sr[m], a[m], k[m], depth[m]), m = n_fine*n_shift,
+    entry (j, h) at j*n_shift + h."""
+    t, mag, sigma = _c32(t), _c32(mag), _c32(sigma)
+    m = n_fine * n_shift
+    fr = np.zeros(m); sr = np.zeros(m); dp = np.zeros(m)
+    a = np.zeros(m, dtype=np.int32); k = np.zeros(m, dtype=np.int32)
+    st = lib().oracle_refine_spectrum(t.size, t, mag, sigma, float(f_lo), float(f_hi), int(n_fine), int(n_shift),
+                                      int(nb), int(kmin), int(kmax), fr, sr, a, k, dp)
+    return st, fr, sr, a, k, dp
+
+
+def refine_pick(sr) -> int:
+    sr = np.ascontiguousarray(sr, dtype=np.float64)
+    return int(lib().oracle_refine_pick(sr.size, sr))
+
+
+def refine_bounds(freqs, q: int):
+    """S2: the fine grid of coarse peak q spans its two neighbours on the coarse grid."""
+    return float(freqs[max(q - 1, 0)]), float(freqs[min(q + 1, len(freqs) - 1)])
 
 
 def host_cores() -> int:

@@ -28,6 +28,11 @@
  *                         with closed-form depth and SR, invariants                   (pinned)
  *   oracle_sr_at        - same brute force, box/complement symmetry                   (pinned)
  *   oracle_peaks        - hand-written spectra with answers written out               (pinned)
+ *   oracle_sde          - hand-written spectra, closed form                           (pinned)
+ *   oracle_bin_shift    - exact rational arithmetic with a bin-grid shift              (pinned)
+ *   oracle_refine       - noiseless box between coarse grid points recovered to the fine
+ *                         step and to the quarter-bin shift (closed-form SR and depth),
+ *                         brute force over boxes with shifted member sets             (pinned)
  */
 #include <math.h>
 #include <stdint.h>
@@ -211,4 +216,88 @@ int oracle_peaks(int64_t nf, const double *sr, int kpk, int64_t *idx)
 void oracle_bins_many(int64_t n, const double *f, const double *t, int nb, int32_t *bins)
 {
     for (int64_t i = 0; i < n; ++i) bins[i] = oracle_bin(f[i], t[i], nb);
+}
+
+/* ---- f1: peak significance and refinement (readings S1-S4) ----
+ * The paper calls its detections "high-confidence" candidates and names the BLS of
+ * Kovacs et al. (L135) without printing a formula; these are the readings:
+ *   S1  significance ("signal detection efficiency"): SDE(q) = (SR[q] - mean(SR)) / sd(SR), mean and
+ *       POPULATION standard deviation over all nf samples of the curve's spectrum (the squared form R1);
+ *       0 if sd = 0;
+ *   S2  fine re-search around a peak at coarse index q: n_fine frequencies f_j = f_lo + j * step,
+ *       step = (f_hi - f_lo)/(n_fine - 1), f_lo = freqs[max(q-1, 0)], f_hi = freqs[min(q+1, nf-1)]
+ *       (n_fine = 1: f_0 = f_lo); each f_j evaluated in fp64 without contraction;
+ *   S3  sub-bin phase resolution: the bin grid is shifted by s_h = h / (n_shift * nb) cycles,
+ *       h = 0 .. n_shift-1: b = floor(nb * frac(f t - s_h)), by the rule of oracle_bin_shift;
+ *   S4  the refined peak is the best box over (j, h), ties to the smallest j, then the smallest h;
+ *       its box covers true phases [(a/nb + s_h), ((a+k)/nb + s_h)). */
+
+/* S1 */
+double oracle_sde(int64_t nf, const double *sr, int64_t q)
+{
+    double mean = 0.0;
+    for (int64_t i = 0; i < nf; ++i) mean += sr[i];
+    mean /= (double)nf;
+    double var = 0.0;
+    for (int64_t i = 0; i < nf; ++i) var += (sr[i] - mean) * (sr[i] - mean);
+    double sd = sqrt(var / (double)nf);
+    return sd > 0.0 ? (sr[q] - mean) / sd : 0.0;
+}
+
+/* S3: the phase rule R8 with the bin grid shifted by `shift` cycles: four individually rounded operations.
+ *   p = RN(f*t) ; p2 = RN(p - shift) ; phi = p2 - floor(p2) (exact) ; b = trunc(RN(phi*nb)), clamped. */
+int oracle_bin_shift(double f, double t, int nb, double shift)
+{
+    volatile double p = f * t;
+    volatile double p2 = p - shift;
+    double phi = p2 - floor(p2);
+    volatile double xb = phi * (double)nb;
+    int b = (int)xb;
+    if (b >= nb) b = nb - 1;
+    return b;
+}
+
+/* S2 + S3: the spectrum of one curve on the fine grid, entry (j, h) at index j*n_shift + h. */
+int oracle_refine_spectrum(int64_t n, const float *t, const float *mag, const float *sigma, double f_lo, double f_hi,
+                           int n_fine, int n_shift, int nb, int kmin, int kmax,
+                           double *freq, double *sr, int32_t *best_a, int32_t *best_k, double *depth)
+{
+    double *w = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    double *x = (double *)malloc(sizeof(double) * (size_t)(n > 0 ? n : 1));
+    double *W = (double *)malloc(sizeof(double) * (size_t)nb);
+    double *Y = (double *)malloc(sizeof(double) * (size_t)nb);
+    int st = oracle_prepare(n, t, mag, sigma, w, x);
+    volatile double step = n_fine > 1 ? (f_hi - f_lo) / (double)(n_fine - 1) : 0.0;
+    for (int j = 0; j < n_fine; ++j) {
+        volatile double js = (double)j * step;
+        double f = f_lo + js;
+        for (int h = 0; h < n_shift; ++h) {
+            int64_t q = (int64_t)j * n_shift + h;
+            freq[q] = f;
+            if (st != 0) { sr[q] = 0.0; best_a[q] = 0; best_k[q] = kmin; depth[q] = 0.0; continue; }
+            double shift = (double)h / (double)(n_shift * nb);
+            for (int b = 0; b < nb; ++b) { W[b] = 0.0; Y[b] = 0.0; }
+            for (int64_t i = 0; i < n; ++i) {
+                int b = oracle_bin_shift(f, (double)t[i], nb, shift);
+                W[b] += w[i];
+                Y[b] += w[i] * x[i];
+            }
+            int a, k;
+            search(nb, kmin, kmax, W, Y, &sr[q], &a, &k, &depth[q]);
+            best_a[q] = a; best_k[q] = k;
+        }
+    }
+    free(w); free(x); free(W); free(Y);
+    return st;
+}
+
+/* S4: index of the refined peak in a fine spectrum of m = n_fine*n_shift entries: the largest SR, ties
+ * to the smallest index (j major, h minor); -1 if every entry is 0. */
+int64_t oracle_refine_pick(int64_t m, const double *sr)
+{
+    int64_t best = -1;
+    double bv = 0.0;
+    for (int64_t q = 0; q < m; ++q)
+        if (sr[q] > bv) { bv = sr[q]; best = q; }
+    return best;
 }

@@ -22,5 +22,6 @@ from .binding import (  # noqa: F401
     Plan,
     debug_fold_bins,
     lib,
+    variability,
 )
 from . import binding  # noqa: F401

@@ -17,7 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libbls_b200.so")
 
 EXPORTS = ["bls_plan_create", "bls_run", "bls_topk", "bls_search_host", "bls_plan_destroy",
-           "bls_plan_query", "bls_strerror", "bls_plan_last_cuda_error", "bls_debug_fold_bins"]
+           "bls_plan_query", "bls_strerror", "bls_plan_last_cuda_error", "bls_debug_fold_bins",
+           "bls_variability"]
 
 BLS_OK = 0
 BLS_ERR_NULL, BLS_ERR_CONFIG, BLS_ERR_BATCH, BLS_ERR_ARG, BLS_ERR_CUDA, BLS_ERR_UNSUPPORTED = -1, -2, -3, -4, -5, -6
@@ -50,6 +51,17 @@ class BlsBatch(C.Structure):
 class BlsOutputs(C.Structure):
     _fields_ = [("sr", C.c_void_p), ("best_start", C.c_void_p), ("best_width", C.c_void_p),
                 ("depth", C.c_void_p), ("status", C.c_void_p)]
+
+
+class BlsVariabilityConfig(C.Structure):
+    _fields_ = [("struct_size", C.c_int32), ("n_groups", C.c_int32), ("mag_lo", C.c_double), ("mag_bin", C.c_double),
+                ("n_mag_bins", C.c_int32), ("max_iter", C.c_int32), ("clip", C.c_double), ("nsig", C.c_double),
+                ("min_members", C.c_int32), ("reserved", C.c_int32)]
+
+
+class BlsVariabilityOutputs(C.Structure):
+    _fields_ = [("status", C.c_void_p), ("mean_mag", C.c_void_p), ("rms", C.c_void_p), ("cell", C.c_void_p),
+                ("expected", C.c_void_p), ("scatter", C.c_void_p), ("kept", C.c_void_p), ("flag", C.c_void_p)]
 
 
 # numpy view of bls_peak (32 bytes, natural alignment)
@@ -94,8 +106,36 @@ def lib():
         L.bls_debug_fold_bins.restype = C.c_int
         L.bls_debug_fold_bins.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32,
                                           C.c_uint32, C.c_void_p, C.POINTER(C.c_int64)]
+        L.bls_variability.restype = C.c_int
+        L.bls_variability.argtypes = [C.c_int32, C.POINTER(BlsVariabilityConfig), C.POINTER(BlsBatch), C.c_void_p,
+                                      C.POINTER(BlsVariabilityOutputs), C.c_void_p]
         _lib = L
     return _lib
+
+
+def variability(offsets, t, mag, sigma, group=None, *, n_groups: int = 1, mag_lo: float = 12.0, mag_bin: float = 0.1,
+                n_mag_bins: int = 80, clip: float = 3.0, nsig: float = 2.0, max_iter: int = 5, min_members: int = 5,
+                device: int = 0, stream: Optional[int] = None):
+    """bls_variability: offsets host int64; t, mag, sigma float32 CUDA tensors; group int32 CUDA tensor or None.
+    Returns a dict of CUDA tensors (status, mean_mag, rms, cell, expected, scatter, kept, flag)."""
+    import torch
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    n = offsets.size - 1
+    dev = torch.device("cuda", device)
+    i32 = lambda: torch.zeros(max(n, 1), dtype=torch.int32, device=dev)
+    f64 = lambda: torch.zeros(max(n, 1), dtype=torch.float64, device=dev)
+    out = dict(status=i32(), mean_mag=f64(), rms=f64(), cell=i32(), expected=f64(), scatter=f64(), kept=i32(), flag=i32())
+    cfg = BlsVariabilityConfig(C.sizeof(BlsVariabilityConfig), int(n_groups), float(mag_lo), float(mag_bin), int(n_mag_bins),
+                               int(max_iter), float(clip), float(nsig), int(min_members), 0)
+    b = BlsBatch(n, offsets.ctypes.data, _ptr(t), _ptr(mag), _ptr(sigma), None)
+    o = BlsVariabilityOutputs(*[_ptr(out[k]) for k in ("status", "mean_mag", "rms", "cell", "expected", "scatter", "kept", "flag")])
+    if stream is None:
+        stream = torch.cuda.current_stream(dev).cuda_stream
+    rc = lib().bls_variability(device, C.byref(cfg), C.byref(b), C.c_void_p(_ptr(group)) if group is not None else None,
+                               C.byref(o), C.c_void_p(stream))
+    if rc != BLS_OK:
+        raise BlsError(rc)
+    return {k: v[:n] for k, v in out.items()}
 
 
 def debug_fold_bins(f, t, n_bins: int, flags: int = 0, device: int = 0):

@@ -418,6 +418,49 @@ int bls_debug_fold_bins(int32_t device, const double *f, const double *t, int64_
     return BLS_OK;
 }
 
+int bls_variability(int32_t device, const bls_variability_config *cfg, const bls_batch *b, const int32_t *group,
+                    const bls_variability_outputs *out, void *cuda_stream)
+{
+    if (!cfg || !b || !out) return BLS_ERR_NULL;
+    if (cfg->struct_size != (int32_t)sizeof(bls_variability_config)) return BLS_ERR_CONFIG;
+    if (cfg->n_groups < 1 || cfg->n_mag_bins < 1 || (int64_t)cfg->n_groups * cfg->n_mag_bins > (1 << 24)) return BLS_ERR_CONFIG;
+    if (!(cfg->mag_bin > 0.0) || !isfinite(cfg->mag_lo) || !(cfg->clip > 0.0) || !isfinite(cfg->nsig)) return BLS_ERR_CONFIG;
+    if (cfg->max_iter < 0 || cfg->max_iter > 100 || cfg->min_members < 0) return BLS_ERR_CONFIG;
+    if (b->n_curves < 0) return BLS_ERR_BATCH;
+    if (!b->offsets) return BLS_ERR_NULL;
+    const int64_t nc = b->n_curves;
+    if (b->offsets[0] != 0) return BLS_ERR_BATCH;
+    for (int64_t c = 0; c < nc; ++c)
+        if (b->offsets[c + 1] < b->offsets[c]) return BLS_ERR_BATCH;
+    if (b->offsets[nc] > 0 && (!b->t || !b->mag || !b->sigma)) return BLS_ERR_NULL;
+    if (nc == 0) return BLS_OK;
+    if (nc > 2147483647LL) return BLS_ERR_BATCH;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int64_t n_cells = (int64_t)cfg->n_groups * cfg->n_mag_bins;
+    // one stream-ordered scratch block: offsets | status | cell | members | count | offset | cursor | mean | rms | keep
+    size_t off = 0;
+    auto take = [&off](size_t bytes) { const size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+    const size_t o_offsets = take((size_t)(nc + 1) * 8), o_status = take((size_t)nc * 4), o_cell = take((size_t)nc * 4);
+    const size_t o_members = take((size_t)nc * 4), o_count = take((size_t)n_cells * 4), o_offset = take((size_t)(n_cells + 1) * 4);
+    const size_t o_cursor = take((size_t)n_cells * 4), o_mean = take((size_t)nc * 8), o_rms = take((size_t)nc * 8);
+    const size_t o_keep = take((size_t)nc);
+    unsigned char *scr = nullptr;
+    if (cudaMallocAsync((void **)&scr, off, st) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    cudaError_t e = cudaMemcpyAsync(scr + o_offsets, b->offsets, (size_t)(nc + 1) * 8, cudaMemcpyHostToDevice, st);
+    int32_t *status = out->status ? out->status : (int32_t *)(scr + o_status);
+    int32_t *cell = out->cell ? out->cell : (int32_t *)(scr + o_cell);
+    double *mean_mag = out->mean_mag ? out->mean_mag : (double *)(scr + o_mean);
+    double *rms = out->rms ? out->rms : (double *)(scr + o_rms);
+    if (e == cudaSuccess)
+        e = launch_variability(b->t, b->mag, b->sigma, (const int64_t *)(scr + o_offsets), group, nc, *cfg, status, mean_mag,
+                               rms, cell, (int32_t *)(scr + o_count), (int32_t *)(scr + o_offset), (int32_t *)(scr + o_cursor),
+                               (int32_t *)(scr + o_members), scr + o_keep, out->expected, out->scatter, out->kept, out->flag, st);
+    const cudaError_t e2 = cudaFreeAsync(scr, st);
+    if (e != cudaSuccess || e2 != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    return BLS_OK;
+}
+
 int bls_topk(bls_plan *p, int32_t k, bls_peak *peaks, void *cuda_stream)
 {
     if (!p || !peaks) return BLS_ERR_NULL;

@@ -114,6 +114,37 @@ __device__ __forceinline__ int fold_bin(double f, double t, int nb, uint32_t G, 
 }
 #endif
 
+#ifdef __CUDACC__
+// Fixed-shape block reductions over kPrepThreads threads (fixed strided accumulation + fixed tree:
+// bitwise reproducible).  `sh` holds kPrepThreads / 32 doubles.
+__device__ __forceinline__ double block_sum(double v, double *sh) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) sh[warp] = v;
+    __syncthreads();
+    double tot = 0.0;
+#pragma unroll
+    for (int w = 0; w < kPrepThreads / 32; ++w) tot += sh[w];
+    return tot;
+}
+
+__device__ __forceinline__ double block_max_d(double v, double *sh) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    __syncthreads();
+    if (lane == 0) sh[warp] = v;
+    __syncthreads();
+    double tot = 0.0;
+#pragma unroll
+    for (int w = 0; w < kPrepThreads / 32; ++w) tot = fmax(tot, sh[w]);
+    return tot;
+}
+
+#endif
+
 // Bin rows a search buffer holds when the start bins are dealt to `slots` half-warps: the nb bins
 // plus the cyclic extension the widest box of the last start reaches (bls_search.cu).
 int search_rows_for(int nb, int kmax, int slots);
@@ -124,6 +155,11 @@ cudaError_t search_configure(int max_smem_optin);
 cudaError_t launch_prep(const float *t, const float *mag, const float *sigma, const int64_t *offsets,
                         int64_t n_curves, double fmax, PointRec *pts, CurveMeta *meta, int32_t *u_status,
                         cudaStream_t st);
+cudaError_t launch_variability(const float *t, const float *mag, const float *sigma, const int64_t *d_offsets,
+                               const int32_t *group, int64_t n, const bls_variability_config &cfg, int32_t *status,
+                               double *mean_mag, double *rms, int32_t *cell, int32_t *count, int32_t *offset,
+                               int32_t *cursor, int32_t *members, unsigned char *keep, double *expected,
+                               double *scatter, int32_t *kept, int32_t *flag, cudaStream_t st);
 cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem, cudaStream_t st);
 cudaError_t launch_peaks(const float *sr, const uint32_t *ak, const float *depth, const CurveMeta *meta,
                          int64_t curve_base, int64_t chunk_curves, int nf, int max_k, PeakCand *cand,

@@ -10,32 +10,6 @@
 
 namespace bls {
 
-__device__ __forceinline__ double block_sum(double v, double *sh) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    __syncthreads();
-    if (lane == 0) sh[warp] = v;
-    __syncthreads();
-    double tot = 0.0;
-#pragma unroll
-    for (int w = 0; w < kPrepThreads / 32; ++w) tot += sh[w];
-    return tot;
-}
-
-__device__ __forceinline__ double block_max(double v, double *sh) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-    int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    __syncthreads();
-    if (lane == 0) sh[warp] = v;
-    __syncthreads();
-    double tot = 0.0;
-#pragma unroll
-    for (int w = 0; w < kPrepThreads / 32; ++w) tot = fmax(tot, sh[w]);
-    return tot;
-}
-
 __global__ void __launch_bounds__(kPrepThreads)
 prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const float *__restrict__ sigma,
             const int64_t *__restrict__ offsets, double fmax_grid, PointRec *__restrict__ pts,
@@ -64,7 +38,7 @@ prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const fl
     }
     if (flags) atomicOr(&s_flags, flags);
     double sw = block_sum(acc, sh);
-    tmax = block_max(tmax, sh);
+    tmax = block_max_d(tmax, sh);
     __syncthreads();
     int status = BLS_CURVE_OK;
     if (n < 2) status = BLS_CURVE_TOO_FEW;
