@@ -226,7 +226,7 @@ def parity_of_sample(batch, grid, freqs, kmin, kmax, k, curves, spectra, peaks):
 
 
 def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_rank=0, flags=0, do_e2e=True,
-                do_cpu=True, workers=1, prefix_warmup=0):
+                do_cpu=True, workers=1, prefix_warmup=0, do_refine=False):
     """Time `steps` passes of the hot path over the configuration (this rank's replica).  Returns the
     fields of the bench line for it.  prefix_warmup > 0: the warm-up runs on that many curves, then one
     full untimed step grows the plan's scratch (long configurations in per_config)."""
@@ -296,6 +296,22 @@ def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_r
     peaks = plan.peaks_to_numpy(raw, k)
     del flush
 
+    # ---- f1: cost of refining the top-k peaks of the timed step (64 fine frequencies x 4 bin shifts each) ----
+    refine = None
+    if do_refine:
+        plan.refine(k, 64, 4)                                 # warm-up (grows nothing: reuses the spectrum scratch)
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record()
+        refined = plan.refine(k, 64, 4)
+        r1.record()
+        torch.cuda.synchronize()
+        rms_ = r0.elapsed_time(r1)
+        ok = refined["freq_index"] >= 0
+        refine = {"api": "bls_refine(k=%d, n_fine=64, n_shift=4)" % k, "ms": rms_, "share_of_step": rms_ / ms_per_step,
+                  "point_folds": float(n_pts) * k * 64 * 4,
+                  "median_sr_gain": float(np.median(refined["sr"][ok] / refined["coarse_sr"][ok])) if ok.any() else None,
+                  "median_sde": float(np.median(refined["sde"][ok])) if ok.any() else None}
+
     # ---- end to end: host buffers in, peaks out, through bls_search_host -------------------------
     e2e = None
     if do_e2e:
@@ -321,7 +337,7 @@ def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_r
         del ht, hm, hs
 
     out = {"value": value, "ms_per_step": ms_per_step, "curves_per_sec": curves_s, "e2e": e2e, "clocks": clocks,
-           "gpu_launches": int(launches_per_step * steps), "wall_s_timed_region": wall, "steps": steps,
+           "gpu_launches": int(launches_per_step * steps), "wall_s_timed_region": wall, "steps": steps, "refine": refine,
            "config": {"workload": workload_name(name, cfg), "curves_per_gpu": n_curves, "points_per_gpu": n_pts,
                       "l2": "flushed between timed iterations (256 MB memset)",
                       "timing": "CUDA events per step on the launching stream, max over ranks",
@@ -390,7 +406,7 @@ def short(r):
             "point_folds_per_sec": r["value"], "curves_per_sec": r["curves_per_sec"], "kernel": rf.get("kernel"),
             "clk_per_pair": rf.get("clk_per_pair"), "roofline_frac": rf.get("frac"),
             "frac_method_floor": rf.get("frac_method_floor"), "kernel_share_of_step": rf.get("kernel_share_of_step"),
-            "clocks": r["clocks"], "generation_s": r["config"]["generation_s"]}
+            "clocks": r["clocks"], "generation_s": r["config"]["generation_s"], "refine_top_k": r.get("refine")}
 
 
 def main():
@@ -434,7 +450,8 @@ def main():
 
     # weak scaling: every rank searches its own n_curves curves (curve ids offset by rank)
     r = time_config(args.config, cfg, args.steps, args.warmup, rank=rank, world=world, dist=dist, local_rank=local_rank,
-                    flags=args.flags, do_e2e=not args.no_e2e, do_cpu=not args.no_cpu_baseline, workers=workers)
+                    flags=args.flags, do_e2e=not args.no_e2e, do_cpu=not args.no_cpu_baseline, workers=workers,
+                    do_refine=(world == 1))
     if rank != 0:
         if dist:
             dist.destroy_process_group()
@@ -459,7 +476,8 @@ def main():
             "vs_baseline": None, "dtype": "int32 fixed-point bins, fp64 phase, fp32 box ranking, fp64 SR from integer box sums",
             "data": "synthetic", "curves_per_sec": r["curves_per_sec"], "config": r["config"],
             "e2e": r["e2e"], "gpu_launches": r["gpu_launches"], "clocks": r["clocks"],
-            "roofline": r.get("roofline"), "cpu_baseline": r.get("cpu_baseline"), "per_config": per_config,
+            "roofline": r.get("roofline"), "cpu_baseline": r.get("cpu_baseline"), "refine_top_k": r.get("refine"),
+            "per_config": per_config,
             "wall_s_timed_region": r["wall_s_timed_region"],
             "canonical_rule_point_folds_per_step": r["canonical_rule_point_folds_per_step"]}
     print(json.dumps(line), flush=True)

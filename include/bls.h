@@ -170,6 +170,36 @@ int bls_search_host(bls_plan *plan, const bls_batch *host_batch, int32_t k, bls_
 int bls_debug_fold_bins(int32_t device, const double *f, const double *t, int64_t n, int32_t n_bins,
                         uint32_t flags, int32_t *bins, int64_t *n_canonical);
 
+/* ---- f1: peak significance and refinement ("high-confidence"
+ * candidates; readings S1-S4 of DESIGN.md section 3) ------------------------------------------------
+ *   S1  sde = (SR_peak - mean(SR)) / sd(SR) over the curve's whole coarse spectrum (population sd);
+ *   S2  fine grid of a peak at coarse index q: f_j = f_lo + j*step, j = 0..n_fine-1,
+ *       f_lo = freqs[max(q-1,0)], step = (freqs[min(q+1,nf-1)] - f_lo)/(n_fine-1);
+ *   S3  the bin grid shifted by s_h = h/(n_shift*nb) cycles, h = 0..n_shift-1: b = floor(nb*frac(f t - s_h));
+ *   S4  the refined peak is the best box over (j, h), ties to the smallest j, then h.               */
+typedef struct {
+    int32_t freq_index;    /* coarse index of the peak this refines; -1 pads short lists            */
+    int32_t fine_index;    /* j of the refined frequency (-1: nothing found)                        */
+    int32_t shift_index;   /* h of the bin-grid shift                                               */
+    uint16_t start_bin;    /* start bin a in the shifted grid                                       */
+    uint16_t width_bins;   /* width k                                                               */
+    float sr;              /* refined SR                                                            */
+    float depth;           /* refined depth (> 0 = dimming)                                         */
+    float sde;             /* S1, from the COARSE spectrum and the coarse peak's SR                 */
+    float coarse_sr;       /* SR of the coarse peak                                                 */
+    double freq;           /* refined frequency, cycles/day                                         */
+    double period;         /* 1 / freq, days                                                        */
+    double epoch;          /* t_origin[c] + ((a + k/2)/nb + s_h)/freq : mid-box time                */
+    double duration;       /* (k/nb)/freq, days                                                     */
+} bls_refined_peak;
+
+/* Refine the k best peaks of every curve of the last bls_run: for each, the BLS search of bls_run over
+ * its n_fine x n_shift fine entries (2 <= n_fine <= 256 or n_fine == 1; 1 <= n_shift <= 8), reduced to one
+ * bls_refined_peak.  out: DEVICE, [n_curves*k].  The batch buffers of that bls_run must still be alive
+ * (the plan keeps its prepared copy; t_origin is re-read from the plan's copy).  Enqueues on cuda_stream
+ * (the stream of that bls_run or one ordered after it); synchronises only if plan scratch must grow.  */
+int bls_refine(bls_plan *plan, int32_t k, int32_t n_fine, int32_t n_shift, bls_refined_peak *out, void *cuda_stream);
+
 /* ---- f3: high-variability pre-filter (section 2.2.1) --------------------------------
  * "We estimate the value and scatter of the locally expected photometric stability as a function of
  * stellar magnitude in 0.1-mag bins, using a sigma-clipped average of the stars detected on each chip.

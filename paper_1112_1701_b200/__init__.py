@@ -19,6 +19,7 @@ from .binding import (  # noqa: F401
     EXPORTS,
     LIB_PATH,
     PEAK_DTYPE,
+    REFINED_DTYPE,
     Plan,
     debug_fold_bins,
     lib,

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libbls_b200.so")
 
 EXPORTS = ["bls_plan_create", "bls_run", "bls_topk", "bls_search_host", "bls_plan_destroy",
            "bls_plan_query", "bls_strerror", "bls_plan_last_cuda_error", "bls_debug_fold_bins",
-           "bls_variability"]
+           "bls_variability", "bls_refine"]
 
 BLS_OK = 0
 BLS_ERR_NULL, BLS_ERR_CONFIG, BLS_ERR_BATCH, BLS_ERR_ARG, BLS_ERR_CUDA, BLS_ERR_UNSUPPORTED = -1, -2, -3, -4, -5, -6
@@ -69,6 +69,12 @@ PEAK_DTYPE = np.dtype([("freq_index", "<i4"), ("sr", "<f4"), ("depth", "<f4"), (
                        ("width_bins", "<u2"), ("freq", "<f8"), ("epoch", "<f8")], align=True)
 assert PEAK_DTYPE.itemsize == 32
 
+# numpy view of bls_refined_peak (64 bytes)
+REFINED_DTYPE = np.dtype([("freq_index", "<i4"), ("fine_index", "<i4"), ("shift_index", "<i4"), ("start_bin", "<u2"),
+                          ("width_bins", "<u2"), ("sr", "<f4"), ("depth", "<f4"), ("sde", "<f4"), ("coarse_sr", "<f4"),
+                          ("freq", "<f8"), ("period", "<f8"), ("epoch", "<f8"), ("duration", "<f8")], align=True)
+assert REFINED_DTYPE.itemsize == 64
+
 _lib = None
 
 
@@ -106,6 +112,8 @@ def lib():
         L.bls_debug_fold_bins.restype = C.c_int
         L.bls_debug_fold_bins.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32,
                                           C.c_uint32, C.c_void_p, C.POINTER(C.c_int64)]
+        L.bls_refine.restype = C.c_int
+        L.bls_refine.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         L.bls_variability.restype = C.c_int
         L.bls_variability.argtypes = [C.c_int32, C.POINTER(BlsVariabilityConfig), C.POINTER(BlsBatch), C.c_void_p,
                                       C.POINTER(BlsVariabilityOutputs), C.c_void_p]
@@ -265,6 +273,17 @@ class Plan:
             stream = torch.cuda.current_stream(dev).cuda_stream
         self._check(lib().bls_topk(self._h, int(k), C.c_void_p(out.data_ptr()), C.c_void_p(stream)))
         return out[: self._n_curves * k * PEAK_DTYPE.itemsize]
+
+    # -- bls_refine --------------------------------------------------------------------------------
+    def refine(self, k: int, n_fine: int = 64, n_shift: int = 4, stream: Optional[int] = None) -> np.ndarray:
+        """bls_refine on the last run; returns host records [n_curves, k] of REFINED_DTYPE (synchronises)."""
+        import torch
+        dev = torch.device("cuda", self.device)
+        out = torch.zeros(max(self._n_curves * k, 1) * REFINED_DTYPE.itemsize, dtype=torch.uint8, device=dev)
+        if stream is None:
+            stream = torch.cuda.current_stream(dev).cuda_stream
+        self._check(lib().bls_refine(self._h, int(k), int(n_fine), int(n_shift), C.c_void_p(out.data_ptr()), C.c_void_p(stream)))
+        return out[: self._n_curves * k * REFINED_DTYPE.itemsize].cpu().numpy().view(REFINED_DTYPE).reshape(-1, k)
 
     def peaks_to_numpy(self, raw, k: int) -> np.ndarray:
         return raw.cpu().numpy().view(PEAK_DTYPE).reshape(-1, k)

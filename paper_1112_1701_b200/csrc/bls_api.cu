@@ -31,7 +31,7 @@ struct bls_plan {
     int64_t *d_offsets = nullptr;
     double *d_origin = nullptr;
     PeakCand *d_cand = nullptr;
-    float *d_sr = nullptr;          int64_t cap_chunk = 0;   // curves per chunk the scratch can hold
+    float *d_sr = nullptr;          int64_t cap_entries = 0; // (sr, ak, depth) entries the spectrum scratch holds
     uint32_t *d_ak = nullptr;
     float *d_depth = nullptr;
     unsigned long long *d_canon = nullptr;
@@ -40,6 +40,9 @@ struct bls_plan {
     bls_peak *d_hpeaks = nullptr;   int64_t cap_host_peaks = 0;
     int32_t *d_hstatus = nullptr;   int64_t cap_host_status = 0;
 
+    double2 *d_sr_stats = nullptr;  // [cap_curves] mean and sd of each curve's spectrum (reading S1)
+    double *d_flo = nullptr, *d_fstep = nullptr;  int64_t cap_refine = 0;   // [n_curves * k] fine grids of bls_refine
+    int64_t last_max_n = 0;
     int64_t last_n_curves = -1;
     bool last_has_origin = false;
     int64_t last_launches = 0;
@@ -90,6 +93,106 @@ void release(T *&ptr)
 {
     if (ptr) cudaFree(ptr);
     ptr = nullptr;
+}
+
+
+// Launch geometry of the search kernels for `nf` frequencies per curve, curves of at most max_n points,
+// `chunk` curves per launch: which kernel, its CTA shape, shared memory and work items.  Fills every
+// field of `a` that does not depend on the caller's output buffers.
+struct SearchLaunch {
+    SearchArgs a;
+    size_t smem;
+    int64_t items;
+};
+
+int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, SearchLaunch &L)
+{
+    SearchArgs &a = L.a;
+    size_t &smem_out = L.smem;
+    const int ntiles = (int)((nf + kTileFreqs - 1) / kTileFreqs);
+    const size_t optin = (size_t)p->max_smem_optin;
+    const size_t sm_smem = (size_t)p->max_smem_sm;
+    const int warps_flag = (int)((p->flags >> 8) & 0xffu);
+    const int fold_flag = (int)((p->flags >> 16) & 0xffu);
+    // Kernel 2 (warp-specialised, two bin buffers) whenever its buffers fit shared memory, with the
+    // curve staged in shared memory if that fits too; otherwise kernel 1 (one buffer, two CTAs per SM).
+    int ws_search = kWsSearchWarps;
+    if (warps_flag >= 1 && warps_flag <= kWsMaxWarps - 1) ws_search = warps_flag;
+    int ws_fold = kWsMaxWarps - ws_search;
+    if (fold_flag >= 1 && fold_flag < ws_fold) ws_fold = fold_flag;
+    const bool ws = !(p->flags & BLS_FLAG_SINGLE_BUFFER) &&
+                    search_smem_bytes(p->nb, p->kmax, ws_search, 2, 0) <= optin;
+    int k1_warps = kMaxSearchWarps;
+    if (warps_flag >= 1 && warps_flag <= kMaxSearchWarps) k1_warps = warps_flag;
+    const int warps = ws ? ws_search : k1_warps;            // warps that walk the boxes
+    const int buffers = ws ? 2 : 1;
+    int pts_in_smem = 1;
+    size_t smem = search_smem_bytes(p->nb, p->kmax, warps, buffers, max_n);
+    if (smem > optin) {                            // curve too long to stage: read it through L1/L2
+        pts_in_smem = 0;
+        smem = search_smem_bytes(p->nb, p->kmax, warps, buffers, 0);
+    }
+    if (smem > optin) return BLS_ERR_UNSUPPORTED;
+    int threads = (ws ? ws_search + ws_fold : k1_warps) * 32;
+    int kernel = ws ? 2 : 1;
+    int nrows = search_rows_for(p->nb, p->kmax, 2 * warps);
+    // Kernel 3 (one warp per tile, warp-private bins) for small shapes: when two CTAs of kWtWarps
+    // warps, each with the curve staged, fit an SM.  There a tile is too little work to pay for the
+    // hand-offs of kernels 1 and 2 (C4: 200 epochs, 64 bins).
+    const int wt_rows = search_rows_for(p->nb, p->kmax, 2);
+    const size_t wt_smem = (size_t)kWtWarps * ((size_t)wt_rows * kTileFreqs * 8 + 256) + (size_t)max_n * sizeof(PointRec);
+    const bool wt_fits = 2 * (wt_smem + 1024) <= sm_smem;
+    if (!(p->flags & (BLS_FLAG_SINGLE_BUFFER | BLS_FLAG_NO_WARP_PER_TILE)) && wt_fits) {
+        kernel = 3; smem = wt_smem; pts_in_smem = 1; threads = kWtWarps * 32; nrows = wt_rows;
+    }
+    int ctas_per_sm = (int)(sm_smem / (smem + 1024));
+    if (ctas_per_sm < 1) ctas_per_sm = 1;
+    const int max_ctas = kernel == 2 ? 1 : 2;                       // register-limited (launch bounds)
+    if (ctas_per_sm > max_ctas) ctas_per_sm = max_ctas;
+    const int waves = kernel == 1 ? 12 : 24;                        // enough waves to hide the tail
+    const int64_t target_ctas = (int64_t)p->sm_count * ctas_per_sm * waves;
+    int64_t items = (target_ctas + chunk - 1) / chunk;
+    if (items < 1) items = 1;
+    if (items > ntiles) items = ntiles;
+    int tiles_per_item = (int)((ntiles + items - 1) / items);
+    items = (ntiles + tiles_per_item - 1) / tiles_per_item;
+    p->last_tiles_per_item = tiles_per_item;
+    p->last_kernel = kernel;
+
+    a.pts = p->d_pts; a.offsets = p->d_offsets; a.meta = p->d_meta; a.freqs = p->d_freqs;
+    a.nf = (int)nf; a.nb = p->nb; a.kmin = p->kmin; a.kmax = p->kmax;
+    a.tiles_per_item = tiles_per_item; a.items_per_curve = (int)items;
+    a.pts_in_smem = pts_in_smem;
+    a.nrows = nrows;
+    a.search_warps = kernel == 2 ? ws_search : 0;
+    a.kernel = kernel;
+    a.threads = threads;
+    a.force_canonical = (p->flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0;
+    a.sr = p->d_sr; a.ak = p->d_ak; a.depth = p->d_depth;
+    a.u_sr = nullptr; a.u_start = nullptr; a.u_width = nullptr; a.u_depth = nullptr;
+    a.f_lo = nullptr; a.f_step = nullptr; a.refine_k = 0; a.n_fine = 0; a.n_shift = 0;
+    a.canon_count = p->d_canon;
+    a.debug = (int)(p->flags >> 24);
+
+    smem_out = smem;
+    L.items = items;
+    return BLS_OK;
+}
+
+// the plan-owned spectrum scratch (sr, ak, depth), `entries` each; growing synchronises the stream
+int grow_spectrum_scratch(bls_plan *p, int64_t entries, cudaStream_t st)
+{
+    if (entries <= p->cap_entries && p->d_sr) return BLS_OK;
+    if (p->d_sr) BLS_CUDA(p, cudaStreamSynchronize(st));
+    release(p->d_sr); release(p->d_ak); release(p->d_depth);
+    p->bytes_owned -= p->cap_entries * 12;
+    p->cap_entries = 0;
+    BLS_CUDA(p, cudaMalloc(&p->d_sr, (size_t)entries * sizeof(float)));
+    BLS_CUDA(p, cudaMalloc(&p->d_ak, (size_t)entries * sizeof(uint32_t)));
+    BLS_CUDA(p, cudaMalloc(&p->d_depth, (size_t)entries * sizeof(float)));
+    p->cap_entries = entries;
+    p->bytes_owned += entries * 12;
+    return BLS_OK;
 }
 
 void widths_from_q(int nb, double qmin, double qmax, int *kmin, int *kmax)
@@ -189,7 +292,7 @@ int bls_plan_destroy(bls_plan *p)
     release(p->d_freqs); release(p->d_pts); release(p->d_meta); release(p->d_offsets);
     release(p->d_origin); release(p->d_cand); release(p->d_sr); release(p->d_ak); release(p->d_depth);
     release(p->d_canon); release(p->d_ht); release(p->d_hmag); release(p->d_hsig);
-    release(p->d_hpeaks); release(p->d_hstatus);
+    release(p->d_hpeaks); release(p->d_hstatus); release(p->d_sr_stats); release(p->d_flo); release(p->d_fstep);
     for (cudaEvent_t e : p->ev) cudaEventDestroy(e);
     delete p;
     return BLS_OK;
@@ -262,15 +365,16 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     {
         if (nc > p->cap_curves || !p->d_meta) {
             if (p->d_meta) BLS_CUDA(p, cudaStreamSynchronize(st));
-            release(p->d_meta); release(p->d_offsets); release(p->d_origin); release(p->d_cand);
-            p->bytes_owned -= p->cap_curves * (int64_t)(sizeof(CurveMeta) + 16 + sizeof(PeakCand) * p->max_top_k);
+            release(p->d_meta); release(p->d_offsets); release(p->d_origin); release(p->d_cand); release(p->d_sr_stats);
+            p->bytes_owned -= p->cap_curves * (int64_t)(sizeof(CurveMeta) + 32 + sizeof(PeakCand) * p->max_top_k);
             p->cap_curves = 0;
             BLS_CUDA(p, cudaMalloc(&p->d_meta, (size_t)nc * sizeof(CurveMeta)));
             BLS_CUDA(p, cudaMalloc(&p->d_offsets, (size_t)(nc + 1) * sizeof(int64_t)));
             BLS_CUDA(p, cudaMalloc(&p->d_origin, (size_t)nc * sizeof(double)));
             BLS_CUDA(p, cudaMalloc(&p->d_cand, (size_t)nc * p->max_top_k * sizeof(PeakCand)));
+            BLS_CUDA(p, cudaMalloc(&p->d_sr_stats, (size_t)nc * sizeof(double2)));
             p->cap_curves = nc;
-            p->bytes_owned += nc * (int64_t)(sizeof(CurveMeta) + 16 + sizeof(PeakCand) * p->max_top_k);
+            p->bytes_owned += nc * (int64_t)(sizeof(CurveMeta) + 32 + sizeof(PeakCand) * p->max_top_k);
         }
     }
     if ((rc = grow(p, p->d_pts, p->cap_pts, npts, true, st)) != BLS_OK) return rc;
@@ -279,17 +383,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     int64_t chunk = p->scratch_budget / per_curve;
     if (chunk < 1) chunk = 1;
     if (chunk > nc) chunk = nc;
-    if (chunk > p->cap_chunk || !p->d_sr) {
-        if (p->d_sr) BLS_CUDA(p, cudaStreamSynchronize(st));
-        release(p->d_sr); release(p->d_ak); release(p->d_depth);
-        p->bytes_owned -= p->cap_chunk * per_curve;
-        p->cap_chunk = 0;
-        BLS_CUDA(p, cudaMalloc(&p->d_sr, (size_t)(chunk * p->nf) * sizeof(float)));
-        BLS_CUDA(p, cudaMalloc(&p->d_ak, (size_t)(chunk * p->nf) * sizeof(uint32_t)));
-        BLS_CUDA(p, cudaMalloc(&p->d_depth, (size_t)(chunk * p->nf) * sizeof(float)));
-        p->cap_chunk = chunk;
-        p->bytes_owned += chunk * per_curve;
-    }
+    if ((rc = grow_spectrum_scratch(p, chunk * p->nf, st)) != BLS_OK) return rc;
 
     // ---- metadata to the device (stream ordered; the caller keeps offsets alive until then) ------
     BLS_CUDA(p, cudaMemcpyAsync(p->d_offsets, b->offsets, (size_t)(nc + 1) * sizeof(int64_t),
@@ -306,73 +400,16 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     p->last_launches += 1;
 
     // ---- launch geometry of the search ---------------------------------------------------------
-    const int ntiles = (int)((p->nf + kTileFreqs - 1) / kTileFreqs);
-    const size_t optin = (size_t)p->max_smem_optin;
-    const size_t sm_smem = (size_t)p->max_smem_sm;
-    const int warps_flag = (int)((p->flags >> 8) & 0xffu);
-    const int fold_flag = (int)((p->flags >> 16) & 0xffu);
-    // Kernel 2 (warp-specialised, two bin buffers) whenever its buffers fit shared memory, with the
-    // curve staged in shared memory if that fits too; otherwise kernel 1 (one buffer, two CTAs per SM).
-    int ws_search = kWsSearchWarps;
-    if (warps_flag >= 1 && warps_flag <= kWsMaxWarps - 1) ws_search = warps_flag;
-    int ws_fold = kWsMaxWarps - ws_search;
-    if (fold_flag >= 1 && fold_flag < ws_fold) ws_fold = fold_flag;
-    const bool ws = !(p->flags & BLS_FLAG_SINGLE_BUFFER) &&
-                    search_smem_bytes(p->nb, p->kmax, ws_search, 2, 0) <= optin;
-    int k1_warps = kMaxSearchWarps;
-    if (warps_flag >= 1 && warps_flag <= kMaxSearchWarps) k1_warps = warps_flag;
-    const int warps = ws ? ws_search : k1_warps;            // warps that walk the boxes
-    const int buffers = ws ? 2 : 1;
-    int pts_in_smem = 1;
-    size_t smem = search_smem_bytes(p->nb, p->kmax, warps, buffers, max_n);
-    if (smem > optin) {                            // curve too long to stage: read it through L1/L2
-        pts_in_smem = 0;
-        smem = search_smem_bytes(p->nb, p->kmax, warps, buffers, 0);
-    }
-    if (smem > optin) return BLS_ERR_UNSUPPORTED;
-    int threads = (ws ? ws_search + ws_fold : k1_warps) * 32;
-    int kernel = ws ? 2 : 1;
-    int nrows = search_rows_for(p->nb, p->kmax, 2 * warps);
-    // Kernel 3 (one warp per tile, warp-private bins) for small shapes: when two CTAs of kWtWarps
-    // warps, each with the curve staged, fit an SM.  There a tile is too little work to pay for the
-    // hand-offs of kernels 1 and 2 (C4: 200 epochs, 64 bins).
-    const int wt_rows = search_rows_for(p->nb, p->kmax, 2);
-    const size_t wt_smem = (size_t)kWtWarps * ((size_t)wt_rows * kTileFreqs * 8 + 256) + (size_t)max_n * sizeof(PointRec);
-    const bool wt_fits = 2 * (wt_smem + 1024) <= sm_smem;
-    if (!(p->flags & (BLS_FLAG_SINGLE_BUFFER | BLS_FLAG_NO_WARP_PER_TILE)) && wt_fits) {
-        kernel = 3; smem = wt_smem; pts_in_smem = 1; threads = kWtWarps * 32; nrows = wt_rows;
-    }
-    int ctas_per_sm = (int)(sm_smem / (smem + 1024));
-    if (ctas_per_sm < 1) ctas_per_sm = 1;
-    const int max_ctas = kernel == 2 ? 1 : 2;                       // register-limited (launch bounds)
-    if (ctas_per_sm > max_ctas) ctas_per_sm = max_ctas;
-    const int waves = kernel == 1 ? 12 : 24;                        // enough waves to hide the tail
-    const int64_t target_ctas = (int64_t)p->sm_count * ctas_per_sm * waves;
-    int64_t items = (target_ctas + chunk - 1) / chunk;
-    if (items < 1) items = 1;
-    if (items > ntiles) items = ntiles;
-    int tiles_per_item = (int)((ntiles + items - 1) / items);
-    items = (ntiles + tiles_per_item - 1) / tiles_per_item;
-    p->last_tiles_per_item = tiles_per_item;
-    p->last_kernel = kernel;
-
-    SearchArgs a;
-    a.pts = p->d_pts; a.offsets = p->d_offsets; a.meta = p->d_meta; a.freqs = p->d_freqs;
-    a.nf = (int)p->nf; a.nb = p->nb; a.kmin = p->kmin; a.kmax = p->kmax;
-    a.tiles_per_item = tiles_per_item; a.items_per_curve = (int)items;
-    a.pts_in_smem = pts_in_smem;
-    a.nrows = nrows;
-    a.search_warps = kernel == 2 ? ws_search : 0;
-    a.kernel = kernel;
-    a.threads = threads;
-    a.force_canonical = (p->flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0;
-    a.sr = p->d_sr; a.ak = p->d_ak; a.depth = p->d_depth;
+    SearchLaunch L;
+    if ((rc = search_launch_setup(p, p->nf, max_n, chunk, L)) != BLS_OK) return rc;
+    SearchArgs &a = L.a;
+    const size_t smem = L.smem;
+    const int64_t items = L.items;
     a.u_sr = out ? out->sr : nullptr;
     a.u_start = out ? out->best_start : nullptr;
     a.u_width = out ? out->best_width : nullptr;
     a.u_depth = out ? out->depth : nullptr;
-    a.canon_count = p->d_canon;
-    a.debug = (int)(p->flags >> 24);
+    p->last_max_n = max_n;
 
     // ---- per chunk of curves: search -> peak candidates ------------------------------------------
     p->last_search_ctas = 0;
@@ -390,7 +427,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
         BLS_CUDA(p, cudaEventRecord(p->ev[p->ev_used + 1], st));
         p->ev_used += 2;
         BLS_CUDA(p, launch_peaks(p->d_sr, p->d_ak, p->d_depth, p->d_meta, base, cc, (int)p->nf,
-                                 p->max_top_k, p->d_cand, st));
+                                 p->max_top_k, p->d_cand, p->d_sr_stats, st));
         p->last_launches += 2;
         p->last_search_ctas += cc * items;
     }
@@ -470,6 +507,52 @@ int bls_topk(bls_plan *p, int32_t k, bls_peak *peaks, void *cuda_stream)
     BLS_CUDA(p, cudaSetDevice(p->device));
     BLS_CUDA(p, launch_format_peaks(p->d_cand, p->max_top_k, k, p->last_n_curves, p->nb, p->d_freqs,
                                     p->last_has_origin ? p->d_origin : nullptr, peaks, st));
+    p->last_launches += 1;
+    return BLS_OK;
+}
+
+int bls_refine(bls_plan *p, int32_t k, int32_t n_fine, int32_t n_shift, bls_refined_peak *out, void *cuda_stream)
+{
+    if (!p || !out) return BLS_ERR_NULL;
+    if (p->last_n_curves < 0) return BLS_ERR_ARG;
+    if (k < 1 || k > p->max_top_k) return BLS_ERR_ARG;
+    if (n_fine < 1 || n_fine > 256 || n_shift < 1 || n_shift > 8) return BLS_ERR_ARG;
+    const int64_t nc = p->last_n_curves;
+    if (nc == 0) return BLS_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    BLS_CUDA(p, cudaSetDevice(p->device));
+    int rc;
+    if (nc * k > p->cap_refine || !p->d_flo) {
+        if (p->d_flo) BLS_CUDA(p, cudaStreamSynchronize(st));
+        release(p->d_flo); release(p->d_fstep);
+        p->bytes_owned -= p->cap_refine * 16;
+        p->cap_refine = 0;
+        BLS_CUDA(p, cudaMalloc(&p->d_flo, (size_t)(nc * k) * sizeof(double)));
+        BLS_CUDA(p, cudaMalloc(&p->d_fstep, (size_t)(nc * k) * sizeof(double)));
+        p->cap_refine = nc * k;
+        p->bytes_owned += nc * k * 16;
+    }
+    // the fine spectrum of a chunk of curves reuses the spectrum scratch of bls_run: [chunk][k*n_fine*n_shift]
+    const int64_t nf = (int64_t)k * n_fine * n_shift;
+    int64_t chunk = p->scratch_budget / (nf * 12);
+    if (chunk < 1) chunk = 1;
+    if (chunk > nc) chunk = nc;
+    if ((rc = grow_spectrum_scratch(p, chunk * nf, st)) != BLS_OK) return rc;
+    BLS_CUDA(p, launch_refine_grid(p->d_cand, p->max_top_k, k, nc, (int)p->nf, n_fine, p->d_freqs, p->d_flo, p->d_fstep, st));
+    SearchLaunch L;
+    if ((rc = search_launch_setup(p, nf, p->last_max_n, chunk, L)) != BLS_OK) return rc;
+    SearchArgs &a = L.a;
+    a.f_lo = p->d_flo; a.f_step = p->d_fstep; a.refine_k = k; a.n_fine = n_fine; a.n_shift = n_shift;
+    a.canon_count = nullptr;
+    for (int64_t base = 0; base < nc; base += chunk) {
+        const int64_t cc = (nc - base < chunk) ? nc - base : chunk;
+        a.curve_base = base;
+        BLS_CUDA(p, launch_search(a, cc, L.smem, st));
+        BLS_CUDA(p, launch_refine_reduce(p->d_sr, p->d_ak, p->d_depth, p->d_cand, p->max_top_k, k, base, cc, n_fine, n_shift,
+                                         p->nb, p->d_flo, p->d_fstep, p->d_sr_stats, p->last_has_origin ? p->d_origin : nullptr,
+                                         out, st));
+        p->last_launches += 2;
+    }
     p->last_launches += 1;
     return BLS_OK;
 }

@@ -52,7 +52,10 @@ struct SearchArgs {
     const PointRec *pts;        // [n_points] prepared points of the whole batch
     const int64_t *offsets;     // device copy of the CSR offsets
     const CurveMeta *meta;      // [n_curves]
-    const double *freqs;        // [nf]
+    const double *freqs;        // [nf] the plan's grid (search mode)
+    const double *f_lo;         // refine mode (n_fine > 0): [n_curves][refine_k] first fine frequency of each peak
+    const double *f_step;       //                           and its fine step
+    int refine_k, n_fine, n_shift;
     int nf, nb, kmin, kmax;
     int tiles_per_item, items_per_curve;
     int64_t curve_base;         // first curve of this chunk
@@ -77,16 +80,16 @@ constexpr double kPhaseMagic = 1572864.0;   // 1.5 * 2^20: ulp = 2^-32, valid fo
 
 #ifdef __CUDACC__
 // Reading R8, the canonical rule: three individually rounded fp64 operations, no FMA.
-__device__ __noinline__ int canonical_bin(double f, double t, int nb);
+__device__ __noinline__ int canonical_bin(double f, double t, int nb, double shift);
 
 // Fast phase.  y = RN(f t + 1.5*2^20) has ulp 2^-32, so its low
 // mantissa word is frac(f t) in units of 2^-32 cycle (error <= 2^-33 cycle, one rounding).
 // ph * nb as a 64-bit product = (bin, position inside the bin in units of 2^-32 bin).  If the
 // position is within G = nb + 8 units of a bin edge the canonical rule decides instead; outside
 // the guard band both rules provably give floor(nb frac(f t)) (needs |f t| < 2^18).
-__device__ __forceinline__ int fast_bin(double f, double t, int nb, uint32_t G, uint32_t &lo)
+__device__ __forceinline__ int fast_bin(double f, double t, int nb, uint32_t G, uint32_t &lo, double magic)
 {
-    const double y = fma(f, t, kPhaseMagic);
+    const double y = fma(f, t, magic);
     const uint32_t ph = (uint32_t)__double2loint(y);
     const unsigned long long pr = (unsigned long long)ph * (uint32_t)nb + (unsigned long long)G;
     lo = (uint32_t)pr;                                 // position * 2^32 + G
@@ -94,20 +97,20 @@ __device__ __forceinline__ int fast_bin(double f, double t, int nb, uint32_t G, 
 }
 
 // Same, returning the whole product: high word = bin, low word = position * 2^32 + G.
-__device__ __forceinline__ unsigned long long fast_bin_pos(double f, double t, int nb, uint32_t G)
+__device__ __forceinline__ unsigned long long fast_bin_pos(double f, double t, int nb, uint32_t G, double magic)
 {
-    const double y = fma(f, t, kPhaseMagic);
+    const double y = fma(f, t, magic);
     const uint32_t ph = (uint32_t)__double2loint(y);
     return (unsigned long long)ph * (uint32_t)nb + (unsigned long long)G;
 }
 
 __device__ __forceinline__ int fold_bin(double f, double t, int nb, uint32_t G, bool force_canon,
-                                        unsigned int &n_canon)
+                                        unsigned int &n_canon, double magic, double shift)
 {
     uint32_t lo;
-    int bin = fast_bin(f, t, nb, G, lo);
+    int bin = fast_bin(f, t, nb, G, lo, magic);
     if (force_canon || lo < 2u * G) {
-        bin = canonical_bin(f, t, nb);
+        bin = canonical_bin(f, t, nb, shift);
         ++n_canon;
     }
     return bin;
@@ -163,7 +166,13 @@ cudaError_t launch_variability(const float *t, const float *mag, const float *si
 cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem, cudaStream_t st);
 cudaError_t launch_peaks(const float *sr, const uint32_t *ak, const float *depth, const CurveMeta *meta,
                          int64_t curve_base, int64_t chunk_curves, int nf, int max_k, PeakCand *cand,
-                         cudaStream_t st);
+                         double2 *sr_stats, cudaStream_t st);
+cudaError_t launch_refine_grid(const PeakCand *cand, int max_k, int k, int64_t n_curves, int nf, int n_fine,
+                               const double *freqs, double *f_lo, double *f_step, cudaStream_t st);
+cudaError_t launch_refine_reduce(const float *sr, const uint32_t *ak, const float *depth, const PeakCand *cand, int max_k,
+                                 int k, int64_t curve_base, int64_t chunk_curves, int n_fine, int n_shift, int nb,
+                                 const double *f_lo, const double *f_step, const double2 *sr_stats, const double *t_origin,
+                                 bls_refined_peak *out, cudaStream_t st);
 cudaError_t launch_format_peaks(const PeakCand *cand, int max_k, int k, int64_t n_curves, int nb,
                                 const double *freqs, const double *t_origin, bls_peak *out, cudaStream_t st);
 

@@ -52,9 +52,9 @@ size_t search_smem_bytes(int nb, int kmax, int warps, int buffers, int64_t n_poi
     return (size_t)buffers * bins + cand + (size_t)n_points_in_smem * sizeof(PointRec);
 }
 
-__device__ __noinline__ int canonical_bin(double f, double t, int nb)
+__device__ __noinline__ int canonical_bin(double f, double t, int nb, double shift)
 {
-    double p = __dmul_rn(f, t);
+    double p = __dsub_rn(__dmul_rn(f, t), shift);        // shift = 0 (the plain rule R8) subtracts exactly nothing
     double phi = __dsub_rn(p, floor(p));
     double xb = __dmul_rn(phi, (double)nb);
     int b = (int)xb;
@@ -153,6 +153,35 @@ static_assert(kRowBytes == 256, "row_addr hard-codes the row pitch");
 // ---- the phases of one tile (32 trial frequencies, one per lane), written for a GROUP of warps:
 //      `gw` = this warp's index in the group, `gnw` = warps in the group -------------------------
 
+// The trial frequency of a lane and the shift of its bin grid (0 except in bls_refine, reading S3).
+struct LaneFreq {
+    double f;        // cycles/day
+    double shift;    // cycles; the bin grid starts at phase `shift`
+    double magic;    // kPhaseMagic - shift: the fast phase's additive constant
+};
+
+// Frequency index q of curve cv.  Search mode: the plan's grid.  Refine mode (a.n_fine > 0): q =
+// (peak * n_fine + j) * n_shift + h -> f = f_lo + j * step (two roundings, as the oracle's S2),
+// shift = h / (n_shift * nb).  Indices past the end repeat the last one (ragged last tile).
+__device__ __forceinline__ LaneFreq lane_freq(const SearchArgs &a, int64_t cv, int q)
+{
+    LaneFreq lf;
+    q = min(q, a.nf - 1);
+    if (a.n_fine > 0) {
+        const int per_peak = a.n_fine * a.n_shift;
+        const int peak = q / per_peak, rem = q - peak * per_peak;
+        const int j = rem / a.n_shift, h = rem - j * a.n_shift;
+        const int64_t pi = cv * a.refine_k + peak;
+        lf.f = __dadd_rn(a.f_lo[pi], __dmul_rn((double)j, a.f_step[pi]));
+        lf.shift = __ddiv_rn((double)h, (double)(a.n_shift * a.nb));
+    } else {
+        lf.f = a.freqs[q];
+        lf.shift = 0.0;
+    }
+    lf.magic = kPhaseMagic - lf.shift;
+    return lf;
+}
+
 struct TileCtx {
     int nb, nrows, kmin, kmax, n;
     uint32_t G;
@@ -168,7 +197,9 @@ __device__ __forceinline__ void load_ctx(TileCtx &c, const SearchArgs &a, const 
     c.force_canon = (a.force_canonical != 0) || (meta.force_canonical != 0);
     c.ncw = meta.ncw; c.cy = meta.cy; c.wx2 = (float)meta.wx2;
     c.swt = meta.swt; c.sr_scale = meta.sr_scale; c.dp_scale = meta.dp_scale;
-    c.G = (uint32_t)a.nb + 8u;                    // guard band, units of 2^-32 bin
+    // guard band, units of 2^-32 bin: fast phase error nb/2 (nb with a shifted grid: kPhaseMagic - shift
+    // rounds the shift to 2^-32 cycle) + canonical rule error nb/8
+    c.G = a.n_fine > 0 ? 2u * (uint32_t)a.nb + 8u : (uint32_t)a.nb + 8u;
 }
 
 __device__ __forceinline__ void zero_bins(uint32_t bins_s, int nb, int gtid, int gthreads)
@@ -181,7 +212,7 @@ __device__ __forceinline__ void zero_bins(uint32_t bins_s, int nb, int gtid, int
 // NG groups of 4 consecutive points (group g at shared address pa + g*step) folded at frequency f:
 // all loads first, then the phases, then the atomics, so 4*NG points are in flight per warp.
 template <int NG>
-__device__ __forceinline__ void fold_groups(const TileCtx &c, double f, uint32_t colw, uint32_t pa, uint32_t step,
+__device__ __forceinline__ void fold_groups(const TileCtx &c, const LaneFreq &lf, uint32_t colw, uint32_t pa, uint32_t step,
                                             unsigned int &n_canon)
 {
     constexpr int NP = 4 * NG;
@@ -194,7 +225,7 @@ __device__ __forceinline__ void fold_groups(const TileCtx &c, double f, uint32_t
     uint32_t lomin = 0xffffffffu;
 #pragma unroll
     for (int u = 0; u < NP; ++u) {
-        pr[u] = fast_bin_pos(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb, G);
+        pr[u] = fast_bin_pos(lf.f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb, G, lf.magic);
         lomin = min(lomin, (uint32_t)pr[u]);
     }
     if (!c.force_canon && lomin >= 2u * G) {
@@ -209,7 +240,7 @@ __device__ __forceinline__ void fold_groups(const TileCtx &c, double f, uint32_t
         for (int u = 0; u < NP; ++u) {
             int bin = (int)(pr[u] >> 32);
             if (c.force_canon || (uint32_t)pr[u] < 2u * G) {
-                bin = canonical_bin(f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb);
+                bin = canonical_bin(lf.f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb, lf.shift);
                 ++n_canon;
             }
             const uint32_t addr = colw + bin * kRowBytes;
@@ -224,7 +255,7 @@ __device__ __forceinline__ void fold_groups(const TileCtx &c, double f, uint32_t
 // hits bank l (and Y sits 128 B after W, one address register), so the native ATOMS.ADD is
 // conflict-free by construction.  Four points in flight hide the LDS / DFMA latency.
 template <bool PTS_SMEM, int NG = 1>
-__device__ __forceinline__ void fold_tile(const TileCtx &c, double f, uint32_t bins_s, uint32_t pts_sa,
+__device__ __forceinline__ void fold_tile(const TileCtx &c, const LaneFreq &lf, uint32_t bins_s, uint32_t pts_sa,
                                           const PointRec *pts_g, int lane, int gw, int gnw, unsigned int &n_canon)
 {
     const int nb = c.nb;
@@ -236,8 +267,8 @@ __device__ __forceinline__ void fold_tile(const TileCtx &c, double f, uint32_t b
         const uint32_t pa_end = pts_sa + ngroups * 64, step = gnw * 64;
         uint32_t pa = pts_sa + gw * 64;
         if (NG == 2)
-            for (; pa + step < pa_end; pa += 2 * step) fold_groups<2>(c, f, colw, pa, step, n_canon);
-        for (; pa < pa_end; pa += step) fold_groups<1>(c, f, colw, pa, step, n_canon);
+            for (; pa + step < pa_end; pa += 2 * step) fold_groups<2>(c, lf, colw, pa, step, n_canon);
+        for (; pa < pa_end; pa += step) fold_groups<1>(c, lf, colw, pa, step, n_canon);
     } else {
         for (int g = gw; g < ngroups; g += gnw) {
             PointRec p[4];
@@ -246,11 +277,11 @@ __device__ __forceinline__ void fold_tile(const TileCtx &c, double f, uint32_t b
 #pragma unroll
             for (int u = 0; u < 4; ++u) p[u] = load_point<false>(pts_g + g * 4 + u);
 #pragma unroll
-            for (int u = 0; u < 4; ++u) bin[u] = fast_bin(f, p[u].t, nb, G, lo[u]);
+            for (int u = 0; u < 4; ++u) bin[u] = fast_bin(lf.f, p[u].t, nb, G, lo[u], lf.magic);
             if (force_canon || min(min(lo[0], lo[1]), min(lo[2], lo[3])) < 2u * G) {
 #pragma unroll
                 for (int u = 0; u < 4; ++u)
-                    if (force_canon || lo[u] < 2u * G) { bin[u] = canonical_bin(f, p[u].t, nb); ++n_canon; }
+                    if (force_canon || lo[u] < 2u * G) { bin[u] = canonical_bin(lf.f, p[u].t, nb, lf.shift); ++n_canon; }
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
@@ -269,7 +300,7 @@ __device__ __forceinline__ void fold_tile(const TileCtx &c, double f, uint32_t b
             } else {
                 p = load_point<false>(pts_g + i);
             }
-            const int bin = fold_bin(f, p.t, nb, G, force_canon, n_canon);
+            const int bin = fold_bin(lf.f, p.t, nb, G, force_canon, n_canon, lf.magic, lf.shift);
             const uint32_t addr = colw + bin * kRowBytes;
             red_add(addr, p.qw);
             red_add(addr + 128, (uint32_t)p.qy);
@@ -783,10 +814,10 @@ search_kernel(const SearchArgs a)
 
     for (int tile = w.tile0; tile < w.tile1; ++tile) {
         const int q0 = tile * kTileFreqs;
-        const double f = a.freqs[min(q0 + lane, a.nf - 1)];   // ragged last tile: surplus lanes repeat the last f
+        const LaneFreq lf = lane_freq(a, w.cv, q0 + lane);      // ragged last tile: surplus lanes repeat the last f
         zero_bins(bins_s, c.nb, tid, nthr);
         __syncthreads();
-        fold_tile<PTS_SMEM>(c, f, bins_s, pts_sa, pts_g, lane, warp, nw, n_canon);
+        fold_tile<PTS_SMEM>(c, lf, bins_s, pts_sa, pts_g, lane, warp, nw, n_canon);
         __syncthreads();
         extend_rows(c, bins_s, tid, nthr);
         __syncthreads();
@@ -869,10 +900,10 @@ search_ws_kernel(const SearchArgs a)
             const int b = it & 1, tile = w.tile0 + it;
             const uint32_t buf = bins_s + b * (uint32_t)buf_bytes;
             if (it >= 2) merge(it - 2);
-            const double f = a.freqs[min(tile * kTileFreqs + lane, a.nf - 1)];
+            const LaneFreq lf = lane_freq(a, w.cv, tile * kTileFreqs + lane);
             zero_bins(buf, c.nb, gtid, gthreads);
             named_sync(kBarFoldGroup, gthreads);
-            if (!(a.debug & 2)) fold_tile<PTS_SMEM>(c, f, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
+            if (!(a.debug & 2)) fold_tile<PTS_SMEM>(c, lf, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
             named_sync(kBarFoldGroup, gthreads);
             extend_rows(c, buf, gtid, gthreads);
             named_arrive(kBarFull0 + b, nthr);
@@ -915,10 +946,10 @@ search_wt_kernel(const SearchArgs a)
 
     for (int tile = w.tile0 + warp; tile < w.tile1; tile += nw) {
         const int q0 = tile * kTileFreqs;
-        const double f = a.freqs[min(q0 + lane, a.nf - 1)];
+        const LaneFreq lf = lane_freq(a, w.cv, q0 + lane);
         zero_bins(buf, c.nb, lane, 32);
         __syncwarp();
-        fold_tile<PTS_SMEM, 2>(c, f, buf, pts_sa, pts_g, lane, 0, 1, n_canon);
+        fold_tile<PTS_SMEM, 2>(c, lf, buf, pts_sa, pts_g, lane, 0, 1, n_canon);
         __syncwarp();
         extend_rows(c, buf, lane, 32);
         __syncwarp();
@@ -939,7 +970,7 @@ __global__ void debug_bins_kernel(const double *__restrict__ f, const double *__
     const uint32_t G = (uint32_t)nb + 8u;
     unsigned int n_canon = 0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        bins[i] = fold_bin(f[i], t[i], nb, G, force_canon != 0, n_canon);
+        bins[i] = fold_bin(f[i], t[i], nb, G, force_canon != 0, n_canon, kPhaseMagic, 0.0);
     if (n_canon && n_canon_out) atomicAdd(n_canon_out, (unsigned long long)n_canon);
 }
 
