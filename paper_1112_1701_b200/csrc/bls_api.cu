@@ -3,6 +3,7 @@
 // bls_search.cu and bls_peaks.cu; this file only validates, allocates and enqueues.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -29,6 +30,8 @@ struct bls_plan {
     PointRec *d_pts = nullptr;      int64_t cap_pts = 0;
     CurveMeta *d_meta = nullptr;    int64_t cap_curves = 0;
     int64_t *d_offsets = nullptr;
+    int64_t *d_poffsets = nullptr;  // offsets of the prepared records (each curve padded to a multiple of 4)
+    int64_t *h_poffsets = nullptr;  int64_t cap_hpoff = 0;   // host staging of those
     double *d_origin = nullptr;
     PeakCand *d_cand = nullptr;
     float *d_sr = nullptr;          int64_t cap_entries = 0; // (sr, ak, depth) entries the spectrum scratch holds
@@ -159,7 +162,7 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     p->last_tiles_per_item = tiles_per_item;
     p->last_kernel = kernel;
 
-    a.pts = p->d_pts; a.offsets = p->d_offsets; a.meta = p->d_meta; a.freqs = p->d_freqs;
+    a.pts = p->d_pts; a.offsets = p->d_offsets; a.poffsets = p->d_poffsets; a.meta = p->d_meta; a.freqs = p->d_freqs;
     a.nf = (int)nf; a.nb = p->nb; a.kmin = p->kmin; a.kmax = p->kmax;
     a.tiles_per_item = tiles_per_item; a.items_per_curve = (int)items;
     a.pts_in_smem = pts_in_smem;
@@ -289,7 +292,8 @@ int bls_plan_destroy(bls_plan *p)
 {
     if (!p) return BLS_OK;
     cudaSetDevice(p->device);
-    release(p->d_freqs); release(p->d_pts); release(p->d_meta); release(p->d_offsets);
+    release(p->d_freqs); release(p->d_pts); release(p->d_meta); release(p->d_offsets); release(p->d_poffsets);
+    free(p->h_poffsets);
     release(p->d_origin); release(p->d_cand); release(p->d_sr); release(p->d_ak); release(p->d_depth);
     release(p->d_canon); release(p->d_ht); release(p->d_hmag); release(p->d_hsig);
     release(p->d_hpeaks); release(p->d_hstatus); release(p->d_sr_stats); release(p->d_flo); release(p->d_fstep);
@@ -345,12 +349,22 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     if (!b->offsets) return BLS_ERR_NULL;
     const int64_t nc = b->n_curves;
     if (b->offsets[0] != 0) return BLS_ERR_BATCH;
-    int64_t max_n = 0;
+    if (nc + 1 > p->cap_hpoff) {
+        free(p->h_poffsets);
+        p->h_poffsets = (int64_t *)malloc((size_t)(nc + 1) * sizeof(int64_t));
+        p->cap_hpoff = p->h_poffsets ? nc + 1 : 0;
+        if (!p->h_poffsets) return BLS_ERR_CUDA;
+    }
+    int64_t max_n = 0, nrec = 0;
     for (int64_t c = 0; c < nc; ++c) {
         const int64_t n = b->offsets[c + 1] - b->offsets[c];
         if (n < 0 || n > 2147483647LL / 64) return BLS_ERR_BATCH;
         if (n > max_n) max_n = n;
+        p->h_poffsets[c] = nrec;
+        nrec += (n + 3) & ~(int64_t)3;
     }
+    p->h_poffsets[nc] = nrec;
+    max_n = (max_n + 3) & ~(int64_t)3;                      // records per curve, padded
     const int64_t npts = b->offsets[nc];
     if (npts > 0 && (!b->t || !b->mag || !b->sigma)) return BLS_ERR_NULL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -365,19 +379,21 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     {
         if (nc > p->cap_curves || !p->d_meta) {
             if (p->d_meta) BLS_CUDA(p, cudaStreamSynchronize(st));
-            release(p->d_meta); release(p->d_offsets); release(p->d_origin); release(p->d_cand); release(p->d_sr_stats);
-            p->bytes_owned -= p->cap_curves * (int64_t)(sizeof(CurveMeta) + 32 + sizeof(PeakCand) * p->max_top_k);
+            release(p->d_meta); release(p->d_offsets); release(p->d_poffsets); release(p->d_origin); release(p->d_cand);
+            release(p->d_sr_stats);
+            p->bytes_owned -= p->cap_curves * (int64_t)(sizeof(CurveMeta) + 40 + sizeof(PeakCand) * p->max_top_k);
             p->cap_curves = 0;
             BLS_CUDA(p, cudaMalloc(&p->d_meta, (size_t)nc * sizeof(CurveMeta)));
             BLS_CUDA(p, cudaMalloc(&p->d_offsets, (size_t)(nc + 1) * sizeof(int64_t)));
+            BLS_CUDA(p, cudaMalloc(&p->d_poffsets, (size_t)(nc + 1) * sizeof(int64_t)));
             BLS_CUDA(p, cudaMalloc(&p->d_origin, (size_t)nc * sizeof(double)));
             BLS_CUDA(p, cudaMalloc(&p->d_cand, (size_t)nc * p->max_top_k * sizeof(PeakCand)));
             BLS_CUDA(p, cudaMalloc(&p->d_sr_stats, (size_t)nc * sizeof(double2)));
             p->cap_curves = nc;
-            p->bytes_owned += nc * (int64_t)(sizeof(CurveMeta) + 32 + sizeof(PeakCand) * p->max_top_k);
+            p->bytes_owned += nc * (int64_t)(sizeof(CurveMeta) + 40 + sizeof(PeakCand) * p->max_top_k);
         }
     }
-    if ((rc = grow(p, p->d_pts, p->cap_pts, npts, true, st)) != BLS_OK) return rc;
+    if ((rc = grow(p, p->d_pts, p->cap_pts, nrec, true, st)) != BLS_OK) return rc;
 
     const int64_t per_curve = p->nf * 12;                       // sr + ak + depth
     int64_t chunk = p->scratch_budget / per_curve;
@@ -388,6 +404,8 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     // ---- metadata to the device (stream ordered; the caller keeps offsets alive until then) ------
     BLS_CUDA(p, cudaMemcpyAsync(p->d_offsets, b->offsets, (size_t)(nc + 1) * sizeof(int64_t),
                                 cudaMemcpyHostToDevice, st));
+    BLS_CUDA(p, cudaMemcpyAsync(p->d_poffsets, p->h_poffsets, (size_t)(nc + 1) * sizeof(int64_t),
+                                cudaMemcpyHostToDevice, st));
     p->last_has_origin = b->t_origin != nullptr;
     if (b->t_origin)
         BLS_CUDA(p, cudaMemcpyAsync(p->d_origin, b->t_origin, (size_t)nc * sizeof(double),
@@ -395,7 +413,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     BLS_CUDA(p, cudaMemsetAsync(p->d_canon, 0, sizeof(unsigned long long), st));
 
     // ---- a0 prep -------------------------------------------------------------------------------
-    BLS_CUDA(p, launch_prep(b->t, b->mag, b->sigma, p->d_offsets, nc, p->fmax, p->d_pts, p->d_meta,
+    BLS_CUDA(p, launch_prep(b->t, b->mag, b->sigma, p->d_offsets, p->d_poffsets, nc, p->fmax, p->d_pts, p->d_meta,
                             out ? out->status : nullptr, st));
     p->last_launches += 1;
 

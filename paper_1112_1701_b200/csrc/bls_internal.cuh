@@ -25,7 +25,9 @@ struct CurveMeta {
     int32_t status;    // BLS_CURVE_*
     int32_t force_canonical;  // 1: |f t| may reach 2^18 cycles, the fast phase is not valid
     uint32_t swt;      // sum_i qw_i (exact; < 2^32)
-    uint32_t pad_;
+    uint32_t w0;       // sum of qw over the zero-time points (t == 0), which are not in the record list
+    int32_t y0;        // sum of qy over them
+    int32_t pad_;
     double sr_scale;   // SWT^2 / SY^2   (0 for a constant curve)
     double dp_scale;   // SWT^2 / SY
     double wx2;        // sum_i w_i x_i^2  (upper bound of SR)
@@ -51,6 +53,7 @@ constexpr int kPeakThreads = 256;
 struct SearchArgs {
     const PointRec *pts;        // [n_points] prepared points of the whole batch
     const int64_t *offsets;     // device copy of the CSR offsets
+    const int64_t *poffsets;    // [n_curves+1] offsets of the prepared records (each curve padded to a multiple of 4)
     const CurveMeta *meta;      // [n_curves]
     const double *freqs;        // [nf] the plan's grid (search mode)
     const double *f_lo;         // refine mode (n_fine > 0): [n_curves][refine_k] first fine frequency of each peak
@@ -156,8 +159,8 @@ cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int n
                               int32_t *bins, unsigned long long *n_canon, int sm_count, cudaStream_t st);
 cudaError_t search_configure(int max_smem_optin);
 cudaError_t launch_prep(const float *t, const float *mag, const float *sigma, const int64_t *offsets,
-                        int64_t n_curves, double fmax, PointRec *pts, CurveMeta *meta, int32_t *u_status,
-                        cudaStream_t st);
+                        const int64_t *poffsets, int64_t n_curves, double fmax, PointRec *pts, CurveMeta *meta,
+                        int32_t *u_status, cudaStream_t st);
 cudaError_t launch_variability(const float *t, const float *mag, const float *sigma, const int64_t *d_offsets,
                                const int32_t *group, int64_t n, const bls_variability_config &cfg, int32_t *status,
                                double *mean_mag, double *rms, int32_t *cell, int32_t *count, int32_t *offset,

@@ -12,14 +12,15 @@ namespace bls {
 
 __global__ void __launch_bounds__(kPrepThreads)
 prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const float *__restrict__ sigma,
-            const int64_t *__restrict__ offsets, double fmax_grid, PointRec *__restrict__ pts,
-            CurveMeta *__restrict__ meta, int32_t *__restrict__ u_status)
+            const int64_t *__restrict__ offsets, const int64_t *__restrict__ poffsets, double fmax_grid,
+            PointRec *__restrict__ pts, CurveMeta *__restrict__ meta, int32_t *__restrict__ u_status)
 {
     __shared__ double sh[kPrepThreads / 32];
     __shared__ int s_flags;
     const int64_t c = blockIdx.x;
     const int64_t beg = offsets[c], end = offsets[c + 1];
     const int64_t n = end - beg;
+    const int64_t pbeg = poffsets[c], n_pad = poffsets[c + 1] - pbeg;      // records: n rounded up to a multiple of 4
     if (threadIdx.x == 0) s_flags = 0;
     __syncthreads();
 
@@ -47,13 +48,13 @@ prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const fl
     else if (!isfinite(sw) || !(sw > 0.0)) status = BLS_CURVE_NONFINITE;
 
     if (status != BLS_CURVE_OK) {
-        for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
+        for (int64_t i = threadIdx.x; i < n_pad; i += kPrepThreads) {
             PointRec r; r.t = 0.0; r.qw = 0u; r.qy = 0;
-            pts[i] = r;
+            pts[pbeg + i] = r;
         }
         if (threadIdx.x == 0) {
             CurveMeta m; m.ncw = 0.f; m.cy = 0.f; m.status = status; m.force_canonical = 0;
-            m.swt = 0u; m.pad_ = 0u; m.sr_scale = 0.0; m.dp_scale = 0.0; m.wx2 = 0.0;
+            m.swt = 0u; m.w0 = 0u; m.y0 = 0; m.pad_ = 0; m.sr_scale = 0.0; m.dp_scale = 0.0; m.wx2 = 0.0;
             meta[c] = m;
             if (u_status) u_status[c] = status;
         }
@@ -83,18 +84,28 @@ prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const fl
     const double SY = (sigw > 0.0 && isfinite(sigw))
                           ? (2147483648.0 - (double)n - 2.0) / (0.5 * sigw * (1.0 + 1e-12)) : 0.0;
 
-    double qsum = 0.0;                                  // integers < 2^32: exact in fp64, any order
-    for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
-        double s = (double)sigma[i];
-        double w = (1.0 / (s * s)) / sw;
-        double x = (double)mag[i] - mu;
+    // Records.  A zero-time point (t == 0, e.g. the curve's first epoch) sits exactly on a bin edge at every
+    // frequency and always belongs to bin 0: it is summed into (w0, y0) instead and its record carries no
+    // weight, so the fold's guard band is not triggered by it.  Weightless records (those and the padding to
+    // a multiple of 4) take the time of the curve's last point: they add zero to whatever bin they hit.
+    double qsum = 0.0, w0 = 0.0, y0 = 0.0;              // integers < 2^32: exact in fp64, any order
+    const double t_pad = tmax;                          // max |t|: inside the fast phase's range, not 0 unless all are
+    for (int64_t i = threadIdx.x; i < n_pad; i += kPrepThreads) {
         PointRec r;
-        r.t = (double)t[i];
-        r.qw = (uint32_t)__double2ll_rn(w * SW);
-        r.qy = (int32_t)__double2ll_rn(w * x * SY);
-        qsum += (double)r.qw;
-        pts[i] = r;
+        r.t = t_pad; r.qw = 0u; r.qy = 0;
+        if (i < n) {
+            double s = (double)sigma[beg + i];
+            double w = (1.0 / (s * s)) / sw;
+            double x = (double)mag[beg + i] - mu;
+            const uint32_t qw = (uint32_t)__double2ll_rn(w * SW);
+            const int32_t qy = (int32_t)__double2ll_rn(w * x * SY);
+            qsum += (double)qw;
+            if (t[beg + i] == 0.0f) { w0 += (double)qw; y0 += (double)qy; }
+            else { r.t = (double)t[beg + i]; r.qw = qw; r.qy = qy; }
+        }
+        pts[pbeg + i] = r;
     }
+    const double w0s = block_sum(w0, sh), y0s = block_sum(y0, sh);
     const double swt = block_sum(qsum, sh);             // SWT = sum_i qw_i <= SW + N/2 < 2^32
     if (threadIdx.x == 0) {
         CurveMeta m;
@@ -104,7 +115,7 @@ prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const fl
         // the fast phase needs |f t| < 2^18 cycles
         m.force_canonical = (fmax_grid * tmax < 262144.0) ? 0 : 1;
         m.swt = (uint32_t)swt;
-        m.pad_ = 0u;
+        m.w0 = (uint32_t)w0s; m.y0 = (int32_t)y0s; m.pad_ = 0;
         m.sr_scale = SY > 0.0 ? (swt / SY) * (swt / SY) : 0.0;
         m.dp_scale = SY > 0.0 ? swt * (swt / SY) : 0.0;
         m.wx2 = wx2;
@@ -114,11 +125,11 @@ prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const fl
 }
 
 cudaError_t launch_prep(const float *t, const float *mag, const float *sigma, const int64_t *offsets,
-                        int64_t n_curves, double fmax, PointRec *pts, CurveMeta *meta, int32_t *u_status,
-                        cudaStream_t st)
+                        const int64_t *poffsets, int64_t n_curves, double fmax, PointRec *pts, CurveMeta *meta,
+                        int32_t *u_status, cudaStream_t st)
 {
     if (n_curves <= 0) return cudaSuccess;
-    prep_kernel<<<(unsigned)n_curves, kPrepThreads, 0, st>>>(t, mag, sigma, offsets, fmax, pts, meta, u_status);
+    prep_kernel<<<(unsigned)n_curves, kPrepThreads, 0, st>>>(t, mag, sigma, offsets, poffsets, fmax, pts, meta, u_status);
     return cudaGetLastError();
 }
 
