@@ -81,8 +81,10 @@ typedef struct {
 #define BLS_FLAG_SINGLE_BUFFER 2u    /* tuning: always use the single-buffer search kernel (every warp
                                        does every phase) instead of the warp-specialised, double-
                                        buffered one.  Never changes results.                       */
-#define BLS_FLAG_NO_WARP_PER_TILE 4u /* tuning: never use the one-warp-per-tile search kernel that small
-                                       shapes get by default.  Never changes results.               */
+#define BLS_FLAG_NO_SMALL_CTAS 4u    /* tuning: never use the small-CTA launch shape (kernel 1 with CTAs of two
+                                       warps) that small shapes get by default.  Never changes results. */
+#define BLS_FLAG_WARP_PER_TILE 8u    /* tuning: use the one-warp-per-tile search kernel (kernel 3, warp-private
+                                       bins) where it fits.  Never changes results.                 */
 #define BLS_FLAG_WARPS(n) (((uint32_t)(n) & 0xffu) << 8) /* tuning: warps per CTA that walk the boxes
                                        (1..10; 0 = the library's choice).  Never changes results. */
 #define BLS_FLAG_FOLD_WARPS(n) (((uint32_t)(n) & 0xffu) << 16) /* tuning: warps per CTA that fold, in

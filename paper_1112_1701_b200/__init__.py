@@ -12,7 +12,8 @@ from .binding import (  # noqa: F401
     BLS_FLAG_CANONICAL_PHASE,
     BLS_FLAG_FOLD_WARPS,
     BLS_FLAG_NONE,
-    BLS_FLAG_NO_WARP_PER_TILE,
+    BLS_FLAG_NO_SMALL_CTAS,
+    BLS_FLAG_WARP_PER_TILE,
     BLS_FLAG_SINGLE_BUFFER,
     BLS_FLAG_WARPS,
     BlsError,

@@ -22,7 +22,7 @@ EXPORTS = ["bls_plan_create", "bls_run", "bls_topk", "bls_search_host", "bls_pla
 
 BLS_OK = 0
 BLS_ERR_NULL, BLS_ERR_CONFIG, BLS_ERR_BATCH, BLS_ERR_ARG, BLS_ERR_CUDA, BLS_ERR_UNSUPPORTED = -1, -2, -3, -4, -5, -6
-BLS_FLAG_NONE, BLS_FLAG_CANONICAL_PHASE, BLS_FLAG_SINGLE_BUFFER, BLS_FLAG_NO_WARP_PER_TILE = 0, 1, 2, 4
+BLS_FLAG_NONE, BLS_FLAG_CANONICAL_PHASE, BLS_FLAG_SINGLE_BUFFER, BLS_FLAG_NO_SMALL_CTAS, BLS_FLAG_WARP_PER_TILE = 0, 1, 2, 4, 8
 
 
 def BLS_FLAG_WARPS(n):

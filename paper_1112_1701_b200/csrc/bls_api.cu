@@ -139,20 +139,31 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     int threads = (ws ? ws_search + ws_fold : k1_warps) * 32;
     int kernel = ws ? 2 : 1;
     int nrows = search_rows_for(p->nb, p->kmax, 2 * warps);
-    // Kernel 3 (one warp per tile, warp-private bins) for small shapes: when two CTAs of kWtWarps
-    // warps, each with the curve staged, fit an SM.  There a tile is too little work to pay for the
-    // hand-offs of kernels 1 and 2 (C4: 200 epochs, 64 bins).
+    // Small shapes (C4: 200 epochs, 64 bins): a tile is too little work to pay for the hand-offs of kernel 2
+    // and one CTA of 20 warps cannot hide its phases' latencies.  When CTAs of kSmallWarps warps (bins, candidates
+    // and the staged curve) fit kSmallCtasMin times on an SM, run kernel 1 with that CTA shape: many small
+    // CTAs in different phases overlap the LSU-bound fold of one with the XU-bound search of another.
+    // (Kernel 3, one warp per tile with warp-private bins, measured slower: BLS_FLAG_WARP_PER_TILE selects it.)
+    const size_t small_smem = search_smem_bytes(p->nb, p->kmax, kSmallWarps, 1, max_n);
+    const bool small = !(p->flags & (BLS_FLAG_SINGLE_BUFFER | BLS_FLAG_NO_SMALL_CTAS)) && warps_flag == 0 &&
+                       (size_t)kSmallCtasMin * (small_smem + 1024) <= sm_smem;
+    if (small) {
+        kernel = 1; smem = small_smem; pts_in_smem = 1; threads = kSmallWarps * 32;
+        nrows = search_rows_for(p->nb, p->kmax, 2 * kSmallWarps);
+    }
     const int wt_rows = search_rows_for(p->nb, p->kmax, 2);
     const size_t wt_smem = (size_t)kWtWarps * ((size_t)wt_rows * kTileFreqs * 8 + 256) + (size_t)max_n * sizeof(PointRec);
-    const bool wt_fits = 2 * (wt_smem + 1024) <= sm_smem;
-    if (!(p->flags & (BLS_FLAG_SINGLE_BUFFER | BLS_FLAG_NO_WARP_PER_TILE)) && wt_fits) {
+    if ((p->flags & BLS_FLAG_WARP_PER_TILE) && 2 * (wt_smem + 1024) <= sm_smem) {
         kernel = 3; smem = wt_smem; pts_in_smem = 1; threads = kWtWarps * 32; nrows = wt_rows;
     }
     int ctas_per_sm = (int)(sm_smem / (smem + 1024));
     if (ctas_per_sm < 1) ctas_per_sm = 1;
-    const int max_ctas = kernel == 2 ? 1 : 2;                       // register-limited (launch bounds)
+    // register-limited residency: kernels 1 and 3 are compiled for 96 registers, kernel 2 for one CTA per SM
+    int max_ctas = kernel == 2 ? 1 : (int)(65536 / (96 * threads));
+    if (kernel == 3) max_ctas = 2;
+    if (max_ctas > 32) max_ctas = 32;
     if (ctas_per_sm > max_ctas) ctas_per_sm = max_ctas;
-    const int waves = kernel == 1 ? 12 : 24;                        // enough waves to hide the tail
+    const int waves = (kernel == 1 && !small) ? 12 : 24;            // enough waves to hide the tail
     const int64_t target_ctas = (int64_t)p->sm_count * ctas_per_sm * waves;
     int64_t items = (target_ctas + chunk - 1) / chunk;
     if (items < 1) items = 1;

@@ -46,6 +46,8 @@ constexpr int kMaxSearchWarps = 10;   // kernel 1 upper bound (BLS_FLAG_WARPS ov
 constexpr int kWsMaxWarps = 20;       // warp-specialised kernel: search warps + fold warps
 constexpr int kWsSearchWarps = 8;     // its default split: 8 search (two per SM sub-partition) + 12 fold; 20 warps = 5 per sub-partition leave 96 registers per thread
 constexpr int kMergeWarps = 8;        // warps of a group that share the exact merge of a tile (one start each, S <= 8)
+constexpr int kSmallWarps = 2;        // small shapes: kernel 1 with CTAs of this many warps ...
+constexpr int kSmallCtasMin = 8;      // ... when at least this many fit an SM
 constexpr int kWtWarps = 5;           // warp-per-tile kernel: warps per CTA (two CTAs per SM)
 constexpr int kPrepThreads = 256;
 constexpr int kPeakThreads = 256;

@@ -86,11 +86,14 @@ def test_small_configs_single_buffer_kernel(name):
 
 
 @pytest.mark.parametrize("name", ["T1", "C4"])
-def test_small_shapes_without_the_warp_per_tile_kernel(name):
-    """nb = 64 shapes default to the one-warp-per-tile kernel; the same cases through the
-    warp-specialised kernel."""
+def test_small_shapes_through_the_other_kernels(name):
+    """nb = 64 shapes default to kernel 1 with small CTAs; the same cases through the warp-specialised
+    kernel and through the one-warp-per-tile kernel."""
     import paper_1112_1701_b200 as bls
-    check_config(name, curve_ids=None if name == "T1" else list(range(8)), flags=bls.BLS_FLAG_NO_WARP_PER_TILE)
+    ids = None if name == "T1" else list(range(8))
+    check_config(name, curve_ids=ids, flags=bls.BLS_FLAG_NO_SMALL_CTAS)
+    g, _ = check_config(name, curve_ids=ids, flags=bls.BLS_FLAG_WARP_PER_TILE)
+    assert g["kernel"] == 3
 
 
 def test_kernel_variants_give_identical_results():
@@ -102,11 +105,11 @@ def test_kernel_variants_give_identical_results():
     cfg = synth.config("T1")
     batch = synth.make_batch(cfg)
     ref = run_gpu(batch, cfg["grid"], top_k=5)
-    variants = [bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_NO_WARP_PER_TILE,
-                bls.BLS_FLAG_NO_WARP_PER_TILE | bls.BLS_FLAG_WARPS(6) | bls.BLS_FLAG_FOLD_WARPS(3),
+    variants = [bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_NO_SMALL_CTAS, bls.BLS_FLAG_WARP_PER_TILE,
+                bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WARPS(6) | bls.BLS_FLAG_FOLD_WARPS(3),
                 bls.BLS_FLAG_WARPS(7) | bls.BLS_FLAG_SINGLE_BUFFER,
-                bls.BLS_FLAG_NO_WARP_PER_TILE | bls.BLS_FLAG_WARPS(10) | bls.BLS_FLAG_FOLD_WARPS(1),
-                bls.BLS_FLAG_NO_WARP_PER_TILE | bls.BLS_FLAG_WARPS(1) | bls.BLS_FLAG_FOLD_WARPS(2)]
+                bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WARPS(10) | bls.BLS_FLAG_FOLD_WARPS(1),
+                bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WARPS(1) | bls.BLS_FLAG_FOLD_WARPS(2)]
     variants += [bls.BLS_FLAG_WARPS(n) | bls.BLS_FLAG_SINGLE_BUFFER for n in (1, 2, 3)]   # fewer than 4 warps
     for flags in variants:
         g = run_gpu(batch, cfg["grid"], top_k=5, flags=flags)
@@ -118,14 +121,14 @@ def test_kernel_variants_give_identical_results():
 
 def test_kernel_selection_per_configuration_and_shape_limit():
     """Which search kernel bls_run picks by itself (BLS_QUERY_SEARCH_KERNEL): the warp-specialised one for
-    C0-C3 shapes, one warp per tile for C4, the single-buffer one where two bin buffers do not fit
+    C0-C3 shapes, kernel 1 with small CTAs for C4, kernel 1 with full CTAs where two bin buffers do not fit
     (nb = 512, q_max = 0.1) -- checked against the oracle there -- and BLS_ERR_UNSUPPORTED beyond the
     shared-memory limit bls.h states."""
     import torch
     import paper_1112_1701_b200 as bls
     from paper_1112_1701_b200 import binding as B
     dev = torch.device("cuda", 0)
-    want = {"C0": 2, "C1": 2, "C2": 2, "C3": 2, "C4": 3, "T0": 2, "T1": 3, "T2": 2}
+    want = {"C0": 2, "C1": 2, "C2": 2, "C3": 2, "C4": 1, "T0": 2, "T1": 1, "T2": 2}
     for name, kern in want.items():
         cfg = synth.config(name)
         grid = cfg["grid"]
