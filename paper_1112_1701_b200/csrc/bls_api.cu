@@ -178,6 +178,11 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     a.tiles_per_item = tiles_per_item; a.items_per_curve = (int)items;
     a.pts_in_smem = pts_in_smem;
     a.nrows = nrows;
+    // long curves (and curves read through L1) want more loads in flight per fold warp; short ones fewer,
+    // so the bursts of LDS/ATOMS do not delay the search warps (clocks per pair with 4 / 8 points in flight:
+    // C1 643 / 649, C2 759 / 730, C3 2100 / 1778; 16 in flight is slower everywhere)
+    a.fold_depth = (!pts_in_smem || max_n >= 2048) ? 2 : 1;
+    if ((p->flags >> 27) & 3) a.fold_depth = (int)((p->flags >> 27) & 3);
     a.search_warps = kernel == 2 ? ws_search : 0;
     a.kernel = kernel;
     a.threads = threads;

@@ -66,6 +66,7 @@ struct SearchArgs {
     int64_t curve_base;         // first curve of this chunk
     int threads;                // CTA size of the search kernel (multiple of 32, <= 32*kMaxSearchWarps)
     int pts_in_smem;            // 1: stage the curve in shared memory, 0: read it through L1
+    int fold_depth;             // kernel 2: groups of 4 points a fold warp keeps in flight (1 or 2)
     int nrows;                  // bin rows per buffer: nb + cyclic extension (search_rows_for)
     int search_warps;           // kernel 2: this many search warps (then the fold warps)
     int kernel;                 // 1 single buffer, 2 warp-specialised double buffer, 3 one warp per tile

@@ -260,18 +260,19 @@ __device__ __forceinline__ void fold_tile(const TileCtx &c, const LaneFreq &lf, 
     }
     uint32_t lomin = 0xffffffffu;
     int g = gw;
-    if (NG == 2) {
-        for (; g + gnw < ngroups; g += 2 * gnw) {    // 8 points in flight
-            uint4 raw[8];
-            unsigned long long pr[8];
+    if (NG > 1) {
+        constexpr int NP = 4 * NG;                   // points in flight
+        for (; g + (NG - 1) * gnw < ngroups; g += NG * gnw) {
+            uint4 raw[NP];
+            unsigned long long pr[NP];
 #pragma unroll
-            for (int u = 0; u < 8; ++u) raw[u] = point_raw<PTS_SMEM>(pts_sa, pts_g, (g + (u >> 2) * gnw) * 4 + (u & 3));
+            for (int u = 0; u < NP; ++u) raw[u] = point_raw<PTS_SMEM>(pts_sa, pts_g, (g + (u >> 2) * gnw) * 4 + (u & 3));
 #pragma unroll
-            for (int u = 0; u < 8; ++u) pr[u] = fast_bin_pos(lf.f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb, G, lf.magic);
+            for (int u = 0; u < NP; ++u) pr[u] = fast_bin_pos(lf.f, __hiloint2double((int)raw[u].y, (int)raw[u].x), nb, G, lf.magic);
 #pragma unroll
-            for (int u = 0; u < 8; u += 2) lomin = min(lomin, min((uint32_t)pr[u], (uint32_t)pr[u + 1]));
+            for (int u = 0; u < NP; u += 2) lomin = min(lomin, min((uint32_t)pr[u], (uint32_t)pr[u + 1]));
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
+            for (int u = 0; u < NP; ++u) {
                 const uint32_t addr = row_addr(colw, (uint32_t)(pr[u] >> 32));
                 red_add(addr, raw[u].z);
                 red_add(addr + 128, raw[u].w);
@@ -916,7 +917,7 @@ search_ws_kernel(const SearchArgs a)
             zero_bins(buf, c.nb, gtid, gthreads);
             named_sync(kBarFoldGroup, gthreads);
             if (!(a.debug & 2)) {
-                if (a.debug & 8) fold_tile<PTS_SMEM, 2>(c, lf, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
+                if (a.fold_depth == 2) fold_tile<PTS_SMEM, 2>(c, lf, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
                 else fold_tile<PTS_SMEM, 1>(c, lf, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
             }
             named_sync(kBarFoldGroup, gthreads);
