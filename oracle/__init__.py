@@ -60,6 +60,9 @@ def lib():
         L.oracle_peaks.argtypes = [C.c_int64, _f64p, C.c_int, _i64p]
         L.oracle_bins_many.restype = None
         L.oracle_bins_many.argtypes = [C.c_int64, _f64p, _f64p, C.c_int, _i32p]
+        L.oracle_detection_efficiency.restype = None
+        L.oracle_detection_efficiency.argtypes = [C.c_int64, _f32p, C.c_int64, _f64p, C.c_double, C.c_int, C.c_int,
+                                                  _i32p, _f64p]
         L.oracle_sde.restype = C.c_double
         L.oracle_sde.argtypes = [C.c_int64, _f64p, C.c_int64]
         L.oracle_bin_shift.restype = C.c_int
@@ -162,6 +165,15 @@ def refine_pick(sr) -> int:
 def refine_bounds(freqs, q: int):
     """S2: the fine grid of coarse peak q spans its two neighbours on the coarse grid."""
     return float(freqs[max(q - 1, 0)]), float(freqs[min(q + 1, len(freqs) - 1)])
+
+
+def detection_efficiency(t, freqs, duration: float, n_phase: int, min_events: int = 2):
+    """f4 (W1-W4): (count[nf] int32, efficiency[nf] f64) of one cadence t (sorted ascending)."""
+    t = _c32(t)
+    freqs = np.ascontiguousarray(freqs, dtype=np.float64)
+    cnt = np.zeros(freqs.size, dtype=np.int32); eff = np.zeros(freqs.size)
+    lib().oracle_detection_efficiency(t.size, t, freqs.size, freqs, float(duration), int(n_phase), int(min_events), cnt, eff)
+    return cnt, eff
 
 
 def host_cores() -> int:

@@ -30,6 +30,8 @@
  *   oracle_peaks        - hand-written spectra with answers written out               (pinned)
  *   oracle_sde          - hand-written spectra, closed form                           (pinned)
  *   oracle_bin_shift    - exact rational arithmetic with a bin-grid shift              (pinned)
+ *   oracle_detection_efficiency - closed forms on regular cadences (d/P, 2d/P), degenerate cases,
+ *                         an event-centred brute force, the integer-day dips of Fig. 13   (pinned)
  *   oracle_refine       - noiseless box between coarse grid points recovered to the fine
  *                         step and to the quarter-bin shift (closed-form SR and depth),
  *                         brute force over boxes with shifted member sets             (pinned)
@@ -300,4 +302,43 @@ int64_t oracle_refine_pick(int64_t m, const double *sr)
     for (int64_t q = 0; q < m; ++q)
         if (sr[q] > bv) { bv = sr[q]; best = q; }
     return best;
+}
+
+/* ---- f4: eclipse detection efficiency of a cadence (Fig. 13) ----
+ * "The detection efficiency is the probability that at least two eclipses will be observed from an
+ * eclipsing target with a specified period, after observing window and weather effects have been taken into
+ * account" -- "based on simulations including the actual observing cadences of the survey".  Readings:
+ *   W1  the cadence is the list of epochs t_i of one light curve, sorted ascending (window and weather are
+ *       whatever made that list);
+ *   W2  a target of frequency f (period 1/f) and eclipse duration d days has mid-eclipse phase phi, uniform in
+ *       [0, 1); the simulation takes the n_phase phases phi_k = (k + 1/2)/n_phase (a stratified grid: no
+ *       random numbers, so both implementations see the same targets);
+ *   W3  epoch t_i is in eclipse iff |x - rint(x)| <= h, x = RN(RN(f t_i) - phi_k), h = RN(RN(0.5 d) f)
+ *       (rint = round half to even); the eclipse it belongs to is cycle m = rint(x);
+ *   W4  an eclipse is "observed" if at least one epoch is inside it; the target is detected iff at least
+ *       min_events DISTINCT cycles are observed (the paper: two); efficiency = detected phases / n_phase.
+ * count[q] receives the number of detected phases at freqs[q], eff[q] = count / n_phase. */
+void oracle_detection_efficiency(int64_t n, const float *t, int64_t nf, const double *freqs, double duration,
+                                 int n_phase, int min_events, int32_t *count, double *eff)
+{
+    for (int64_t q = 0; q < nf; ++q) {
+        const double f = freqs[q];
+        volatile double hd = 0.5 * duration;
+        volatile double h = hd * f;
+        int32_t det = 0;
+        for (int k = 0; k < n_phase; ++k) {
+            const double phi = ((double)k + 0.5) / (double)n_phase;
+            int events = 0;
+            double last = 0.0;
+            for (int64_t i = 0; i < n; ++i) {
+                volatile double u = f * (double)t[i];
+                volatile double x = u - phi;
+                double m = rint(x);
+                if (fabs(x - m) <= h && (events == 0 || m != last)) { ++events; last = m; }
+            }
+            if (events >= min_events) ++det;
+        }
+        count[q] = det;
+        eff[q] = (double)det / (double)n_phase;
+    }
 }
