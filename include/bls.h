@@ -245,6 +245,22 @@ typedef struct {
 int bls_variability(int32_t device, const bls_variability_config *cfg, const bls_batch *batch,
                     const int32_t *group, const bls_variability_outputs *out, void *cuda_stream);
 
+/* ---- f4: eclipse detection efficiency of a cadence (Fig. 13; used at L426) ----------
+ * "The detection efficiency is the probability that at least two eclipses will be observed from an eclipsing
+ * target with a specified period, after observing window and weather effects have been taken into account."
+ * Readings W1-W4: the cadence is the epoch list t of each curve of `batch` (only
+ * offsets and t are read; t sorted ascending); for each of the n_freq target frequencies (HOST, cycles/day)
+ * and each of the n_phase mid-eclipse phases (k + 1/2)/n_phase an epoch is in eclipse iff
+ * |x - rint(x)| <= h, x = RN(RN(f t) - phase), h = RN(RN(duration/2) f); the target is detected iff at least
+ * min_events distinct eclipses (cycles rint(x)) are observed.
+ *   count      DEVICE int32 [n_curves*n_freq] detected phases, or NULL
+ *   efficiency DEVICE double [n_curves*n_freq] = count / n_phase, or NULL
+ * duration in days (> 0); 1 <= n_phase <= 2^20; min_events >= 1; n_curves <= 65535.  Needs no plan;
+ * scratch is stream-ordered.  Enqueues on cuda_stream. */
+int bls_detection_efficiency(int32_t device, const bls_batch *batch, int64_t n_freq, const double *freqs,
+                             double duration, int32_t n_phase, int32_t min_events, int32_t *count,
+                             double *efficiency, void *cuda_stream);
+
 /* NULL is a no-op. */
 int bls_plan_destroy(bls_plan *plan);
 

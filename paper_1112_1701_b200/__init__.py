@@ -23,6 +23,7 @@ from .binding import (  # noqa: F401
     REFINED_DTYPE,
     Plan,
     debug_fold_bins,
+    detection_efficiency,
     lib,
     variability,
 )

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libbls_b200.so")
 
 EXPORTS = ["bls_plan_create", "bls_run", "bls_topk", "bls_search_host", "bls_plan_destroy",
            "bls_plan_query", "bls_strerror", "bls_plan_last_cuda_error", "bls_debug_fold_bins",
-           "bls_variability", "bls_refine"]
+           "bls_variability", "bls_refine", "bls_detection_efficiency"]
 
 BLS_OK = 0
 BLS_ERR_NULL, BLS_ERR_CONFIG, BLS_ERR_BATCH, BLS_ERR_ARG, BLS_ERR_CUDA, BLS_ERR_UNSUPPORTED = -1, -2, -3, -4, -5, -6
@@ -114,11 +114,35 @@ def lib():
                                           C.c_uint32, C.c_void_p, C.POINTER(C.c_int64)]
         L.bls_refine.restype = C.c_int
         L.bls_refine.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
+        L.bls_detection_efficiency.restype = C.c_int
+        L.bls_detection_efficiency.argtypes = [C.c_int32, C.POINTER(BlsBatch), C.c_int64, C.c_void_p, C.c_double, C.c_int32,
+                                               C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
         L.bls_variability.restype = C.c_int
         L.bls_variability.argtypes = [C.c_int32, C.POINTER(BlsVariabilityConfig), C.POINTER(BlsBatch), C.c_void_p,
                                       C.POINTER(BlsVariabilityOutputs), C.c_void_p]
         _lib = L
     return _lib
+
+
+def detection_efficiency(offsets, t, freqs, duration: float, n_phase: int = 1000, min_events: int = 2, device: int = 0,
+                         stream: Optional[int] = None):
+    """bls_detection_efficiency: offsets host int64, t float32 CUDA tensor (each cadence sorted), freqs host float64.
+    Returns (count int32 [n_curves, n_freq], efficiency float64 [n_curves, n_freq]) CUDA tensors."""
+    import torch
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    freqs = np.ascontiguousarray(freqs, dtype=np.float64)
+    n = offsets.size - 1
+    dev = torch.device("cuda", device)
+    cnt = torch.zeros((max(n, 1), freqs.size), dtype=torch.int32, device=dev)
+    eff = torch.zeros((max(n, 1), freqs.size), dtype=torch.float64, device=dev)
+    b = BlsBatch(n, offsets.ctypes.data, _ptr(t), None, None, None)
+    if stream is None:
+        stream = torch.cuda.current_stream(dev).cuda_stream
+    rc = lib().bls_detection_efficiency(device, C.byref(b), freqs.size, C.c_void_p(freqs.ctypes.data), float(duration), int(n_phase),
+                                        int(min_events), C.c_void_p(cnt.data_ptr()), C.c_void_p(eff.data_ptr()), C.c_void_p(stream))
+    if rc != BLS_OK:
+        raise BlsError(rc)
+    return cnt[:n], eff[:n]
 
 
 def variability(offsets, t, mag, sigma, group=None, *, n_groups: int = 1, mag_lo: float = 12.0, mag_bin: float = 0.1,

@@ -532,6 +532,40 @@ int bls_variability(int32_t device, const bls_variability_config *cfg, const bls
     return BLS_OK;
 }
 
+int bls_detection_efficiency(int32_t device, const bls_batch *b, int64_t n_freq, const double *freqs, double duration,
+                             int32_t n_phase, int32_t min_events, int32_t *count, double *efficiency, void *cuda_stream)
+{
+    if (!b || !freqs) return BLS_ERR_NULL;
+    if (b->n_curves < 0 || b->n_curves > 65535) return BLS_ERR_BATCH;
+    if (!b->offsets) return BLS_ERR_NULL;
+    if (n_freq < 1 || n_freq > 2147483647LL || !(duration > 0.0) || !isfinite(duration)) return BLS_ERR_ARG;
+    if (n_phase < 1 || n_phase > (1 << 20) || min_events < 1) return BLS_ERR_ARG;
+    const int64_t nc = b->n_curves;
+    if (b->offsets[0] != 0) return BLS_ERR_BATCH;
+    for (int64_t c = 0; c < nc; ++c)
+        if (b->offsets[c + 1] < b->offsets[c]) return BLS_ERR_BATCH;
+    for (int64_t q = 0; q < n_freq; ++q)
+        if (!isfinite(freqs[q]) || !(freqs[q] > 0.0)) return BLS_ERR_ARG;
+    if (b->offsets[nc] > 0 && !b->t) return BLS_ERR_NULL;
+    if (nc == 0) return BLS_OK;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    size_t off = 0;
+    auto take = [&off](size_t bytes) { const size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+    const size_t o_off = take((size_t)(nc + 1) * 8), o_f = take((size_t)n_freq * 8);
+    const size_t o_cnt = take((size_t)(nc * n_freq) * 4), o_eff = take((size_t)(nc * n_freq) * 8);
+    unsigned char *scr = nullptr;
+    if (cudaMallocAsync((void **)&scr, off, st) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    cudaError_t e = cudaMemcpyAsync(scr + o_off, b->offsets, (size_t)(nc + 1) * 8, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(scr + o_f, freqs, (size_t)n_freq * 8, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess)
+        e = launch_window(b->t, (const int64_t *)(scr + o_off), nc, (int)n_freq, (const double *)(scr + o_f), duration, n_phase,
+                          min_events, count ? count : (int32_t *)(scr + o_cnt), efficiency ? efficiency : (double *)(scr + o_eff), st);
+    const cudaError_t e2 = cudaFreeAsync(scr, st);
+    if (e != cudaSuccess || e2 != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    return BLS_OK;
+}
+
 int bls_topk(bls_plan *p, int32_t k, bls_peak *peaks, void *cuda_stream)
 {
     if (!p || !peaks) return BLS_ERR_NULL;

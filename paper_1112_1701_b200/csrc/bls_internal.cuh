@@ -169,6 +169,8 @@ cudaError_t launch_variability(const float *t, const float *mag, const float *si
                                double *mean_mag, double *rms, int32_t *cell, int32_t *count, int32_t *offset,
                                int32_t *cursor, int32_t *members, unsigned char *keep, double *expected,
                                double *scatter, int32_t *kept, int32_t *flag, cudaStream_t st);
+cudaError_t launch_window(const float *t, const int64_t *d_offsets, int64_t n_curves, int nf, const double *d_freqs,
+                          double duration, int n_phase, int min_events, int32_t *count, double *eff, cudaStream_t st);
 cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem, cudaStream_t st);
 cudaError_t launch_peaks(const float *sr, const uint32_t *ak, const float *depth, const CurveMeta *meta,
                          int64_t curve_base, int64_t chunk_curves, int nf, int max_k, PeakCand *cand,
