@@ -153,6 +153,28 @@ int bls_plan_create(const bls_config *cfg, bls_plan **out_plan);
  * bls_topk.  `out` may be NULL (peaks only).  Enqueues on cuda_stream. */
 int bls_run(bls_plan *plan, const bls_batch *batch, const bls_outputs *out, void *cuda_stream);
 
+/* ---- f2: field-shared cadence ------------------------------------------
+ * All stars of a pointing are measured on the same exposures ("about 3,000 M-dwarfs in each
+ * pointing"; L115: per-epoch zeropoints, 0-2 % of the epochs rejected per field, quality flags per star), so a
+ * field is one epoch list and a dense [stars][epochs] matrix of magnitudes and errors.  An entry whose mag or
+ * sigma is not finite, or whose sigma <= 0, is an epoch ABSENT for that star (flagged measurement): it simply
+ * does not take part; it is not a data fault.  The result for each star is by definition that of bls_run on the
+ * star's present epochs.  DESIGN.md section 6.5 says why the bin indices are NOT shared between stars on this
+ * hardware (a table lookup costs more shared-memory issue slots than recomputing the phase). */
+typedef struct {
+    int64_t n_stars;
+    int64_t n_epochs;        /* >= 1                                                                  */
+    const float *t;          /* DEVICE [n_epochs] days relative to the field's origin, shared by every star */
+    const float *mag;        /* DEVICE [n_stars][n_epochs] row-major                                  */
+    const float *sigma;      /* DEVICE [n_stars][n_epochs]                                            */
+    const double *t_origin;  /* HOST, ONE value (HJD of t = 0) or NULL                                */
+} bls_field_batch;
+
+/* bls_run for a field: same outputs, same bls_topk / bls_refine afterwards (curve index = star index).
+ * A star with fewer than 2 present epochs gets status BLS_CURVE_TOO_FEW; a non-finite epoch time makes every
+ * star BLS_CURVE_NONFINITE. */
+int bls_run_field(bls_plan *plan, const bls_field_batch *field, const bls_outputs *out, void *cuda_stream);
+
 /* Write the k best peaks of every curve of the last bls_run to peaks (DEVICE, [n_curves*k]).
  * 1 <= k <= max_top_k.  Enqueues on cuda_stream (must be the stream of that bls_run, or one
  * ordered after it). */

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libbls_b200.so")
 
 EXPORTS = ["bls_plan_create", "bls_run", "bls_topk", "bls_search_host", "bls_plan_destroy",
            "bls_plan_query", "bls_strerror", "bls_plan_last_cuda_error", "bls_debug_fold_bins",
-           "bls_variability", "bls_refine", "bls_detection_efficiency"]
+           "bls_variability", "bls_refine", "bls_detection_efficiency", "bls_run_field"]
 
 BLS_OK = 0
 BLS_ERR_NULL, BLS_ERR_CONFIG, BLS_ERR_BATCH, BLS_ERR_ARG, BLS_ERR_CUDA, BLS_ERR_UNSUPPORTED = -1, -2, -3, -4, -5, -6
@@ -46,6 +46,11 @@ class BlsConfig(C.Structure):
 class BlsBatch(C.Structure):
     _fields_ = [("n_curves", C.c_int64), ("offsets", C.c_void_p), ("t", C.c_void_p),
                 ("mag", C.c_void_p), ("sigma", C.c_void_p), ("t_origin", C.c_void_p)]
+
+
+class BlsFieldBatch(C.Structure):
+    _fields_ = [("n_stars", C.c_int64), ("n_epochs", C.c_int64), ("t", C.c_void_p), ("mag", C.c_void_p),
+                ("sigma", C.c_void_p), ("t_origin", C.c_void_p)]
 
 
 class BlsOutputs(C.Structure):
@@ -97,6 +102,8 @@ def lib():
         L.bls_plan_create.argtypes = [C.POINTER(BlsConfig), C.POINTER(C.c_void_p)]
         L.bls_run.restype = C.c_int
         L.bls_run.argtypes = [C.c_void_p, C.POINTER(BlsBatch), C.POINTER(BlsOutputs), C.c_void_p]
+        L.bls_run_field.restype = C.c_int
+        L.bls_run_field.argtypes = [C.c_void_p, C.POINTER(BlsFieldBatch), C.POINTER(BlsOutputs), C.c_void_p]
         L.bls_topk.restype = C.c_int
         L.bls_topk.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p]
         L.bls_search_host.restype = C.c_int
@@ -286,6 +293,27 @@ class Plan:
                            C.c_void_p(stream))
         self._check(rc)
         self._n_curves = n_curves
+
+    # -- bls_run_field ----------------------------------------------------------------------------
+    def run_field(self, t, mag, sigma, t_origin: Optional[float] = None, *, sr=None, best_start=None, best_width=None,
+                  depth=None, status=None, stream: Optional[int] = None):
+        """t: float32 CUDA [n_epochs]; mag, sigma: float32 CUDA [n_stars, n_epochs] (non-finite / sigma <= 0 = absent)."""
+        import torch
+        assert mag.dim() == 2 and mag.shape == sigma.shape and mag.shape[1] == t.numel()
+        for name, x in (("t", t), ("mag", mag), ("sigma", sigma)):
+            if not (x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()):
+                raise TypeError("%s must be a contiguous float32 CUDA tensor" % name)
+        origin = None if t_origin is None else np.array([float(t_origin)], dtype=np.float64)
+        fb = BlsFieldBatch(mag.shape[0], mag.shape[1], _ptr(t), _ptr(mag), _ptr(sigma),
+                           None if origin is None else origin.ctypes.data)
+        outs = None
+        if any(x is not None for x in (sr, best_start, best_width, depth, status)):
+            outs = BlsOutputs(_ptr(sr), _ptr(best_start), _ptr(best_width), _ptr(depth), _ptr(status))
+        if stream is None:
+            stream = torch.cuda.current_stream(t.device).cuda_stream
+        self._keep = (origin, t, mag, sigma)
+        self._check(lib().bls_run_field(self._h, C.byref(fb), C.byref(outs) if outs is not None else None, C.c_void_p(stream)))
+        self._n_curves = int(mag.shape[0])
 
     # -- bls_topk ---------------------------------------------------------------------------------
     def topk(self, k: int, stream: Optional[int] = None):

@@ -358,13 +358,18 @@ int bls_plan_query(const bls_plan *p, int32_t what, int64_t *value)
     return BLS_OK;
 }
 
-int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_stream)
+#pragma GCC visibility pop
+}  // extern "C"
+
+namespace {
+
+// bls_run and bls_run_field.  field_epochs == 0: CSR batch `b`.  field_epochs > 0: b->offsets is NULL, every one
+// of the b->n_curves stars has field_epochs entries (b->t shared, b->mag / b->sigma row-major) and b->t_origin
+// points to ONE value.
+int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_outputs *out, void *cuda_stream)
 {
-    if (!p || !b) return BLS_ERR_NULL;
-    if (b->n_curves < 0) return BLS_ERR_BATCH;
-    if (!b->offsets) return BLS_ERR_NULL;
+    const bool field = field_epochs > 0;
     const int64_t nc = b->n_curves;
-    if (b->offsets[0] != 0) return BLS_ERR_BATCH;
     if (nc + 1 > p->cap_hpoff) {
         free(p->h_poffsets);
         p->h_poffsets = (int64_t *)malloc((size_t)(nc + 1) * sizeof(int64_t));
@@ -373,7 +378,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     }
     int64_t max_n = 0, nrec = 0;
     for (int64_t c = 0; c < nc; ++c) {
-        const int64_t n = b->offsets[c + 1] - b->offsets[c];
+        const int64_t n = field ? field_epochs : b->offsets[c + 1] - b->offsets[c];
         if (n < 0 || n > 2147483647LL / 64) return BLS_ERR_BATCH;
         if (n > max_n) max_n = n;
         p->h_poffsets[c] = nrec;
@@ -381,7 +386,7 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     }
     p->h_poffsets[nc] = nrec;
     max_n = (max_n + 3) & ~(int64_t)3;                      // records per curve, padded
-    const int64_t npts = b->offsets[nc];
+    const int64_t npts = field ? nc * field_epochs : b->offsets[nc];
     if (npts > 0 && (!b->t || !b->mag || !b->sigma)) return BLS_ERR_NULL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     BLS_CUDA(p, cudaSetDevice(p->device));
@@ -418,19 +423,25 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     if ((rc = grow_spectrum_scratch(p, chunk * p->nf, st)) != BLS_OK) return rc;
 
     // ---- metadata to the device (stream ordered; the caller keeps offsets alive until then) ------
-    BLS_CUDA(p, cudaMemcpyAsync(p->d_offsets, b->offsets, (size_t)(nc + 1) * sizeof(int64_t),
-                                cudaMemcpyHostToDevice, st));
+    if (!field)
+        BLS_CUDA(p, cudaMemcpyAsync(p->d_offsets, b->offsets, (size_t)(nc + 1) * sizeof(int64_t),
+                                    cudaMemcpyHostToDevice, st));
     BLS_CUDA(p, cudaMemcpyAsync(p->d_poffsets, p->h_poffsets, (size_t)(nc + 1) * sizeof(int64_t),
                                 cudaMemcpyHostToDevice, st));
     p->last_has_origin = b->t_origin != nullptr;
-    if (b->t_origin)
+    if (b->t_origin && !field)
         BLS_CUDA(p, cudaMemcpyAsync(p->d_origin, b->t_origin, (size_t)nc * sizeof(double),
                                     cudaMemcpyHostToDevice, st));
+    if (b->t_origin && field) {                 // one origin for the whole field: replicated through the staging buffer
+        for (int64_t c = 0; c < nc; ++c) memcpy(&p->h_poffsets[c], b->t_origin, sizeof(double));
+        BLS_CUDA(p, cudaMemcpyAsync(p->d_origin, p->h_poffsets, (size_t)nc * sizeof(double), cudaMemcpyHostToDevice, st));
+        BLS_CUDA(p, cudaStreamSynchronize(st));  // the staging buffer is reused by the next run
+    }
     BLS_CUDA(p, cudaMemsetAsync(p->d_canon, 0, sizeof(unsigned long long), st));
 
     // ---- a0 prep -------------------------------------------------------------------------------
-    BLS_CUDA(p, launch_prep(b->t, b->mag, b->sigma, p->d_offsets, p->d_poffsets, nc, p->fmax, p->d_pts, p->d_meta,
-                            out ? out->status : nullptr, st));
+    BLS_CUDA(p, launch_prep(b->t, b->mag, b->sigma, p->d_offsets, p->d_poffsets, nc, field_epochs, p->fmax, p->d_pts,
+                            p->d_meta, out ? out->status : nullptr, st));
     p->last_launches += 1;
 
     // ---- launch geometry of the search ---------------------------------------------------------
@@ -467,6 +478,29 @@ int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_
     }
     p->last_n_curves = nc;
     return BLS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+#pragma GCC visibility push(default)
+
+int bls_run(bls_plan *p, const bls_batch *b, const bls_outputs *out, void *cuda_stream)
+{
+    if (!p || !b) return BLS_ERR_NULL;
+    if (b->n_curves < 0) return BLS_ERR_BATCH;
+    if (!b->offsets) return BLS_ERR_NULL;
+    if (b->offsets[0] != 0) return BLS_ERR_BATCH;
+    return run_impl(p, b, 0, out, cuda_stream);
+}
+
+int bls_run_field(bls_plan *p, const bls_field_batch *fb, const bls_outputs *out, void *cuda_stream)
+{
+    if (!p || !fb) return BLS_ERR_NULL;
+    if (fb->n_stars < 0 || fb->n_epochs < 1) return BLS_ERR_BATCH;
+    bls_batch b;
+    b.n_curves = fb->n_stars; b.offsets = nullptr; b.t = fb->t; b.mag = fb->mag; b.sigma = fb->sigma; b.t_origin = fb->t_origin;
+    return run_impl(p, &b, fb->n_epochs, out, cuda_stream);
 }
 
 int bls_debug_fold_bins(int32_t device, const double *f, const double *t, int64_t n, int32_t n_bins,

@@ -162,8 +162,8 @@ cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int n
                               int32_t *bins, unsigned long long *n_canon, int sm_count, cudaStream_t st);
 cudaError_t search_configure(int max_smem_optin);
 cudaError_t launch_prep(const float *t, const float *mag, const float *sigma, const int64_t *offsets,
-                        const int64_t *poffsets, int64_t n_curves, double fmax, PointRec *pts, CurveMeta *meta,
-                        int32_t *u_status, cudaStream_t st);
+                        const int64_t *poffsets, int64_t n_curves, int64_t field_epochs, double fmax, PointRec *pts,
+                        CurveMeta *meta, int32_t *u_status, cudaStream_t st);
 cudaError_t launch_variability(const float *t, const float *mag, const float *sigma, const int64_t *d_offsets,
                                const int32_t *group, int64_t n, const bls_variability_config &cfg, int32_t *status,
                                double *mean_mag, double *rms, int32_t *cell, int32_t *count, int32_t *offset,

@@ -10,42 +10,59 @@
 
 namespace bls {
 
+// FIELD = false: CSR batch, curve c owns points [offsets[c], offsets[c+1]) of t / mag / sigma.
+// FIELD = true (f2, field-shared cadence): every star shares the epoch list t[0..n_epochs) and owns row c of
+// mag / sigma [n_curves][n_epochs]; an entry whose mag or sigma is not finite or whose sigma <= 0 is an ABSENT
+// epoch of that star (a flagged measurement), not a data fault: it gets a weightless record.
+template <bool FIELD>
 __global__ void __launch_bounds__(kPrepThreads)
 prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const float *__restrict__ sigma,
-            const int64_t *__restrict__ offsets, const int64_t *__restrict__ poffsets, double fmax_grid,
+            const int64_t *__restrict__ offsets, const int64_t *__restrict__ poffsets, int64_t n_epochs, double fmax_grid,
             PointRec *__restrict__ pts, CurveMeta *__restrict__ meta, int32_t *__restrict__ u_status)
 {
     __shared__ double sh[kPrepThreads / 32];
     __shared__ int s_flags;
     const int64_t c = blockIdx.x;
-    const int64_t beg = offsets[c], end = offsets[c + 1];
-    const int64_t n = end - beg;
-    const int64_t pbeg = poffsets[c], n_pad = poffsets[c + 1] - pbeg;      // records: n rounded up to a multiple of 4
+    const int64_t beg = FIELD ? c * n_epochs : offsets[c];
+    const int64_t n = FIELD ? n_epochs : offsets[c + 1] - beg;
+    const int64_t tbeg = FIELD ? 0 : beg;
+    const int64_t pbeg = FIELD ? c * ((n_epochs + 3) & ~(int64_t)3) : poffsets[c];
+    const int64_t n_pad = (n + 3) & ~(int64_t)3;                            // records: n rounded up to a multiple of 4
+    auto present = [&](int64_t i) {
+        if (!FIELD) return true;
+        const float mi = mag[beg + i], si = sigma[beg + i];
+        return isfinite(mi) && isfinite(si) && si > 0.0f;
+    };
     if (threadIdx.x == 0) s_flags = 0;
     __syncthreads();
 
-    // pass 1: validity, sum of inverse variances, max |t|
-    double acc = 0.0, tmax = 0.0;
+    // pass 1: validity, sum of inverse variances, max |t|, number of present points
+    double acc = 0.0, tmax = 0.0, cnt = 0.0;
     int flags = 0;
-    for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
-        float ti = t[i], mi = mag[i], si = sigma[i];
-        if (!isfinite(ti) || !isfinite(mi) || !isfinite(si)) flags |= 1;
+    for (int64_t i = threadIdx.x; i < n; i += kPrepThreads) {
+        const float ti = t[tbeg + i], mi = mag[beg + i], si = sigma[beg + i];
+        if (!isfinite(ti)) flags |= 1;
+        else if (FIELD && !present(i)) continue;
+        else if (!isfinite(mi) || !isfinite(si)) flags |= 1;
         else if (!(si > 0.0f)) flags |= 2;
         else {
             double s = (double)si;
             acc += 1.0 / (s * s);
             tmax = fmax(tmax, fabs((double)ti));
+            cnt += 1.0;
         }
     }
     if (flags) atomicOr(&s_flags, flags);
     double sw = block_sum(acc, sh);
     tmax = block_max_d(tmax, sh);
+    const double n_present = block_sum(cnt, sh);
     __syncthreads();
     int status = BLS_CURVE_OK;
-    if (n < 2) status = BLS_CURVE_TOO_FEW;
-    else if (s_flags & 1) status = BLS_CURVE_NONFINITE;
+    if (s_flags & 1) status = BLS_CURVE_NONFINITE;
     else if (s_flags & 2) status = BLS_CURVE_BAD_SIGMA;
+    else if (n_present < 2.0) status = BLS_CURVE_TOO_FEW;
     else if (!isfinite(sw) || !(sw > 0.0)) status = BLS_CURVE_NONFINITE;
+    if (!FIELD && n < 2) status = BLS_CURVE_TOO_FEW;
 
     if (status != BLS_CURVE_OK) {
         for (int64_t i = threadIdx.x; i < n_pad; i += kPrepThreads) {
@@ -63,45 +80,47 @@ prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const fl
 
     // pass 2: weighted mean
     acc = 0.0;
-    for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
-        double s = (double)sigma[i];
-        acc += ((1.0 / (s * s)) / sw) * (double)mag[i];
+    for (int64_t i = threadIdx.x; i < n; i += kPrepThreads) {
+        if (!present(i)) continue;
+        double s = (double)sigma[beg + i];
+        acc += ((1.0 / (s * s)) / sw) * (double)mag[beg + i];
     }
     const double mu = block_sum(acc, sh);
 
     // pass 3: weighted variance (bounds every box sum, sets the fixed-point scale of qy)
     acc = 0.0;
-    for (int64_t i = beg + threadIdx.x; i < end; i += kPrepThreads) {
-        double s = (double)sigma[i];
+    for (int64_t i = threadIdx.x; i < n; i += kPrepThreads) {
+        if (!present(i)) continue;
+        double s = (double)sigma[beg + i];
         double w = (1.0 / (s * s)) / sw;
-        double x = (double)mag[i] - mu;
+        double x = (double)mag[beg + i] - mu;
         acc += w * x * x;
     }
     const double wx2 = block_sum(acc, sh);
 
-    const double SW = 4294967296.0 - 2.0 * (double)n - 2.0;
+    const double SW = 4294967296.0 - 2.0 * n_present - 2.0;
     const double sigw = sqrt(wx2);
     const double SY = (sigw > 0.0 && isfinite(sigw))
-                          ? (2147483648.0 - (double)n - 2.0) / (0.5 * sigw * (1.0 + 1e-12)) : 0.0;
+                          ? (2147483648.0 - n_present - 2.0) / (0.5 * sigw * (1.0 + 1e-12)) : 0.0;
 
     // Records.  A zero-time point (t == 0, e.g. the curve's first epoch) sits exactly on a bin edge at every
     // frequency and always belongs to bin 0: it is summed into (w0, y0) instead and its record carries no
-    // weight, so the fold's guard band is not triggered by it.  Weightless records (those and the padding to
-    // a multiple of 4) take the time of the curve's last point: they add zero to whatever bin they hit.
+    // weight, so the fold's guard band is not triggered by it.  Weightless records (those, absent epochs of a
+    // field and the padding to a multiple of 4) take the time max|t|: they add zero to whatever bin they hit.
     double qsum = 0.0, w0 = 0.0, y0 = 0.0;              // integers < 2^32: exact in fp64, any order
-    const double t_pad = tmax;                          // max |t|: inside the fast phase's range, not 0 unless all are
+    const double t_pad = tmax;                          // inside the fast phase's range, not 0 unless all are
     for (int64_t i = threadIdx.x; i < n_pad; i += kPrepThreads) {
         PointRec r;
         r.t = t_pad; r.qw = 0u; r.qy = 0;
-        if (i < n) {
+        if (i < n && present(i)) {
             double s = (double)sigma[beg + i];
             double w = (1.0 / (s * s)) / sw;
             double x = (double)mag[beg + i] - mu;
             const uint32_t qw = (uint32_t)__double2ll_rn(w * SW);
             const int32_t qy = (int32_t)__double2ll_rn(w * x * SY);
             qsum += (double)qw;
-            if (t[beg + i] == 0.0f) { w0 += (double)qw; y0 += (double)qy; }
-            else { r.t = (double)t[beg + i]; r.qw = qw; r.qy = qy; }
+            if (t[tbeg + i] == 0.0f) { w0 += (double)qw; y0 += (double)qy; }
+            else { r.t = (double)t[tbeg + i]; r.qw = qw; r.qy = qy; }
         }
         pts[pbeg + i] = r;
     }
@@ -125,11 +144,16 @@ prep_kernel(const float *__restrict__ t, const float *__restrict__ mag, const fl
 }
 
 cudaError_t launch_prep(const float *t, const float *mag, const float *sigma, const int64_t *offsets,
-                        const int64_t *poffsets, int64_t n_curves, double fmax, PointRec *pts, CurveMeta *meta,
-                        int32_t *u_status, cudaStream_t st)
+                        const int64_t *poffsets, int64_t n_curves, int64_t field_epochs, double fmax, PointRec *pts,
+                        CurveMeta *meta, int32_t *u_status, cudaStream_t st)
 {
     if (n_curves <= 0) return cudaSuccess;
-    prep_kernel<<<(unsigned)n_curves, kPrepThreads, 0, st>>>(t, mag, sigma, offsets, poffsets, fmax, pts, meta, u_status);
+    if (field_epochs > 0)
+        prep_kernel<true><<<(unsigned)n_curves, kPrepThreads, 0, st>>>(t, mag, sigma, offsets, poffsets, field_epochs, fmax, pts,
+                                                                      meta, u_status);
+    else
+        prep_kernel<false><<<(unsigned)n_curves, kPrepThreads, 0, st>>>(t, mag, sigma, offsets, poffsets, 0, fmax, pts, meta,
+                                                                       u_status);
     return cudaGetLastError();
 }
 
