@@ -63,10 +63,12 @@ typedef struct bls_plan bls_plan; /* opaque */
 typedef struct {
     int32_t struct_size;   /* = sizeof(bls_config)                                                  */
     int32_t device;        /* CUDA device ordinal                                                   */
-    int64_t n_freq;        /* nf >= 1                                                               */
+    int64_t n_freq;        /* 1 <= nf <= 2^27                                                       */
     const double *freqs;   /* HOST, nf trial frequencies in cycles/day, finite, > 0; NULL = uniform */
     double f0, df;         /* used iff freqs == NULL: f_k = f0 + k*df evaluated in fp64 (R13)       */
-    int32_t n_bins;        /* nb, 4 <= nb <= 2048                                                   */
+    int32_t n_bins;        /* nb >= 4; one bin buffer, (nb + kmax + 7) rows of 256 B plus 5 KB, must fit the
+                              227 KB of shared memory a CTA can have: nb + kmax <= 880 (nb <= 800 at
+                              q_max = 0.1), else bls_plan_create returns BLS_ERR_UNSUPPORTED              */
     double q_min, q_max;   /* 0 < q_min <= q_max <= 0.5; widths kmin..kmax bins by reading R9:
                               kmin = max(1, floor(q_min*nb + 1e-9)), kmax = min(nb-1, ceil(q_max*nb - 1e-9)) */
     int32_t max_top_k;     /* 1..32: upper bound for bls_topk's k                                   */
@@ -79,17 +81,22 @@ typedef struct {
                                        (R8) instead of the guarded fast path; results identical   */
 
 #define BLS_FLAG_SINGLE_BUFFER 2u    /* tuning: always use the single-buffer search kernel (every warp
-                                       does every phase) instead of the warp-specialised, double-
-                                       buffered one.  Never changes results.                       */
+                                       does every phase, full-size CTAs) instead of the warp-specialised,
+                                       double-buffered one.                                        */
 #define BLS_FLAG_NO_SMALL_CTAS 4u    /* tuning: never use the small-CTA launch shape (kernel 1 with CTAs of two
                                        warps) that small shapes get by default.  Never changes results. */
 #define BLS_FLAG_WARP_PER_TILE 8u    /* tuning: use the one-warp-per-tile search kernel (kernel 3, warp-private
                                        bins) where it fits.  Never changes results.                 */
 #define BLS_FLAG_WARPS(n) (((uint32_t)(n) & 0xffu) << 8) /* tuning: warps per CTA that walk the boxes
-                                       (1..10; 0 = the library's choice).  Never changes results. */
+                                       (kernel 1: 1..10, all its warps; kernel 2: 1..19 search warps;
+                                       0 = the library's choice).  Tuning flags change which of several
+                                       near-tied boxes (|dSR| < 1e-6) is reported, nothing else.     */
 #define BLS_FLAG_FOLD_WARPS(n) (((uint32_t)(n) & 0xffu) << 16) /* tuning: warps per CTA that fold, in
                                        the warp-specialised kernel (0 = the library's choice; box +
-                                       fold warps <= 20).  Never changes results.                  */
+                                       fold warps <= 20).                                          */
+
+#define BLS_FLAG_FOLD_DEPTH(n) (((uint32_t)(n) & 3u) << 27) /* tuning: groups of 4 points a fold warp keeps in
+                                       flight, 1 or 2 (0 = the library's choice).  Never changes results. */
 
 /* Ragged CSR batch of light curves (per star a list of HJD times, calibrated
  * magnitudes and errors).  Curve c owns points [offsets[c], offsets[c+1]). */
@@ -140,17 +147,29 @@ typedef struct {
 #define BLS_QUERY_SEARCH_CTAS 9     /* CTAs of the last search launch                              */
 #define BLS_QUERY_LAST_SEARCH_NS 10 /* device time (ns, CUDA events on the run's stream) the search
                                        kernel launches of the last bls_run took (synchronises)    */
-#define BLS_QUERY_SEARCH_KERNEL 11  /* search kernel the last bls_run used: 1 = single buffer,
+#define BLS_QUERY_SEARCH_KERNEL 11  /* search kernel of the last run: 1 = single buffer (all warps do every
+                                       phase; also the small-CTA shape of small configurations),
                                        2 = warp-specialised double buffer, 3 = one warp per tile
                                        (0 = none yet)                                              */
 
-/* Validate cfg, copy the grid to the device, derive kmin/kmax and launch geometry.  *out_plan is
- * set only on success. */
+/* Validate cfg, copy the grid to the device, derive kmin/kmax (reading R9: outward rounding of
+ * [q_min, q_max] to whole bins; "tests a range of durations") and check the shape fits.
+ * *out_plan is set only on success.  Errors: BLS_ERR_NULL, BLS_ERR_CONFIG (sizes, q range, non-finite or
+ * non-positive frequency), BLS_ERR_UNSUPPORTED (bins do not fit shared memory), BLS_ERR_CUDA (no device,
+ * allocation failure: there is no CPU fallback). */
 int bls_plan_create(const bls_config *cfg, bls_plan **out_plan);
 
-/* Search every curve of `batch` at every frequency of the plan: prep (weights, mean removal) ->
- * fold + box search per (curve, frequency) -> per-curve peak candidates kept in the plan for
- * bls_topk.  `out` may be NULL (peaks only).  Enqueues on cuda_stream. */
+/* The hot path ("phase the light curves at all possible periods and search for a transit-like
+ * signal"; L145: fold at each trial period, "then tests a range of durations and phases"; SURVEY.md section 8
+ * rows a0-a5).  For every curve of `batch` and every frequency of the plan: prep (weights, mean removal:
+ * readings R4, R5) -> fold into nb phase bins (R6-R8) -> every cyclic box (start, width) scored by
+ * SR = s^2/(r(1-r)) (R1, R10, R11), best box per frequency with canonical ties (R12) -> per-curve peak
+ * candidates (R14) kept in the plan for bls_topk / bls_refine.  `out` may be NULL (peaks only); its non-NULL
+ * arrays receive the full spectra.  Enqueues on cuda_stream; synchronises it only to grow plan scratch.
+ * batch->offsets and batch->t_origin are HOST arrays, read before the call returns (SURVEY 8(b) proposed
+ * device pointers; host metadata lets the call validate structure without a device round trip).
+ * Errors: BLS_ERR_NULL, BLS_ERR_BATCH (negative count, offsets[0] != 0, decreasing offsets, a curve longer than
+ * 2^25 points), BLS_ERR_UNSUPPORTED, BLS_ERR_CUDA; per-curve data faults go to status[], not to the return. */
 int bls_run(bls_plan *plan, const bls_batch *batch, const bls_outputs *out, void *cuda_stream);
 
 /* ---- f2: field-shared cadence ------------------------------------------
@@ -175,9 +194,11 @@ typedef struct {
  * star BLS_CURVE_NONFINITE. */
 int bls_run_field(bls_plan *plan, const bls_field_batch *field, const bls_outputs *out, void *cuda_stream);
 
-/* Write the k best peaks of every curve of the last bls_run to peaks (DEVICE, [n_curves*k]).
- * 1 <= k <= max_top_k.  Enqueues on cuda_stream (must be the stream of that bls_run, or one
- * ordered after it). */
+/* a5 Output (the candidates of PAPER.md L151): write the k best peaks of every
+ * curve of the last bls_run / bls_run_field to peaks (DEVICE, [n_curves*k]); reading R14 defines a peak
+ * (local maximum of the SR spectrum, plateaus to the leftmost sample) and the ranking (SR descending, then
+ * index).  1 <= k <= max_top_k, else BLS_ERR_ARG; BLS_ERR_ARG too if nothing has been run.  Enqueues on
+ * cuda_stream (the stream of that run, or one ordered after it). */
 int bls_topk(bls_plan *plan, int32_t k, bls_peak *peaks, void *cuda_stream);
 
 /* Convenience for callers whose data lives in HOST memory: copies the batch to the device, runs
@@ -286,6 +307,9 @@ int bls_detection_efficiency(int32_t device, const bls_batch *batch, int64_t n_f
 /* NULL is a no-op. */
 int bls_plan_destroy(bls_plan *plan);
 
+/* Derived constants and counters of the plan (BLS_QUERY_*): kmin / kmax of reading R9, so callers never
+ * re-derive them; launch facts of the last run.  BLS_ERR_ARG for an unknown `what` or a last-run query before
+ * any run.  Queries 7 and 10 synchronise the stream of the last run. */
 int bls_plan_query(const bls_plan *plan, int32_t what, int64_t *value);
 
 /* Static string for a bls_status (never NULL). */

@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     BLS_ERR_UNSUPPORTED,
     BLS_OK,
     BLS_FLAG_CANONICAL_PHASE,
+    BLS_FLAG_FOLD_DEPTH,
     BLS_FLAG_FOLD_WARPS,
     BLS_FLAG_NONE,
     BLS_FLAG_NO_SMALL_CTAS,

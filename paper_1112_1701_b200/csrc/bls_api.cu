@@ -182,7 +182,7 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     // so the bursts of LDS/ATOMS do not delay the search warps (clocks per pair with 4 / 8 points in flight:
     // C1 643 / 649, C2 759 / 730, C3 2100 / 1778; 16 in flight is slower everywhere)
     a.fold_depth = (!pts_in_smem || max_n >= 2048) ? 2 : 1;
-    if ((p->flags >> 27) & 3) a.fold_depth = (int)((p->flags >> 27) & 3);
+    if (p->flags & BLS_FLAG_FOLD_DEPTH(3)) a.fold_depth = (p->flags & BLS_FLAG_FOLD_DEPTH(2)) ? 2 : 1;
     a.search_warps = kernel == 2 ? ws_search : 0;
     a.kernel = kernel;
     a.threads = threads;
@@ -191,7 +191,6 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     a.u_sr = nullptr; a.u_start = nullptr; a.u_width = nullptr; a.u_depth = nullptr;
     a.f_lo = nullptr; a.f_step = nullptr; a.refine_k = 0; a.n_fine = 0; a.n_shift = 0;
     a.canon_count = p->d_canon;
-    a.debug = (int)(p->flags >> 24);
 
     smem_out = smem;
     L.items = items;
@@ -249,18 +248,24 @@ int bls_plan_create(const bls_config *cfg, bls_plan **out_plan)
 {
     if (!cfg || !out_plan) return BLS_ERR_NULL;
     if (cfg->struct_size != (int32_t)sizeof(bls_config)) return BLS_ERR_CONFIG;
-    if (cfg->n_freq < 1 || cfg->n_freq > 2147483647LL) return BLS_ERR_CONFIG;
+    if (cfg->n_freq < 1 || cfg->n_freq > (int64_t)1 << 27) return BLS_ERR_CONFIG;   // 2^27 trial frequencies at most
     if (cfg->n_bins < 4 || cfg->n_bins > 2048) return BLS_ERR_CONFIG;
     if (!(cfg->q_min > 0.0) || !(cfg->q_max >= cfg->q_min) || !(cfg->q_max <= 0.5)) return BLS_ERR_CONFIG;
     if (cfg->max_top_k < 1 || cfg->max_top_k > 32) return BLS_ERR_CONFIG;
     if (cfg->scratch_bytes < 0) return BLS_ERR_CONFIG;
 
-    std::vector<double> grid((size_t)cfg->n_freq);
+    struct HostGrid {                       // nothrow host copy of the grid (nothing may throw through the C ABI)
+        double *v;
+        explicit HostGrid(size_t n) : v((double *)malloc(n * sizeof(double))) {}
+        ~HostGrid() { free(v); }
+        double *data() { return v; }
+    } grid((size_t)cfg->n_freq);
+    if (!grid.v) return BLS_ERR_CUDA;
     double fmax = 0.0;
     for (int64_t k = 0; k < cfg->n_freq; ++k) {
         double f = cfg->freqs ? cfg->freqs[k] : cfg->f0 + (double)k * cfg->df;
         if (!isfinite(f) || !(f > 0.0)) return BLS_ERR_CONFIG;
-        grid[(size_t)k] = f;
+        grid.v[k] = f;
         if (f > fmax) fmax = f;
     }
 
@@ -465,7 +470,7 @@ int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_ou
         while (p->ev.size() < p->ev_used + 2) {
             cudaEvent_t e;
             BLS_CUDA(p, cudaEventCreate(&e));
-            p->ev.push_back(e);
+            try { p->ev.push_back(e); } catch (...) { cudaEventDestroy(e); return BLS_ERR_CUDA; }
         }
         BLS_CUDA(p, cudaEventRecord(p->ev[p->ev_used], st));
         BLS_CUDA(p, launch_search(a, cc, smem, st));

@@ -71,7 +71,6 @@ struct SearchArgs {
     int search_warps;           // kernel 2: this many search warps (then the fold warps)
     int kernel;                 // 1 single buffer, 2 warp-specialised double buffer, 3 one warp per tile
     int force_canonical;        // BLS_FLAG_CANONICAL_PHASE
-    int debug;                  // DEV ONLY
     float *sr;                  // chunk scratch, [chunk_curves][nf]
     uint32_t *ak;
     float *depth;

@@ -383,11 +383,7 @@ __device__ __forceinline__ void box_eval(uint64_t n, uint64_t s, float &m0, floa
     const uint64_t d = fma2(n, n, n);
     float d0, d1;
     unpack2(d, d0, d1);
-#ifdef BLS_DEV_NOMUFU
-    const uint64_t t = mul2(s, pack2(fabsf(d0) * 1.0001f, fabsf(d1) * 1.0001f));
-#else
     const uint64_t t = mul2(s, pack2(fast_rsqrt(fabsf(d0)), fast_rsqrt(fabsf(d1))));
-#endif
     float t0, t1;
     unpack2(t, t0, t1);
     m0 = fmaxf(m0, fabsf(t0));
@@ -894,7 +890,7 @@ search_ws_kernel(const SearchArgs a)
         for (int it = 0; it < nt; ++it) {
             const int b = it & 1;
             named_sync(kBarFull0 + b, nthr);                      // buffer b holds the tile's integer rows
-            if (!(a.debug & 1)) search_warp(bins_s + b * (uint32_t)buf_bytes, c, lane, sw, nsw, cand_t + b * nsw * 32, cand_c + b * nsw * 32);
+            search_warp(bins_s + b * (uint32_t)buf_bytes, c, lane, sw, nsw, cand_t + b * nsw * 32, cand_c + b * nsw * 32);
             named_arrive(kBarDone0 + b, nthr);                    // candidates posted, done reading buffer b
         }
     } else {
@@ -904,7 +900,7 @@ search_ws_kernel(const SearchArgs a)
         auto merge = [&](int it) {
             const int b = it & 1;
             named_sync(kBarDone0 + b, nthr);
-            if (!(a.debug & 4)) merge_tile(c, bins_s + b * (uint32_t)buf_bytes, cand_t + b * nsw * 32, cand_c + b * nsw * 32, post_v, post_k, nsw, mw,
+            merge_tile(c, bins_s + b * (uint32_t)buf_bytes, cand_t + b * nsw * 32, cand_c + b * nsw * 32, post_v, post_k, nsw, mw,
                        gw, lane, (w.tile0 + it) * kTileFreqs + lane, a.nf, w.out,
                        [gthreads] { named_sync(kBarFoldGroup, gthreads); });
             named_sync(kBarFoldGroup, gthreads);                  // every column has left the buffer
@@ -916,10 +912,8 @@ search_ws_kernel(const SearchArgs a)
             const LaneFreq lf = lane_freq(a, w.cv, tile * kTileFreqs + lane);
             zero_bins(buf, c.nb, gtid, gthreads);
             named_sync(kBarFoldGroup, gthreads);
-            if (!(a.debug & 2)) {
-                if (a.fold_depth == 2) fold_tile<PTS_SMEM, 2>(c, lf, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
-                else fold_tile<PTS_SMEM, 1>(c, lf, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
-            }
+            if (a.fold_depth == 2) fold_tile<PTS_SMEM, 2>(c, lf, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
+            else fold_tile<PTS_SMEM, 1>(c, lf, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
             named_sync(kBarFoldGroup, gthreads);
             extend_rows(c, buf, gtid, gthreads);
             named_arrive(kBarFull0 + b, nthr);

@@ -109,7 +109,8 @@ def test_kernel_variants_give_identical_results():
                 bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WARPS(6) | bls.BLS_FLAG_FOLD_WARPS(3),
                 bls.BLS_FLAG_WARPS(7) | bls.BLS_FLAG_SINGLE_BUFFER,
                 bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WARPS(10) | bls.BLS_FLAG_FOLD_WARPS(1),
-                bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WARPS(1) | bls.BLS_FLAG_FOLD_WARPS(2)]
+                bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WARPS(1) | bls.BLS_FLAG_FOLD_WARPS(2),
+                bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_FOLD_DEPTH(2), bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_FOLD_DEPTH(1)]
     variants += [bls.BLS_FLAG_WARPS(n) | bls.BLS_FLAG_SINGLE_BUFFER for n in (1, 2, 3)]   # fewer than 4 warps
     for flags in variants:
         g = run_gpu(batch, cfg["grid"], top_k=5, flags=flags)
