@@ -38,7 +38,7 @@ METRIC = "bls_point_folds_per_sec"
 UNIT = "point-folds/s"
 
 # Roofline constants, measured on B200 by paper_1112_1701_b200/microbench/issue_rates.cu
-# (profiles/r02_microbench.md): lane-operations per clock per SM.
+# (profiles/r02a_microbench.md): lane-operations per clock per SM.
 LSU_LANE_OPS_PER_CLK_SM = 32.0       # shared wavefront pipe: conflict-free ATOMS.ADD 31.97
 XU_LANE_OPS_PER_CLK_SM = 16.0        # MUFU.RSQ 16.00: one per box
 ISSUE_LANE_INSTR_PER_CLK_SM = 128.0  # 4 schedulers x 32 lanes
@@ -275,7 +275,7 @@ def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_r
     torch.cuda.synchronize()
     sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
-    search_ns = 0
+    search_ns, search_launches = 0, 0
     wall0 = time.perf_counter()
     for i in range(steps):
         flush.zero_()                       # L2 flush between timed iterations (outside the events)
@@ -283,6 +283,7 @@ def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_r
         raw = step()
         ev[i][1].record()
         search_ns += plan.query(B.QUERY_LAST_SEARCH_NS)   # synchronises; outside the event pair
+        search_launches += plan.query(B.QUERY_LAST_SEARCH_LAUNCHES)
     torch.cuda.synchronize()
     wall = time.perf_counter() - wall0
     clocks = sampler.stop()
@@ -358,12 +359,19 @@ def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_r
     clk_per_pair = n_sm * max_hz * search_s / (n_curves * grid.nf)
     peak = n_sm * max_hz * n_mean / pc["min"]
     facts = profile_facts(name)
+    # per launch (one launch = one chunk of curves): pairs, algorithmic point-folds, average duration, DRAM bytes
+    pairs_per_launch = n_curves * grid.nf * steps / max(search_launches, 1)
+    bpp = facts.get("dram_bytes_per_pair")
     out["roofline"] = {
         "bound": "alu", "kernel": kernel_name, "achieved": achieved, "peak": peak, "unit": UNIT, "frac": achieved / peak,
-        "traffic": facts.get("dram_bytes_per_launch"),
+        "traffic": (bpp * pairs_per_launch) if bpp else None,
+        "per_launch": {"launches_per_step": search_launches / steps, "avg_launch_ms": 1e3 * search_s * steps / max(search_launches, 1),
+                       "point_folds": pf_per_step * steps / max(search_launches, 1),
+                       "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per (curve, frequency) pair of the "
+                                         "ncu --set full capture (%s) x pairs per launch" % facts.get("source")},
         "peak_def": "n_SM*f_max*N/t_min per (curve,frequency) pair, t_min = max(LSU (2N+2(nb+kmax))/32, XU nb*nk/16, "
                     "issue (5N+3.5 nb nk)/128) clk = max(%.0f, %.0f, %.0f); rates measured by microbench/issue_rates.cu "
-                    "(profiles/r02_microbench.md); f_max=%d MHz, n_SM=%d (DESIGN.md section 7)" % (
+                    "(profiles/r02a_microbench.md); f_max=%d MHz, n_SM=%d (DESIGN.md section 7)" % (
                         pc["lsu"], pc["xu"], pc["issue"], max_hz / 1e6, n_sm),
         "clk_per_pair": clk_per_pair,
         "frac_method_floor": pc["method"] / clk_per_pair,

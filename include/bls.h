@@ -151,6 +151,8 @@ typedef struct {
                                        phase; also the small-CTA shape of small configurations),
                                        2 = warp-specialised double buffer, 3 = one warp per tile
                                        (0 = none yet)                                              */
+#define BLS_QUERY_LAST_SEARCH_LAUNCHES 12 /* search kernel launches of the last bls_run (one per chunk of
+                                       curves): LAST_SEARCH_NS / this = the average launch duration */
 
 /* Validate cfg, copy the grid to the device, derive kmin/kmax (reading R9: outward rounding of
  * [q_min, q_max] to whole bins; "tests a range of durations") and check the shape fits.

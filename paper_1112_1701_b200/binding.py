@@ -37,7 +37,7 @@ def BLS_FLAG_FOLD_DEPTH(n):
     return (int(n) & 3) << 27
 (QUERY_KMIN, QUERY_KMAX, QUERY_NBINS, QUERY_NFREQ, QUERY_SCRATCH_BYTES, QUERY_LAST_LAUNCHES,
  QUERY_LAST_CANONICAL, QUERY_TILE_FREQS, QUERY_SEARCH_CTAS, QUERY_LAST_SEARCH_NS,
- QUERY_SEARCH_KERNEL) = range(1, 12)
+ QUERY_SEARCH_KERNEL, QUERY_LAST_SEARCH_LAUNCHES) = range(1, 13)
 
 
 class BlsConfig(C.Structure):

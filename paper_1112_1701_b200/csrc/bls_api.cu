@@ -336,6 +336,7 @@ int bls_plan_query(const bls_plan *p, int32_t what, int64_t *value)
         case BLS_QUERY_TILE_FREQS: *value = (int64_t)p->last_tiles_per_item * kTileFreqs; break;
         case BLS_QUERY_SEARCH_CTAS: *value = p->last_search_ctas; break;
         case BLS_QUERY_SEARCH_KERNEL: *value = p->last_kernel; break;
+        case BLS_QUERY_LAST_SEARCH_LAUNCHES: *value = (int64_t)(p->ev_used / 2); break;
         case BLS_QUERY_LAST_SEARCH_NS: {
             if (p->last_n_curves < 0) return BLS_ERR_ARG;
             if (cudaSetDevice(p->device) != cudaSuccess) return BLS_ERR_CUDA;

@@ -33,11 +33,11 @@ constexpr int kThreads = 1024;
 constexpr int kIters = 2048;
 
 enum Test { ATOMS_CF, ATOMS_RAND, LDS128_BCAST, LDS32_CF, MUFU_RSQ, FADD, FADD2, FFMA, FFMA2, FMNMX3, DFMA, IMAD_WIDE,
-            FOLD_MIX, BOX_MIX, BOX_MIX2, ATOMS_CF2, LDS64_BCAST, LDS32_BCAST, LDS64_CF, I2FP, MUFU_I2FP, FMUL2, BOX_PACKED, BOX_PACKED_CVT, N_TESTS };
+            FOLD_MIX, BOX_MIX, BOX_MIX2, ATOMS_CF2, LDS64_BCAST, LDS32_BCAST, LDS64_CF, I2FP, MUFU_I2FP, FMUL2, BOX_PACKED, BOX_PACKED_CVT, BOX_PACKED_THRESH, BOX_PACKED_PAIRDIV, N_TESTS };
 static const char *kNames[N_TESTS] = {"atoms_add_cf", "atoms_add_rand", "lds128_bcast", "lds32_cf", "mufu_rsq", "fadd",
                                       "fadd2", "ffma", "ffma2", "fmnmx3", "dfma", "imad_wide", "fold_mix", "box_mix",
                                       "box_mix_fadd2", "atoms_add_cf_min", "lds64_bcast", "lds32_bcast", "lds64_cf", "i2fp",
-                                      "mufu_plus_i2fp", "fmul2", "box_packed", "box_packed_cvt"};
+                                      "mufu_plus_i2fp", "fmul2", "box_packed", "box_packed_cvt", "box_nodiv_thresh", "box_nodiv_pair"};
 // lane-operations each thread performs per inner iteration (what the rate is quoted in)
 static const double kOpsPerIter[N_TESTS] = {8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 4, 8, 8, 8, 8, 8, 8, 8, 8, 8, 14, 14};
 static const char *kUnit[N_TESTS] = {"ATOMS lane-ops", "ATOMS lane-ops", "LDS.128 lane-loads", "LDS.32 lane-loads",
@@ -45,7 +45,9 @@ static const char *kUnit[N_TESTS] = {"ATOMS lane-ops", "ATOMS lane-ops", "LDS.12
                                      "FFMA2 lane-instr (2 fmas each)", "FMNMX3 lane-ops (+1/8 FADD)", "DFMA lane-ops",
                                      "IMAD.WIDE lane-ops", "point-folds", "boxes", "boxes", "ATOMS lane-ops", "LDS.64 lane-loads", "LDS.32 lane-loads", "LDS.64 lane-loads",
                                      "I2FP lane-ops", "MUFU lane-ops (each with one I2FP beside it)", "FMUL2 lane-instr (2 muls each)",
-                                     "boxes (packed f32x2 search mix, rows already fp32)", "boxes (packed f32x2 search mix, int rows converted on the fly)"};
+                                     "boxes (packed f32x2 search mix, rows already fp32)", "boxes (packed f32x2 search mix, int rows converted on the fly)",
+                                     "boxes (no division: excess s^2 - B r(1-r) against a threshold B, FMNMX3; finds no argmax by itself)",
+                                     "boxes (division-free compare of two boxes: cross-multiplied, one MUFU.RCP per two boxes)"};
 
 __device__ __forceinline__ float rsq(float x) { float y; asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ unsigned long long add2(unsigned long long a, unsigned long long b)
@@ -203,6 +205,53 @@ __global__ void __launch_bounds__(kThreads, 1) bench(long long *cycles, float *s
                 f6 = fmaxf(f6, fabsf(t0)); f7 = fmaxf(f7, fabsf(t1));
             }
             p0 = rs[0]; p1 = rs[1]; p2 = rs[2]; p3 = rs[3]; p4 = rs[4]; p5 = rs[5]; p6 = rs[6];
+        } else if (T == BOX_PACKED_THRESH) {
+            // DESIGN.md section 7, "division-free evaluate", form 1: per box pair FFMA2, FADD2, FFMA2 (n^2 + n), FMUL2 (s^2),
+            // FFMA2 (s^2 - B r(1-r)), and one FMNMX3 per box pair: no MUFU at all.  It only says whether a box beats the
+            // threshold B; the argmax needs a second pass over the groups that did.
+            const uint2 wi = *reinterpret_cast<const uint2 *>(sm + (it % nb) * 64 + (lane & 15) * 2);
+            const uint2 yi = *reinterpret_cast<const uint2 *>(sm + (it % nb) * 64 + 32 + (lane & 15) * 2);
+            const unsigned long long W = pack2(__uint2float_rn(wi.x), __uint2float_rn(wi.y));
+            const unsigned long long Y = pack2(__int2float_rn((int)yi.x), __int2float_rn((int)yi.y));
+            unsigned long long *rn = q;
+            unsigned long long rs[7] = {p0, p1, p2, p3, p4, p5, p6};
+#pragma unroll
+            for (int u = 0; u < 7; ++u) {
+                rn[u] = fma2(W, pm, rn[u]);
+                rs[u] = add2(rs[u], Y);
+                const unsigned long long d = fma2(rn[u], rn[u], rn[u]);
+                const unsigned long long e = fma2(p7, d, mul2(rs[u], rs[u]));
+                float e0, e1; unpack2(e, e0, e1);
+                f6 = fmax3(f6, e0, e1);
+            }
+            p0 = rs[0]; p1 = rs[1]; p2 = rs[2]; p3 = rs[3]; p4 = rs[4]; p5 = rs[5]; p6 = rs[6];
+        } else if (T == BOX_PACKED_PAIRDIV) {
+            // form 2: boxes A, B of the same frequency share one reciprocal: SR_A = s_A^2 d_B / (d_A d_B).  Per two box
+            // pairs (4 boxes): 2 FFMA2 + 2 FADD2 + 2 FFMA2 (sums, d), FMUL2 (d_A d_B), 2 FMUL2 (s^2), 2 FMUL2 (cross),
+            // 2 MUFU.RCP, 2 FMUL2, 2 FMNMX3 = 17 instructions
+            const uint2 wi = *reinterpret_cast<const uint2 *>(sm + (it % nb) * 64 + (lane & 15) * 2);
+            const uint2 yi = *reinterpret_cast<const uint2 *>(sm + (it % nb) * 64 + 32 + (lane & 15) * 2);
+            const unsigned long long W = pack2(__uint2float_rn(wi.x), __uint2float_rn(wi.y));
+            const unsigned long long Y = pack2(__int2float_rn((int)yi.x), __int2float_rn((int)yi.y));
+            unsigned long long *rn = q;
+            unsigned long long rs[6] = {p0, p1, p2, p3, p4, p5};
+#pragma unroll
+            for (int u = 0; u < 6; u += 2) {
+                rn[u] = fma2(W, pm, rn[u]); rn[u + 1] = fma2(W, pm, rn[u + 1]);
+                rs[u] = add2(rs[u], Y); rs[u + 1] = add2(rs[u + 1], Y);
+                const unsigned long long dA = fma2(rn[u], rn[u], rn[u]), dB = fma2(rn[u + 1], rn[u + 1], rn[u + 1]);
+                const unsigned long long P = mul2(dA, dB);
+                const unsigned long long xA = mul2(mul2(rs[u], rs[u]), dB), xB = mul2(mul2(rs[u + 1], rs[u + 1]), dA);
+                float P0, P1; unpack2(P, P0, P1);
+                float i0, i1;
+                asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(i0) : "f"(P0));
+                asm volatile("rcp.approx.ftz.f32 %0, %1;" : "=f"(i1) : "f"(P1));
+                const unsigned long long inv = pack2(i0, i1);
+                float a0, a1, b0, b1;
+                unpack2(mul2(xA, inv), a0, a1); unpack2(mul2(xB, inv), b0, b1);
+                f6 = fmax3(f6, a0, b0); f7 = fmax3(f7, a1, b1);
+            }
+            p0 = rs[0]; p1 = rs[1]; p2 = rs[2]; p3 = rs[3]; p4 = rs[4]; p5 = rs[5];
         } else if (T == BOX_MIX2) {
             // 8 boxes with packed (r, s) running sums: FADD2, FFMA, MUFU, FMUL, 1/2 FMNMX3 per box
             const unsigned long long wy = ((unsigned long long)sm[(it % nb) * 64 + lane] << 32) | 0x2b8cbccbu;
@@ -285,5 +334,7 @@ int main()
     run<FMUL2>(n_sm, nb, d_cyc, d_sink);
     run<BOX_PACKED>(n_sm, nb, d_cyc, d_sink);
     run<BOX_PACKED_CVT>(n_sm, nb, d_cyc, d_sink);
+    run<BOX_PACKED_THRESH>(n_sm, nb, d_cyc, d_sink);
+    run<BOX_PACKED_PAIRDIV>(n_sm, nb, d_cyc, d_sink);
     return 0;
 }
