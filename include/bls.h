@@ -95,6 +95,10 @@ typedef struct {
                                        the warp-specialised kernel (0 = the library's choice; box +
                                        fold warps <= 20).                                          */
 
+#define BLS_FLAG_MERGE_WARPS(n) (((uint32_t)(n) & 7u) << 24) /* tuning: warps per CTA that share the exact
+                                       merge of a tile, 1..7 (0 = the library's choice).  Changes which of
+                                       several near-tied boxes is reported, nothing else.          */
+
 #define BLS_FLAG_FOLD_DEPTH(n) (((uint32_t)(n) & 3u) << 27) /* tuning: groups of 4 points a fold warp keeps in
                                        flight, 1 or 2 (0 = the library's choice).  Never changes results. */
 

@@ -117,6 +117,7 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     const size_t sm_smem = (size_t)p->max_smem_sm;
     const int warps_flag = (int)((p->flags >> 8) & 0xffu);
     const int fold_flag = (int)((p->flags >> 16) & 0xffu);
+    const int merge_flag = (int)((p->flags >> 24) & 7u);
     // Kernel 2 (warp-specialised, two bin buffers) whenever its buffers fit shared memory, with the
     // curve staged in shared memory if that fits too; otherwise kernel 1 (one buffer, two CTAs per SM).
     int ws_search = kWsSearchWarps;
@@ -184,6 +185,9 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     a.fold_depth = (!pts_in_smem || max_n >= 2048) ? 2 : 1;
     if (p->flags & BLS_FLAG_FOLD_DEPTH(3)) a.fold_depth = (p->flags & BLS_FLAG_FOLD_DEPTH(2)) ? 2 : 1;
     a.search_warps = kernel == 2 ? ws_search : 0;
+    // the exact merge re-walks ONE start per column (kmax rows): its widths are split over a few warps
+    a.merge_warps = kernel == 2 ? 2 : (small ? kSmallWarps : 4);
+    if (merge_flag >= 1 && merge_flag <= kMergeWarps) a.merge_warps = merge_flag;
     a.kernel = kernel;
     a.threads = threads;
     a.force_canonical = (p->flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0;

@@ -45,7 +45,7 @@ constexpr int kTileFreqs = 32;        // frequencies per tile = lanes of a warp
 constexpr int kMaxSearchWarps = 10;   // kernel 1 upper bound (BLS_FLAG_WARPS override); 2 CTAs x 10 warps x 96 registers fill an SM
 constexpr int kWsMaxWarps = 20;       // warp-specialised kernel: search warps + fold warps
 constexpr int kWsSearchWarps = 8;     // its default split: 8 search (two per SM sub-partition) + 12 fold; 20 warps = 5 per sub-partition leave 96 registers per thread
-constexpr int kMergeWarps = 8;        // warps of a group that share the exact merge of a tile (one start each, S <= 8)
+constexpr int kMergeWarps = 8;        // upper bound of the warps that share the exact merge of a tile (BLS_FLAG_MERGE_WARPS)
 constexpr int kSmallWarps = 2;        // small shapes: kernel 1 with CTAs of this many warps ...
 constexpr int kSmallCtasMin = 8;      // ... when at least this many fit an SM
 constexpr int kWtWarps = 5;           // warp-per-tile kernel: warps per CTA (two CTAs per SM)
@@ -69,6 +69,7 @@ struct SearchArgs {
     int fold_depth;             // kernel 2: groups of 4 points a fold warp keeps in flight (1 or 2)
     int nrows;                  // bin rows per buffer: nb + cyclic extension (search_rows_for)
     int search_warps;           // kernel 2: this many search warps (then the fold warps)
+    int merge_warps;            // warps that share the exact merge of a tile (1..kMergeWarps; they split the widths)
     int kernel;                 // 1 single buffer, 2 warp-specialised double buffer, 3 one warp per tile
     int force_canonical;        // BLS_FLAG_CANONICAL_PHASE
     float *sr;                  // chunk scratch, [chunk_curves][nf]
