@@ -12,6 +12,8 @@ from .binding import (  # noqa: F401
     BLS_FLAG_CANONICAL_PHASE,
     BLS_FLAG_FOLD_DEPTH,
     BLS_FLAG_FOLD_WARPS,
+    BLS_FLAG_MERGE_WARPS,
+    BLS_FLAG_WS_SHAPE,
     BLS_FLAG_NONE,
     BLS_FLAG_NO_SMALL_CTAS,
     BLS_FLAG_WARP_PER_TILE,

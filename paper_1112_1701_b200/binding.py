@@ -35,6 +35,14 @@ def BLS_FLAG_FOLD_WARPS(n):
 
 def BLS_FLAG_FOLD_DEPTH(n):
     return (int(n) & 3) << 27
+
+
+def BLS_FLAG_MERGE_WARPS(n):
+    return (int(n) & 7) << 24
+
+
+def BLS_FLAG_WS_SHAPE(n):
+    return (int(n) & 7) << 4
 (QUERY_KMIN, QUERY_KMAX, QUERY_NBINS, QUERY_NFREQ, QUERY_SCRATCH_BYTES, QUERY_LAST_LAUNCHES,
  QUERY_LAST_CANONICAL, QUERY_TILE_FREQS, QUERY_SEARCH_CTAS, QUERY_LAST_SEARCH_NS,
  QUERY_SEARCH_KERNEL, QUERY_LAST_SEARCH_LAUNCHES) = range(1, 13)

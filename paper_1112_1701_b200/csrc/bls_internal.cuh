@@ -45,6 +45,9 @@ constexpr int kTileFreqs = 32;        // frequencies per tile = lanes of a warp
 constexpr int kMaxSearchWarps = 10;   // kernel 1 upper bound (BLS_FLAG_WARPS override); 2 CTAs x 10 warps x 96 registers fill an SM
 constexpr int kWsMaxWarps = 20;       // warp-specialised kernel: search warps + fold warps
 constexpr int kWsSearchWarps = 8;     // its default split: 8 search (two per SM sub-partition) + 12 fold; 20 warps = 5 per sub-partition leave 96 registers per thread
+constexpr int kSmax = 8;              // starts per start tile a search thread holds at 96 registers
+constexpr int kSmaxWide = 13;         // ... and with the registers the fold warps hand over (kernel 2, shapes 1 and 2)
+constexpr int kWsShapes = 3;          // kernel 2 launch shapes (WsShape<0..2> in bls_search.cu)
 constexpr int kMergeWarps = 8;        // upper bound of the warps that share the exact merge of a tile (BLS_FLAG_MERGE_WARPS)
 constexpr int kSmallWarps = 2;        // small shapes: kernel 1 with CTAs of this many warps ...
 constexpr int kSmallCtasMin = 8;      // ... when at least this many fit an SM
@@ -69,6 +72,7 @@ struct SearchArgs {
     int fold_depth;             // kernel 2: groups of 4 points a fold warp keeps in flight (1 or 2)
     int nrows;                  // bin rows per buffer: nb + cyclic extension (search_rows_for)
     int search_warps;           // kernel 2: this many search warps (then the fold warps)
+    int ws_shape;               // kernel 2: 0 = equal registers, run-time split; 1.. = fixed splits with setmaxnreg (WsShape)
     int merge_warps;            // warps that share the exact merge of a tile (1..kMergeWarps; they split the widths)
     int kernel;                 // 1 single buffer, 2 warp-specialised double buffer, 3 one warp per tile
     int force_canonical;        // BLS_FLAG_CANONICAL_PHASE
@@ -157,6 +161,7 @@ __device__ __forceinline__ double block_max_d(double v, double *sh) {
 // Bin rows a search buffer holds when the start bins are dealt to `slots` half-warps: the nb bins
 // plus the cyclic extension the widest box of the last start reaches (bls_search.cu).
 int search_rows_for(int nb, int kmax, int slots);
+int ws_shape_warps(int shape, int *search_warps);   // kernel 2 launch shape -> warps per CTA, search warps (0 = run-time)
 size_t search_smem_bytes(int nb, int kmax, int warps, int buffers, int64_t n_points_in_smem);
 cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int nb, int force_canon,
                               int32_t *bins, unsigned long long *n_canon, int sm_count, cudaStream_t st);
