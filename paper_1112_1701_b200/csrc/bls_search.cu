@@ -44,7 +44,8 @@ size_t search_smem_bytes(int nb, int kmax, int warps, int buffers, int64_t n_poi
 {
     const size_t bins = (size_t)search_rows_for(nb, kmax, 2 * warps) * kTileFreqs * 8;
     // candidates (rank, code) per buffer; merge posts: kernel 2 kMergeWarps, kernel 1 all its warps
-    const size_t cand = (size_t)buffers * warps * kTileFreqs * 8 + (size_t)(buffers == 2 ? kMergeWarps : warps) * kTileFreqs * 8;
+    const size_t cand = (size_t)buffers * warps * kTileFreqs * 8 + (size_t)(buffers == 2 ? kMergeWarps : warps) * kTileFreqs * 8 +
+                        (buffers == 2 ? 16 : 0);                  // kernel 2: two mbarriers
     return (size_t)buffers * bins + cand + (size_t)n_points_in_smem * sizeof(PointRec);
 }
 
@@ -804,8 +805,9 @@ search_kernel(const SearchArgs a)
 //      (atomics + point broadcasts), the box search by the XU pipe (one MUFU.RSQ per box): they run
 //      CONCURRENTLY on different warps.  "Search warps" rank the boxes of tile i in one bin buffer
 //      while "fold warps" merge tile i-1 out of the other buffer and then zero / fold / extend tile
-//      i+1 into it.  Hand-off by named barriers (bar.arrive on the producing side, bar.sync on the
-//      consuming side): FULL[b] fold -> search, DONE[b] search -> fold; one barrier for the fold group.
+//      i+1 into it.  Hand-off: FULL[b] fold -> search is an mbarrier each search warp polls on its own,
+//      DONE[b] search -> fold a named barrier (bar.arrive by the search warps, bar.sync by the fold warps);
+//      one named barrier for the fold group.
 __device__ __forceinline__ void named_sync(int id, int count)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
@@ -815,7 +817,27 @@ __device__ __forceinline__ void named_arrive(int id, int count)
     __threadfence_block();
     asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory");
 }
-enum { kBarFull0 = 1, kBarFull1 = 2, kBarDone0 = 3, kBarDone1 = 4, kBarFoldGroup = 5 };
+enum { kBarDone0 = 3, kBarDone1 = 4, kBarFoldGroup = 5 };
+
+// FULL[b] (fold -> search) is an mbarrier in shared memory: every fold thread arrives (release), every search
+// warp polls on its own, so the search warps are not re-aligned at every tile: they drift apart and one warp's
+// tile prologue / epilogue overlaps the steady loops of the others on the XU pipe.
+__device__ __forceinline__ void mbar_init(uint32_t addr, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(addr), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t addr)
+{
+    asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(addr) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t addr, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    } while (!ok);
+}
 
 // Launch shapes of kernel 2.  Shape 0: up to 20 warps at equal registers (96), the search / fold split chosen at
 // run time (BLS_FLAG_WARPS / BLS_FLAG_FOLD_WARPS).  Shapes 1 and 2: 24 warps launched at 80 registers; the fold
@@ -852,13 +874,14 @@ search_ws_kernel(const SearchArgs a)
     const int sw = warp - nfw;
     TileCtx c;
     const WorkItem w = work_item(a, c);
-    // smem: bins[2] [nrows][256 B] | cand_t[2], cand_c[2] [nsw][32] | post_v, post_k [kMergeWarps][32] | points [n]
+    // smem: bins[2] [nrows][256 B] | cand_t[2], cand_c[2] [nsw][32] | post_v, post_k [kMergeWarps][32] | FULL[2] | points [n]
     const size_t buf_bytes = (size_t)c.nrows * kRowBytes;
     float *cand_t = reinterpret_cast<float *>(smem_raw + 2 * buf_bytes);
     uint32_t *cand_c = reinterpret_cast<uint32_t *>(cand_t + 2 * nsw * 32);
     float *post_v = reinterpret_cast<float *>(cand_c + 2 * nsw * 32);
     uint32_t *post_k = reinterpret_cast<uint32_t *>(post_v + kMergeWarps * 32);
-    PointRec *pts_s = reinterpret_cast<PointRec *>(post_k + kMergeWarps * 32);
+    const uint32_t full_bar = smem_u32(post_k + kMergeWarps * 32);          // two 8-byte mbarriers
+    PointRec *pts_s = reinterpret_cast<PointRec *>(post_k + kMergeWarps * 32 + 4);
 
     if (w.meta.status != BLS_CURVE_OK) {
         zero_fill_outputs(w.out, w.tile0 * kTileFreqs, min(w.tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
@@ -866,6 +889,7 @@ search_ws_kernel(const SearchArgs a)
     }
     const PointRec *pts_g = a.pts + w.beg;
     stage_curve<PTS_SMEM>(pts_g, pts_s, c.n_pad, tid, nthr);        // a1 Load, by all warps
+    if (tid == 0) { mbar_init(full_bar, nfw * 32); mbar_init(full_bar + 8, nfw * 32); }
     __syncthreads();
     const uint32_t bins_s = smem_u32(smem_raw), pts_sa = smem_u32(pts_s);
     const int nt = w.tile1 - w.tile0;
@@ -875,7 +899,7 @@ search_ws_kernel(const SearchArgs a)
         if constexpr (SHAPE != 0) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(Shape::kSearchRegs));
         for (int it = 0; it < nt; ++it) {
             const int b = it & 1;
-            named_sync(kBarFull0 + b, nthr);                      // buffer b holds the tile's integer rows
+            mbar_wait(full_bar + 8 * b, (it >> 1) & 1);           // buffer b holds the tile's integer rows
             search_warp<Shape::kTileStarts>(bins_s + b * (uint32_t)buf_bytes, c, lane, sw, nsw, cand_t + b * nsw * 32,
                                       cand_c + b * nsw * 32);
             named_arrive(kBarDone0 + b, nthr);                    // candidates posted, done reading buffer b
@@ -904,7 +928,7 @@ search_ws_kernel(const SearchArgs a)
             else fold_tile<PTS_SMEM, 1>(c, lf, buf, pts_sa, pts_g, lane, gw, nfw, n_canon);
             named_sync(kBarFoldGroup, gthreads);
             extend_rows(c, buf, gtid, gthreads);
-            named_arrive(kBarFull0 + b, nthr);
+            mbar_arrive(full_bar + 8 * b);
         }
         for (int it = max(nt - 2, 0); it < nt; ++it) merge(it);   // drain
         count_canonical(a, n_canon, lane);

@@ -33,13 +33,13 @@ constexpr int kThreads = 1024;
 constexpr int kIters = 2048;
 
 enum Test { ATOMS_CF, ATOMS_RAND, LDS128_BCAST, LDS32_CF, MUFU_RSQ, FADD, FADD2, FFMA, FFMA2, FMNMX3, DFMA, IMAD_WIDE,
-            FOLD_MIX, BOX_MIX, BOX_MIX2, ATOMS_CF2, LDS64_BCAST, LDS32_BCAST, LDS64_CF, I2FP, MUFU_I2FP, FMUL2, BOX_PACKED, BOX_PACKED_CVT, BOX_PACKED_THRESH, BOX_PACKED_PAIRDIV, N_TESTS };
+            FOLD_MIX, BOX_MIX, BOX_MIX2, ATOMS_CF2, LDS64_BCAST, LDS32_BCAST, LDS64_CF, I2FP, MUFU_I2FP, FMUL2, BOX_PACKED, BOX_PACKED_CVT, BOX_PACKED_THRESH, BOX_PACKED_PAIRDIV, FFMA2_ALU, FFMA2_MUFU, FFMA_ALU, MUFU_ALU, N_TESTS };
 static const char *kNames[N_TESTS] = {"atoms_add_cf", "atoms_add_rand", "lds128_bcast", "lds32_cf", "mufu_rsq", "fadd",
                                       "fadd2", "ffma", "ffma2", "fmnmx3", "dfma", "imad_wide", "fold_mix", "box_mix",
                                       "box_mix_fadd2", "atoms_add_cf_min", "lds64_bcast", "lds32_bcast", "lds64_cf", "i2fp",
-                                      "mufu_plus_i2fp", "fmul2", "box_packed", "box_packed_cvt", "box_nodiv_thresh", "box_nodiv_pair"};
+                                      "mufu_plus_i2fp", "fmul2", "box_packed", "box_packed_cvt", "box_nodiv_thresh", "box_nodiv_pair", "ffma2_plus_alu", "ffma2_plus_mufu", "ffma_plus_alu", "mufu_plus_alu"};
 // lane-operations each thread performs per inner iteration (what the rate is quoted in)
-static const double kOpsPerIter[N_TESTS] = {8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 4, 8, 8, 8, 8, 8, 8, 8, 8, 8, 14, 14};
+static const double kOpsPerIter[N_TESTS] = {8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 4, 8, 8, 8, 8, 8, 8, 8, 8, 8, 14, 14, 14, 12, 16, 12, 16, 12};
 static const char *kUnit[N_TESTS] = {"ATOMS lane-ops", "ATOMS lane-ops", "LDS.128 lane-loads", "LDS.32 lane-loads",
                                      "MUFU lane-ops", "FADD lane-ops", "FADD2 lane-instr (2 adds each)", "FFMA lane-ops",
                                      "FFMA2 lane-instr (2 fmas each)", "FMNMX3 lane-ops (+1/8 FADD)", "DFMA lane-ops",
@@ -47,7 +47,11 @@ static const char *kUnit[N_TESTS] = {"ATOMS lane-ops", "ATOMS lane-ops", "LDS.12
                                      "I2FP lane-ops", "MUFU lane-ops (each with one I2FP beside it)", "FMUL2 lane-instr (2 muls each)",
                                      "boxes (packed f32x2 search mix, rows already fp32)", "boxes (packed f32x2 search mix, int rows converted on the fly)",
                                      "boxes (no division: excess s^2 - B r(1-r) against a threshold B, FMNMX3; finds no argmax by itself)",
-                                     "boxes (division-free compare of two boxes: cross-multiplied, one MUFU.RCP per two boxes)"};
+                                     "boxes (division-free compare of two boxes: cross-multiplied, one MUFU.RCP per two boxes)",
+                                     "warp-instr lanes (8 FFMA2 + 8 LOP3 per iteration: does a packed instruction hold the issue port for 2 clocks?)",
+                                     "warp-instr lanes (8 FFMA2 + 4 MUFU.RSQ per iteration)",
+                                     "warp-instr lanes (8 FFMA + 8 LOP3 per iteration)",
+                                     "warp-instr lanes (4 MUFU.RSQ + 8 LOP3 per iteration)"};
 
 __device__ __forceinline__ float rsq(float x) { float y; asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ unsigned long long add2(unsigned long long a, unsigned long long b)
@@ -252,6 +256,24 @@ __global__ void __launch_bounds__(kThreads, 1) bench(long long *cycles, float *s
                 f6 = fmax3(f6, a0, b0); f7 = fmax3(f7, a1, b1);
             }
             p0 = rs[0]; p1 = rs[1]; p2 = rs[2]; p3 = rs[3]; p4 = rs[4]; p5 = rs[5];
+        } else if (T == FFMA2_ALU) {
+            // if FFMA2 only held the FMA pipe for 2 clocks, the 8 LOP3 would issue in its shadow: 16 clocks per
+            // iteration per SM sub-partition warp slot; if it holds the issue port, 24
+            p0 = fma2(p0, pm, pc); x ^= (x >> 3) | 0x11u; p1 = fma2(p1, pm, pc); acc ^= (acc >> 5) | 0x101ull;
+            p2 = fma2(p2, pm, pc); x ^= (x >> 7) | 0x21u; p3 = fma2(p3, pm, pc); acc ^= (acc >> 9) | 0x201ull;
+            p4 = fma2(p4, pm, pc); x ^= (x >> 11) | 0x41u; p5 = fma2(p5, pm, pc); acc ^= (acc >> 13) | 0x401ull;
+            p6 = fma2(p6, pm, pc); x ^= (x >> 15) | 0x81u; p7 = fma2(p7, pm, pc); acc ^= (acc >> 17) | 0x801ull;
+        } else if (T == FFMA_ALU) {
+            f0 = fmaf(f0, fm, fc); x ^= (x >> 3) | 0x11u; f1 = fmaf(f1, fm, fc); acc ^= (acc >> 5) | 0x101ull;
+            f2 = fmaf(f2, fm, fc); x ^= (x >> 7) | 0x21u; f3 = fmaf(f3, fm, fc); acc ^= (acc >> 9) | 0x201ull;
+            f4 = fmaf(f4, fm, fc); x ^= (x >> 11) | 0x41u; f5 = fmaf(f5, fm, fc); acc ^= (acc >> 13) | 0x401ull;
+            f6 = fmaf(f6, fm, fc); x ^= (x >> 15) | 0x81u; f7 = fmaf(f7, fm, fc); acc ^= (acc >> 17) | 0x801ull;
+        } else if (T == FFMA2_MUFU) {
+            p0 = fma2(p0, pm, pc); p1 = fma2(p1, pm, pc); f0 = rsq(f0); p2 = fma2(p2, pm, pc); p3 = fma2(p3, pm, pc); f1 = rsq(f1);
+            p4 = fma2(p4, pm, pc); p5 = fma2(p5, pm, pc); f2 = rsq(f2); p6 = fma2(p6, pm, pc); p7 = fma2(p7, pm, pc); f3 = rsq(f3);
+        } else if (T == MUFU_ALU) {
+            f0 = rsq(f0); x ^= (x >> 3) | 0x11u; acc ^= (acc >> 5) | 0x101ull; f1 = rsq(f1); x ^= (x >> 7) | 0x21u; acc ^= (acc >> 9) | 0x201ull;
+            f2 = rsq(f2); x ^= (x >> 11) | 0x41u; acc ^= (acc >> 13) | 0x401ull; f3 = rsq(f3); x ^= (x >> 15) | 0x81u; acc ^= (acc >> 17) | 0x801ull;
         } else if (T == BOX_MIX2) {
             // 8 boxes with packed (r, s) running sums: FADD2, FFMA, MUFU, FMUL, 1/2 FMNMX3 per box
             const unsigned long long wy = ((unsigned long long)sm[(it % nb) * 64 + lane] << 32) | 0x2b8cbccbu;
@@ -335,6 +357,10 @@ int main()
     run<BOX_PACKED>(n_sm, nb, d_cyc, d_sink);
     run<BOX_PACKED_CVT>(n_sm, nb, d_cyc, d_sink);
     run<BOX_PACKED_THRESH>(n_sm, nb, d_cyc, d_sink);
+    run<FFMA2_ALU>(n_sm, nb, d_cyc, d_sink);
+    run<FFMA2_MUFU>(n_sm, nb, d_cyc, d_sink);
+    run<FFMA_ALU>(n_sm, nb, d_cyc, d_sink);
+    run<MUFU_ALU>(n_sm, nb, d_cyc, d_sink);
     run<BOX_PACKED_PAIRDIV>(n_sm, nb, d_cyc, d_sink);
     return 0;
 }
