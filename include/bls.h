@@ -96,10 +96,11 @@ typedef struct {
                                        fold warps <= 20).                                          */
 
 #define BLS_FLAG_WS_SHAPE(n) (((uint32_t)(n) & 7u) << 4) /* tuning: launch shape of the warp-specialised kernel:
-                                       1 = 20 warps at equal registers (what WARPS / FOLD_WARPS address),
-                                       2 = 8 search + 16 fold warps, 3 = 12 + 12, registers moved from the fold
-                                       to the search warps with setmaxnreg (0 = the library's choice).  Changes
-                                       which of several near-tied boxes is reported, nothing else.  */
+                                       1 = 20 warps at equal registers (what WARPS / FOLD_WARPS address; the fold
+                                       warps also merge), 2 = 8 search + 4 merge + 16 fold warps, 3 = 12 + 4 + 12,
+                                       registers moved from the other roles to the search warps with setmaxnreg
+                                       (0 = the library's choice).  Changes which of several near-tied boxes is
+                                       reported, nothing else.                                     */
 #define BLS_FLAG_MERGE_WARPS(n) (((uint32_t)(n) & 7u) << 24) /* tuning: warps per CTA that share the exact
                                        merge of a tile, 1..7 (0 = the library's choice).  Changes which of
                                        several near-tied boxes is reported, nothing else.          */

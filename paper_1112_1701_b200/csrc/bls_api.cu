@@ -122,25 +122,34 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     // Kernel 2 (warp-specialised, two bin buffers) whenever its buffers fit shared memory, with the
     // curve staged in shared memory if that fits too; otherwise kernel 1 (one buffer, two CTAs per SM).
     // Kernel 2 launch shape (WsShape in bls_search.cu): 0 = 20 warps at equal registers with a run-time split (what
-    // the WARPS / FOLD_WARPS tuning flags address); 1 = 8 search + 16 fold warps, 2 = 12 + 12, registers moved from the
-    // fold to the search warps with setmaxnreg.  Measured (clocks per pair, shapes 0 / 1 / 2): C1 651 / 624 / 600,
-    // C2 725 / 692 / 709, C3 1762 / 1666 / does not fit.  So: 12 search warps where the box search outweighs the
-    // fold (3 N <= nb nk), else 16 fold warps; whichever does not fit shared memory falls back to the next.
-    const int nk = p->kmax - p->kmin + 1;
-    int ws_shape = (3 * max_n <= (int64_t)p->nb * nk) ? 2 : 1;
+    // the WARPS / FOLD_WARPS tuning flags address), the fold warps also merge; 1 = 8 search + 4 merge + 16 fold warps,
+    // 2 = 12 search + 4 merge + 12 fold, registers moved to the search warps with setmaxnreg.  Measured (clocks per
+    // pair, shapes 0 / 1 / 2): C1 651 / 597 / 568, C2 725 / 652 / 640, C3 1762 / 1620 / does not fit.  So shape 2
+    // wherever its candidate arrays fit shared memory beside the bins, else shape 1, else shape 0.
+    int ws_shape = 2;
     if (shape_flag >= 1 && shape_flag <= kWsShapes) ws_shape = shape_flag - 1;
     if (warps_flag || fold_flag) ws_shape = 0;
     int ws_search = kWsSearchWarps, ws_fold = 0;
-    for (;; ws_shape = ws_shape == 2 ? 1 : 0) {
+    auto shape_warps = [&](int shape) {
         ws_search = kWsSearchWarps;
         if (warps_flag >= 1 && warps_flag <= kWsMaxWarps - 1) ws_search = warps_flag;
         ws_fold = kWsMaxWarps - ws_search;
         if (fold_flag >= 1 && fold_flag < ws_fold) ws_fold = fold_flag;
-        if (ws_shape > 0) {
-            const int total = ws_shape_warps(ws_shape, &ws_search);
+        if (shape > 0) {
+            const int total = ws_shape_warps(shape, &ws_search);
             ws_fold = total - ws_search;
         }
-        if (ws_shape == 0 || search_smem_bytes(p->nb, p->kmax, ws_search, 2, 0) <= optin) break;
+    };
+    {   // first the shapes that still leave room for the staged curve, then those that fit without it
+        const int first = ws_shape;
+        int pick = -1;
+        for (int with_pts = 1; with_pts >= 0 && pick < 0; --with_pts)
+            for (int sh = first; sh >= 0 && pick < 0; --sh) {
+                shape_warps(sh);
+                if (search_smem_bytes(p->nb, p->kmax, ws_search, 2, with_pts ? max_n : 0) <= optin) pick = sh;
+            }
+        ws_shape = pick < 0 ? 0 : pick;
+        shape_warps(ws_shape);
     }
     const bool ws = !(p->flags & BLS_FLAG_SINGLE_BUFFER) &&
                     search_smem_bytes(p->nb, p->kmax, ws_search, 2, 0) <= optin;
@@ -204,7 +213,7 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     if (p->flags & BLS_FLAG_FOLD_DEPTH(3)) a.fold_depth = (p->flags & BLS_FLAG_FOLD_DEPTH(2)) ? 2 : 1;
     a.search_warps = kernel == 2 ? ws_search : 0;
     // the exact merge re-walks ONE start per column (kmax rows): its widths are split over a few warps
-    a.merge_warps = kernel == 2 ? 4 : (small ? kSmallWarps : 4);
+    a.merge_warps = kernel == 2 ? 4 : (small ? kSmallWarps : 4);      // (kernel 2 shapes 1, 2: the four merge-role warps)
     if (merge_flag >= 1 && merge_flag <= kMergeWarps) a.merge_warps = merge_flag;
     a.kernel = kernel;
     a.ws_shape = kernel == 2 ? ws_shape : 0;

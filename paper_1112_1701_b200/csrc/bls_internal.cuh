@@ -72,7 +72,7 @@ struct SearchArgs {
     int fold_depth;             // kernel 2: groups of 4 points a fold warp keeps in flight (1 or 2)
     int nrows;                  // bin rows per buffer: nb + cyclic extension (search_rows_for)
     int search_warps;           // kernel 2: this many search warps (then the fold warps)
-    int ws_shape;               // kernel 2: 0 = equal registers, run-time split; 1.. = fixed splits with setmaxnreg (WsShape)
+    int ws_shape;               // kernel 2: 0 = equal registers, run-time split; 1, 2 = three roles, registers moved with setmaxnreg (WsShape)
     int merge_warps;            // warps that share the exact merge of a tile (1..kMergeWarps; they split the widths)
     int kernel;                 // 1 single buffer, 2 warp-specialised double buffer, 3 one warp per tile
     int force_canonical;        // BLS_FLAG_CANONICAL_PHASE

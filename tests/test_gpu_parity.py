@@ -112,7 +112,7 @@ def test_kernel_variants_give_identical_results():
                 bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WARPS(1) | bls.BLS_FLAG_FOLD_WARPS(2),
                 bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_FOLD_DEPTH(2), bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_FOLD_DEPTH(1)]
     variants += [bls.BLS_FLAG_WARPS(n) | bls.BLS_FLAG_SINGLE_BUFFER for n in (1, 2, 3)]   # fewer than 4 warps
-    # kernel 2's launch shapes (equal registers / registers moved to 8 or 12 search warps) and the merge's warp count
+    # kernel 2's launch shapes (equal registers / three roles with 8 or 12 search warps) and the merge's warp count
     variants += [bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WS_SHAPE(n) for n in (1, 2, 3)]
     variants += [bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WS_SHAPE(n) | bls.BLS_FLAG_MERGE_WARPS(m) for n in (1, 2, 3) for m in (1, 5)]
     variants += [bls.BLS_FLAG_MERGE_WARPS(1), bls.BLS_FLAG_SINGLE_BUFFER | bls.BLS_FLAG_MERGE_WARPS(7)]
