@@ -38,7 +38,7 @@ METRIC = "bls_point_folds_per_sec"
 UNIT = "point-folds/s"
 
 # Roofline constants, measured on B200 by paper_1112_1701_b200/microbench/issue_rates.cu
-# (profiles/r02a_microbench.md): lane-operations per clock per SM.
+# (profiles/r02b_microbench.md): lane-operations per clock per SM.
 LSU_LANE_OPS_PER_CLK_SM = 32.0       # shared wavefront pipe: conflict-free ATOMS.ADD 31.97
 XU_LANE_OPS_PER_CLK_SM = 16.0        # MUFU.RSQ 16.00: one per box
 ISSUE_LANE_INSTR_PER_CLK_SM = 128.0  # 4 schedulers x 32 lanes
@@ -371,7 +371,7 @@ def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_r
                                          "ncu --set full capture (%s) x pairs per launch" % facts.get("source")},
         "peak_def": "n_SM*f_max*N/t_min per (curve,frequency) pair, t_min = max(LSU (2N+2(nb+kmax))/32, XU nb*nk/16, "
                     "issue (5N+3.5 nb nk)/128) clk = max(%.0f, %.0f, %.0f); rates measured by microbench/issue_rates.cu "
-                    "(profiles/r02a_microbench.md); f_max=%d MHz, n_SM=%d (DESIGN.md section 7)" % (
+                    "(profiles/r02b_microbench.md); f_max=%d MHz, n_SM=%d (DESIGN.md section 7)" % (
                         pc["lsu"], pc["xu"], pc["issue"], max_hz / 1e6, n_sm),
         "clk_per_pair": clk_per_pair,
         "frac_method_floor": pc["method"] / clk_per_pair,

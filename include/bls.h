@@ -66,8 +66,8 @@ typedef struct {
     int64_t n_freq;        /* 1 <= nf <= 2^27                                                       */
     const double *freqs;   /* HOST, nf trial frequencies in cycles/day, finite, > 0; NULL = uniform */
     double f0, df;         /* used iff freqs == NULL: f_k = f0 + k*df evaluated in fp64 (R13)       */
-    int32_t n_bins;        /* nb >= 4; one bin buffer, (nb + kmax + 7) rows of 256 B plus 5 KB, must fit the
-                              227 KB of shared memory a CTA can have: nb + kmax <= 880 (nb <= 800 at
+    int32_t n_bins;        /* nb >= 4; one bin buffer, (nb + kmax) rows of 256 B plus 5 KB, must fit the
+                              227 KB of shared memory a CTA can have: nb + kmax <= 888 (nb <= 807 at
                               q_max = 0.1), else bls_plan_create returns BLS_ERR_UNSUPPORTED              */
     double q_min, q_max;   /* 0 < q_min <= q_max <= 0.5; widths kmin..kmax bins by reading R9:
                               kmin = max(1, floor(q_min*nb + 1e-9)), kmax = min(nb-1, ceil(q_max*nb - 1e-9)) */

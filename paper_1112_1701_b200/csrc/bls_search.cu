@@ -17,14 +17,18 @@
 //     edge fall back to the canonical 3-rounding fp64 rule, so bin indices equal the oracle's
 //     bit for bit (DESIGN.md "Fold / fast phase" has the error bound);
 //   * the box search ranks boxes in packed fp32 (add/fma/mul.f32x2): a thread owns TWO adjacent
-//     frequencies and S consecutive start bins; it walks the bin rows once, converting each row
-//     (one LDS.64 per plane, I2FP) as it arrives, so a row feeds 2S boxes.  Per pair of boxes:
-//     FFMA2 (n -= W/SWT), FADD2 (s += Y), FFMA2 (n^2 + n = -r(1-r)), 2 MUFU.RSQ, FMUL2, FMNMX3.
-//     Running sums are direct (no prefix differences).  Only the maximum of |s| rsqrt(r(1-r)) per
-//     group of 4 rows is tracked; the group id goes to the merge step;
-//   * the merge step (one warp, lane = frequency) re-walks the winning group in EXACT integer
-//     arithmetic, applies the canonical tie-break (reading R12) and writes SR and depth from the
-//     integer box sums (R, S) in fp64, rounded once to fp32.
+//     frequencies and S consecutive start bins (S up to 8 at 96 registers, up to 13 with the registers the
+//     other warp roles hand over); it walks the bin rows once, converting each row (one LDS.64 per plane,
+//     I2FP) as it arrives, so a row feeds 2S boxes.  Per pair of boxes: FFMA2 (n -= W/SWT), FADD2 (s += Y),
+//     FFMA2 (n^2 + n = -r(1-r)), 2 MUFU.RSQ, FMUL2, and one FMNMX3 per frequency that takes the boxes of
+//     two consecutive rows of the SAME start.  Running sums are direct (no prefix differences).  The
+//     maximum of |s| rsqrt(r(1-r)) is kept per start; the best start of the column goes to the merge step;
+//   * the merge step (lane = frequency) re-walks that ONE start in EXACT integer arithmetic (its widths
+//     split over a few warps), applies the canonical tie-break (reading R12) and writes SR and depth from
+//     the integer box sums (R, S) in fp64, rounded once to fp32;
+//   * three warp roles run concurrently on consecutive tiles (kernel 2): fold warps (zero / fold / extend
+//     tile i+1), search warps (rank the boxes of tile i), merge warps (exact merge of tile i-1); registers
+//     are moved from the fold and merge warps to the search warps with setmaxnreg.
 #include "bls_internal.cuh"
 
 namespace bls {
@@ -802,12 +806,15 @@ search_kernel(const SearchArgs a)
 }
 
 // ---- kernel 2: warp-specialised, double-buffered.  The fold is bound by the shared-memory pipe
-//      (atomics + point broadcasts), the box search by the XU pipe (one MUFU.RSQ per box): they run
-//      CONCURRENTLY on different warps.  "Search warps" rank the boxes of tile i in one bin buffer
-//      while "fold warps" merge tile i-1 out of the other buffer and then zero / fold / extend tile
-//      i+1 into it.  Hand-off: FULL[b] fold -> search is an mbarrier each search warp polls on its own,
-//      DONE[b] search -> fold a named barrier (bar.arrive by the search warps, bar.sync by the fold warps);
-//      one named barrier for the fold group.
+//      (atomics + point broadcasts), the box search by the XU pipe (one MUFU.RSQ per box), the exact
+//      merge by latency: they run CONCURRENTLY on different warps.  "Search warps" rank the boxes of
+//      tile i in one bin buffer while "fold warps" zero / fold / extend tile i+1 into the other and
+//      "merge warps" (shapes 1, 2; in shape 0 the fold warps, in front of their fold) finish tile i-1.
+//      A buffer's life: fold -> FULL[b] -> search -> DONE[b] -> merge -> FREE[b] -> fold ...
+//        FULL[b]  mbarrier: every fold thread arrives, every search warp polls on its own;
+//        DONE[b]  named barrier: bar.arrive by the search warps, bar.sync by the merging warps;
+//        FREE[b]  named barrier (shapes 1, 2): bar.arrive by the merge warps, bar.sync by the fold warps;
+//      one named barrier for the fold group and one for the merge group.
 __device__ __forceinline__ void named_sync(int id, int count)
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
@@ -833,10 +840,11 @@ __device__ __forceinline__ void mbar_arrive(uint32_t addr)
 __device__ __forceinline__ void mbar_wait(uint32_t addr, uint32_t parity)
 {
     uint32_t ok;
-    do {
+    for (;;) {
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(ok) : "r"(addr), "r"(parity), "r"(20000u) : "memory");        // suspend-time hint (ns): sleep, do not spin
-    } while (!ok);
+                     : "=r"(ok) : "r"(addr), "r"(parity), "r"(20000u) : "memory");        // suspend-time hint (ns)
+        if (ok) break;                   // (a __nanosleep between polls measured no better: C1 573 against 568)
+    }
 }
 
 // Launch shapes of kernel 2.  Shape 0: up to 20 warps at equal registers (96), the search / fold split chosen at

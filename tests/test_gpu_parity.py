@@ -155,13 +155,16 @@ def test_kernel_selection_per_configuration_and_shape_limit():
     tt, mm, ss = b.curve(0)
     r = compare_spectrum(tt, mm, ss, g["freqs"], grid.nb, g["kmin"], g["kmax"], g["sr"][0], g["a"][0], g["k"][0], g["depth"][0])
     compare_peaks(r["oracle"][1], g["peaks"][0]["freq_index"], g["peaks"][0]["sr"], 3, g_spectrum=g["sr"][0])
-    # the limit: (nb + kmax + 7) rows of 256 B plus the candidate area must fit 227 KB
+    # the limit bls.h states: (nb + kmax) rows of 256 B plus 5 KB of candidates must fit 227 KB: nb + kmax <= 888
     f = np.array([0.5, 0.6])
-    with bls.Plan(n_bins=800, q_min=0.01, q_max=0.1, freqs=f) as plan:       # 800 + 80 + 7 rows: fits
+    with bls.Plan(n_bins=800, q_min=0.01, q_max=0.1, freqs=f) as plan:       # 800 + 80 rows: fits
         assert plan.kmax == 80
-    with pytest.raises(bls.BlsError) as ei:
-        bls.Plan(n_bins=1024, q_min=0.01, q_max=0.1, freqs=f)
-    assert ei.value.code == bls.BLS_ERR_UNSUPPORTED
+    with bls.Plan(n_bins=808, q_min=0.01, q_max=0.099, freqs=f) as plan:     # 808 + 80 = 888 rows: the last that fits
+        assert plan.kmax == 80
+    for nb, qmax in ((809, 0.0988), (1024, 0.1)):                            # 809 + 80 = 889 rows; far beyond
+        with pytest.raises(bls.BlsError) as ei:
+            bls.Plan(n_bins=nb, q_min=0.01, q_max=qmax, freqs=f)
+        assert ei.value.code == bls.BLS_ERR_UNSUPPORTED
 
 
 def test_low_weight_outlier_and_boxes_holding_almost_all_the_weight():
@@ -465,11 +468,12 @@ def test_c4_4096_short_curves():
 def test_handoff_stress_bitwise_repeatable_and_kernels_agree():
     """Race check by determinism (compute-sanitizer is not available on this pool).  Bins are exact
     integers, so every output is independent of the order in which warps run; a race in the
-    warp-specialised kernel's hand-off (box search reading a buffer before its conversion finished,
-    the fold zeroing a buffer before its merge finished) would change outputs from run to run as
-    timing varies.  200 C1 curves x 625 tiles = 125,000 buffer hand-offs per run, three runs with
-    different co-resident work, all outputs bitwise equal; and the single-buffer kernel, which has
-    no hand-off at all, agrees."""
+    warp-specialised kernel's hand-offs (FULL: box search reading a buffer before its fold finished;
+    DONE: the merge reading candidates before the search posted them; FREE: the fold zeroing a buffer
+    before its merge finished) would change outputs from run to run as timing varies.  200 C1 curves x
+    625 tiles = 125,000 buffer hand-offs per run, three runs with different co-resident work, all
+    outputs bitwise equal; the other launch shapes of kernel 2 (different warp counts per role, the
+    fold warps merging themselves) and the single-buffer kernel, which has no hand-off at all, agree."""
     import torch
     import paper_1112_1701_b200 as bls
     cfg = synth.config("C1")
@@ -482,8 +486,9 @@ def test_handoff_stress_bitwise_repeatable_and_kernels_agree():
         for key in ("sr", "a", "k", "depth"):
             assert np.array_equal(g[key], ref[key]), "run %d: %s differs between identical runs" % (rep, key)
         assert np.array_equal(g["peaks"], ref["peaks"])
-    sb = run_gpu(batch, cfg["grid"], top_k=5, flags=bls.BLS_FLAG_SINGLE_BUFFER)
-    same = (sb["a"] == ref["a"]) & (sb["k"] == ref["k"])
-    assert same.mean() > 0.9999                      # the rest: exact rank ties merged in warp order
-    assert np.array_equal(sb["sr"][same], ref["sr"][same]) and np.array_equal(sb["depth"][same], ref["depth"][same])
-    np.testing.assert_allclose(sb["sr"], ref["sr"], rtol=2e-6, atol=0)
+    for flags in (bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_WS_SHAPE(1), bls.BLS_FLAG_WS_SHAPE(2)):
+        sb = run_gpu(batch, cfg["grid"], top_k=5, flags=flags)
+        same = (sb["a"] == ref["a"]) & (sb["k"] == ref["k"])
+        assert same.mean() > 0.9999                      # the rest: exact rank ties merged in warp order
+        assert np.array_equal(sb["sr"][same], ref["sr"][same]) and np.array_equal(sb["depth"][same], ref["depth"][same])
+        np.testing.assert_allclose(sb["sr"], ref["sr"], rtol=2e-6, atol=0)
