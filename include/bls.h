@@ -163,6 +163,9 @@ typedef struct {
                                        (0 = none yet)                                              */
 #define BLS_QUERY_LAST_SEARCH_LAUNCHES 12 /* search kernel launches of the last bls_run (one per chunk of
                                        curves): LAST_SEARCH_NS / this = the average launch duration */
+#define BLS_QUERY_WS_SHAPE 13       /* launch shape of the warp-specialised kernel in the last run: 0 = equal registers,
+                                       the fold warps merge; 1 = 8 search + 4 merge + 16 fold warps; 2 = 12 + 4 + 12
+                                       (-1 = another kernel ran)                                  */
 
 /* Validate cfg, copy the grid to the device, derive kmin/kmax (reading R9: outward rounding of
  * [q_min, q_max] to whole bins; "tests a range of durations") and check the shape fits.

@@ -45,7 +45,7 @@ def BLS_FLAG_WS_SHAPE(n):
     return (int(n) & 7) << 4
 (QUERY_KMIN, QUERY_KMAX, QUERY_NBINS, QUERY_NFREQ, QUERY_SCRATCH_BYTES, QUERY_LAST_LAUNCHES,
  QUERY_LAST_CANONICAL, QUERY_TILE_FREQS, QUERY_SEARCH_CTAS, QUERY_LAST_SEARCH_NS,
- QUERY_SEARCH_KERNEL, QUERY_LAST_SEARCH_LAUNCHES) = range(1, 13)
+ QUERY_SEARCH_KERNEL, QUERY_LAST_SEARCH_LAUNCHES, QUERY_WS_SHAPE) = range(1, 14)
 
 
 class BlsConfig(C.Structure):

@@ -52,6 +52,7 @@ struct bls_plan {
     int64_t last_search_ctas = 0;
     int last_tiles_per_item = 0;
     int last_kernel = 0;
+    int last_ws_shape = 0;
     cudaStream_t last_stream = nullptr;
     std::vector<cudaEvent_t> ev;    // event pairs bracketing each search launch of the last run
     size_t ev_used = 0;
@@ -212,6 +213,7 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     items = (ntiles + tiles_per_item - 1) / tiles_per_item;
     p->last_tiles_per_item = tiles_per_item;
     p->last_kernel = kernel;
+    p->last_ws_shape = kernel == 2 ? ws_shape : -1;
 
     a.pts = p->d_pts; a.offsets = p->d_offsets; a.poffsets = p->d_poffsets; a.meta = p->d_meta; a.freqs = p->d_freqs;
     a.nf = (int)nf; a.nb = p->nb; a.kmin = p->kmin; a.kmax = p->kmax;
@@ -380,6 +382,7 @@ int bls_plan_query(const bls_plan *p, int32_t what, int64_t *value)
         case BLS_QUERY_TILE_FREQS: *value = (int64_t)p->last_tiles_per_item * kTileFreqs; break;
         case BLS_QUERY_SEARCH_CTAS: *value = p->last_search_ctas; break;
         case BLS_QUERY_SEARCH_KERNEL: *value = p->last_kernel; break;
+        case BLS_QUERY_WS_SHAPE: *value = p->last_ws_shape; break;
         case BLS_QUERY_LAST_SEARCH_LAUNCHES: *value = (int64_t)(p->ev_used / 2); break;
         case BLS_QUERY_LAST_SEARCH_NS: {
             if (p->last_n_curves < 0) return BLS_ERR_ARG;

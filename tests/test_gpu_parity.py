@@ -134,6 +134,8 @@ def test_kernel_selection_per_configuration_and_shape_limit():
     from paper_1112_1701_b200 import binding as B
     dev = torch.device("cuda", 0)
     want = {"C0": 2, "C1": 2, "C2": 2, "C3": 2, "C4": 1, "T0": 2, "T1": 1, "T2": 2}
+    # kernel 2's launch shape: 12 search warps wherever their candidate arrays fit beside the bins, else 8 (C3, T2: nb = 400)
+    shape = {"C0": 2, "C1": 2, "C2": 2, "C3": 1, "C4": -1, "T0": 2, "T1": -1, "T2": 1}
     for name, kern in want.items():
         cfg = synth.config(name)
         grid = cfg["grid"]
@@ -143,6 +145,7 @@ def test_kernel_selection_per_configuration_and_shape_limit():
                      torch.from_numpy(batch.sigma).to(dev))
             torch.cuda.synchronize()
             assert plan.query(B.QUERY_SEARCH_KERNEL) == kern, name
+            assert plan.query(B.QUERY_WS_SHAPE) == shape[name], name
     # nb = 512, widths 1..52: two buffers need 2 * 571 rows * 256 B > 227 KB -> kernel 1 on its own
     rng = np.random.default_rng(31)
     n = 900
