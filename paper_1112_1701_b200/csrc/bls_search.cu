@@ -918,7 +918,7 @@ search_ws_kernel(const SearchArgs a)
             named_arrive(kBarDone0 + b, nmw ? (nsw + nmw) * 32 : nthr);   // candidates posted, done reading buffer b
         }
     } else if (nmw > 0 && warp >= nfw) {
-        // ================= merge warps (shapes 3 / 4): exact merge of tile i while the fold warps fold tile i+1 =================
+        // ================= merge warps (shapes 1 / 2): exact merge of tile i while the fold warps fold tile i+1 =================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(Shape::kFoldRegs));
         for (int it = 0; it < nt; ++it) {
             const int b = it & 1;
