@@ -495,3 +495,33 @@ def test_handoff_stress_bitwise_repeatable_and_kernels_agree():
         assert same.mean() > 0.9999                      # the rest: exact rank ties merged in warp order
         assert np.array_equal(sb["sr"][same], ref["sr"][same]) and np.array_equal(sb["depth"][same], ref["depth"][same])
         np.testing.assert_allclose(sb["sr"], ref["sr"], rtol=2e-6, atol=0)
+
+
+def test_random_shapes_and_every_launch_shape_against_the_oracle():
+    """Shapes the graded configurations do not have, each through every kernel / launch shape: bin counts that
+    do not divide over the search warps (nb = 16, 37, 101, 150, 257: some warps get one start more, some get
+    none), kmin > 1 (the search's general geometry and the merge's width split start above 1), kmax close to
+    nb/2, a ragged frequency tail, few and many points per bin.  Element by element against the oracle."""
+    import paper_1112_1701_b200 as bls
+    rng = np.random.default_rng(20241105)
+    shapes = [(16, 0.07, 0.45), (37, 0.01, 0.2), (101, 0.03, 0.12), (150, 0.02, 0.3), (257, 0.012, 0.05), (64, 0.1, 0.1)]
+    variants = [0, bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WS_SHAPE(1), bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WS_SHAPE(2),
+                bls.BLS_FLAG_NO_SMALL_CTAS | bls.BLS_FLAG_WS_SHAPE(3), bls.BLS_FLAG_SINGLE_BUFFER, bls.BLS_FLAG_WARP_PER_TILE]
+    for nb, qmin, qmax in shapes:
+        curves = []
+        for n in (int(rng.integers(20, 60)), int(rng.integers(300, 900))):
+            t = np.sort(rng.integers(0, 40, n) + rng.uniform(0, 0.3, n))
+            period, q = rng.uniform(0.6, 3.0), rng.uniform(0.03, 0.12)
+            mag = 16 + rng.normal(0, 0.02, n) + 0.08 * ((((t - 0.2) / period) % 1.0) < q)
+            curves.append((t - t[0], mag, rng.uniform(0.01, 0.03, n)))
+        b = _batch(curves)
+        grid = synth.Grid(77, 0.25, 2.1, nb, qmin, qmax)             # 77 frequencies: two tiles and a ragged tail of 13
+        for flags in variants:
+            g = run_gpu(b, grid, top_k=3, flags=flags)
+            assert (g["status"] == 0).all()
+            assert g["kmin"] >= 1 and g["kmax"] < nb
+            for c in range(b.n_curves):
+                tt, mm, ss = b.curve(c)
+                r = compare_spectrum(tt, mm, ss, g["freqs"], nb, g["kmin"], g["kmax"], g["sr"][c], g["a"][c], g["k"][c],
+                                     g["depth"][c], label="nb=%d flags=%#x curve %d" % (nb, flags, c))
+                compare_peaks(r["oracle"][1], g["peaks"][c]["freq_index"], g["peaks"][c]["sr"], 3, g_spectrum=g["sr"][c])
