@@ -403,20 +403,30 @@ __device__ __forceinline__ void search_tile(uint32_t p, int kmin, int kmax, uint
     RowI nx = ld_row(p);
     uint64_t W, Y;
     if (kmin == 1 && kmax >= S - 1) {
+        uint64_t WB, YB;
 #pragma unroll
-        for (int x = 0; x < S - 1; ++x) {                    // head: row x serves starts u <= x
+        for (int x = 0; x + 1 < S - 1; x += 2) {             // head, rows x and x+1: row x serves starts u <= x
+            const RowI ra = nx;
+            const RowI rb = ld_row(p + kRowBytes);
+            p += 2 * kRowBytes; nx = ld_row(p);
+            cvt_row(ra, W, Y);
+            cvt_row(rb, WB, YB);
+#pragma unroll
+            for (int u = 0; u <= x; ++u) box_step2(rn[u], rs[u], W, Y, WB, YB, ncw2, m0[u], m1[u]);
+            box_step(rn[x + 1], rs[x + 1], WB, YB, ncw2, m0[x + 1], m1[x + 1]);
+        }
+        if ((S - 1) & 1) {                                   // the odd last head row S-2
             const RowI cur = nx;
             p += kRowBytes; nx = ld_row(p);
             cvt_row(cur, W, Y);
 #pragma unroll
-            for (int u = 0; u <= x; ++u) box_step(rn[u], rs[u], W, Y, ncw2, m0[u], m1[u]);
+            for (int u = 0; u <= S - 2; ++u) box_step(rn[u], rs[u], W, Y, ncw2, m0[u], m1[u]);
         }
         int x = S - 1;
         for (; x + 2 <= kmax; x += 2) {                      // full rows, two at a time: every start, no checks
             const RowI ra = nx;
             const RowI rb = ld_row(p + kRowBytes);
             p += 2 * kRowBytes; nx = ld_row(p);
-            uint64_t WB, YB;
             cvt_row(ra, W, Y);
             cvt_row(rb, WB, YB);
 #pragma unroll
@@ -430,12 +440,20 @@ __device__ __forceinline__ void search_tile(uint32_t p, int kmin, int kmax, uint
             for (int u = 0; u < S; ++u) box_step(rn[u], rs[u], W, Y, ncw2, m0[u], m1[u]);
         }
 #pragma unroll
-        for (int d = 0; d < S - 1; ++d) {                    // tail: row kmax+d serves starts u > d
-            const RowI cur = nx;
-            if (d < S - 2) { p += kRowBytes; nx = ld_row(p); }
-            cvt_row(cur, W, Y);
+        for (int d = 0; d + 1 < S - 1; d += 2) {             // tail, rows kmax+d and kmax+d+1: row kmax+d serves starts u > d
+            const RowI ra = nx;
+            const RowI rb = ld_row(p + kRowBytes);
+            p += 2 * kRowBytes;
+            if (d + 2 < S - 1) nx = ld_row(p);
+            cvt_row(ra, W, Y);
+            cvt_row(rb, WB, YB);
+            box_step(rn[d + 1], rs[d + 1], W, Y, ncw2, m0[d + 1], m1[d + 1]);
 #pragma unroll
-            for (int u = d + 1; u < S; ++u) box_step(rn[u], rs[u], W, Y, ncw2, m0[u], m1[u]);
+            for (int u = d + 2; u < S; ++u) box_step2(rn[u], rs[u], W, Y, WB, YB, ncw2, m0[u], m1[u]);
+        }
+        if ((S - 1) & 1) {                                   // the odd last tail row kmax+S-2 serves start S-1
+            cvt_row(nx, W, Y);
+            box_step(rn[S - 1], rs[S - 1], W, Y, ncw2, m0[S - 1], m1[S - 1]);
         }
     } else {
         const int xend = kmax + S - 1;
