@@ -197,17 +197,23 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     int64_t items = (target_ctas + chunk - 1) / chunk;
     if (items < 1) items = 1;
     if (items > ntiles) items = ntiles;
-    {   // among a few more items per curve take the count whose last wave of CTAs is fullest (equal curves: C3 at
-        // 24.1 waves lost 3.5 % to a 25th, nearly empty wave)
+    {   // where the last wave of CTAs would be mostly empty (equal curves: C3 at 24.1 waves lost 3.5 % to a 25th),
+        // take a few more items per curve: the first count that loses less than 1 %, else the fullest
         const double per_wave = (double)p->sm_count * ctas_per_sm;
-        double best_loss = 2.0;
-        int64_t best = items;
-        for (int64_t it = items; it < items + 8 && it <= ntiles; ++it) {
+        auto tail_loss = [&](int64_t it) {
             const double w = (double)chunk * (double)it / per_wave, full = ceil(w - 1e-9);
-            const double loss = full > 0.0 ? (full - w) / full : 0.0;
-            if (loss < best_loss - 1e-3) { best_loss = loss; best = it; }
+            return full > 0.0 ? (full - w) / full : 0.0;
+        };
+        if (tail_loss(items) > 0.015) {
+            double best_loss = tail_loss(items);
+            int64_t best = items;
+            for (int64_t it = items + 1; it < items + 8 && it <= ntiles; ++it) {
+                const double loss = tail_loss(it);
+                if (loss < best_loss) { best_loss = loss; best = it; }
+                if (loss < 0.01) break;
+            }
+            items = best;
         }
-        items = best;
     }
     int tiles_per_item = (int)((ntiles + items - 1) / items);
     items = (ntiles + tiles_per_item - 1) / tiles_per_item;
