@@ -44,7 +44,7 @@ struct PeakCand {
 constexpr int kTileFreqs = 32;        // frequencies per tile = lanes of a warp
 constexpr int kMaxSearchWarps = 10;   // kernel 1 upper bound (BLS_FLAG_WARPS override); 2 CTAs x 10 warps x 96 registers fill an SM
 constexpr int kWsMaxWarps = 20;       // warp-specialised kernel: search warps + fold warps
-constexpr int kWsSearchWarps = 8;     // its default split: 8 search (two per SM sub-partition) + 12 fold; 20 warps = 5 per sub-partition leave 96 registers per thread
+constexpr int kWsSearchWarps = 8;     // launch shape 0 (equal registers): 8 search (two per SM sub-partition) + 12 fold; 20 warps = 5 per sub-partition leave 96 registers per thread
 constexpr int kSmax = 8;              // starts per start tile a search thread holds at 96 registers
 constexpr int kSmaxWide = 13;         // ... and with the registers the fold warps hand over (kernel 2, shapes 1 and 2)
 constexpr int kWsShapes = 3;          // kernel 2 launch shapes (WsShape<0..2> in bls_search.cu)
