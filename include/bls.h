@@ -47,7 +47,9 @@ typedef enum {
     BLS_ERR_BATCH = -3,       /* bad bls_batch (negative count, NULL arrays)                       */
     BLS_ERR_ARG = -4,         /* bad call argument (k out of range, topk before run)               */
     BLS_ERR_CUDA = -5,        /* a CUDA call failed (no device, out of memory, launch failure)     */
-    BLS_ERR_UNSUPPORTED = -6  /* shape the kernels cannot hold (curve too long for shared memory)  */
+    BLS_ERR_UNSUPPORTED = -6, /* shape the kernels cannot hold (curve too long for shared memory)  */
+    BLS_ERR_CAPACITY = -7     /* bls_variability_noalloc only: more stars or cells than its fixed,
+                                 built-in scratch holds (BLS_NOALLOC_MAX_STARS / _MAX_CELLS)        */
 } bls_status;
 
 /* per-curve data status written to bls_outputs.status / readable after bls_run */
@@ -302,6 +304,44 @@ typedef struct {
  * stream.  Needs no plan.  Errors: BLS_ERR_NULL / BLS_ERR_CONFIG / BLS_ERR_BATCH / BLS_ERR_CUDA. */
 int bls_variability(int32_t device, const bls_variability_config *cfg, const bls_batch *batch,
                     const int32_t *group, const bls_variability_outputs *out, void *cuda_stream);
+
+/* ---- f3 without any allocation ---------------------------------------------------------------------
+ * bls_variability needs about 40 bytes of working memory per star (a device copy of the offsets, the cell
+ * membership lists of its counting sort, the clip's keep marks) and gets it from cudaMallocAsync.  Some
+ * programs that want the pre-filter cannot allocate at the point where they call it:
+ *   - a pipeline stage inside a process that has already given all of the GPU's free memory to its own pool
+ *     (a tensor framework's caching allocator, a serving runtime): a fresh cudaMalloc there simply fails;
+ *   - a per-exposure reduction loop with a latency bound: cudaMalloc / cudaFree may stall the whole device
+ *     while they run and may fail half way through a night;
+ *   - code that is handed a stream by its host application and is forbidden to create, grow or touch any
+ *     memory pool of that application.
+ * bls_variability_noalloc is the same filter (same kernels, same order, same results bit for bit) whose
+ * working memory is one fixed array compiled into the library, so the call makes no cudaMalloc, cudaMallocAsync,
+ * cudaFree or other allocating call.  The price:
+ *   - a hard size limit: n_curves <= BLS_NOALLOC_MAX_STARS and n_groups * n_mag_bins <= BLS_NOALLOC_MAX_CELLS
+ *     (a PTF pointing has about 3,000 M-dwarfs on 11 chips; 12 chips x 80 bins = 960 cells).
+ *     Anything larger returns BLS_ERR_CAPACITY before touching the GPU; use bls_variability for it;
+ *   - BLS_NOALLOC_SCRATCH_BYTES (about 0.6 MB) of device memory is held by every GPU on which this library
+ *     is loaded, from load until the process exits, whether or not this function is ever called;
+ *   - the array is shared by every call on that GPU and still holds what the previous call left there.  The
+ *     function itself re-zeroes the one part that has to start at zero (the per-cell member counts) on the
+ *     caller's stream and overwrites the rest before reading it, so calls issued one after another on ONE
+ *     stream are safe.  Two calls that can run on the GPU at the same time (different streams without an
+ *     event between them, two host threads) write over each other's working memory and give wrong results:
+ *     the caller serialises them;
+ *   - the first call on each GPU looks up where the array lives on that GPU (one cudaGetSymbolAddress, no
+ *     allocation) and remembers it.  Make that first call during start-up, before any stream capture is
+ *     begun on the device.
+ * Inputs and outputs are passed exactly as for bls_variability (outputs left NULL are simply not written;
+ * the intermediate ones among them live in the built-in array instead).  batch->offsets (HOST) is copied into
+ * the built-in array with cudaMemcpyAsync: if it lives in pinned memory, keep it unchanged until the stream
+ * has passed the call.
+ * Errors: those of bls_variability, plus BLS_ERR_CAPACITY, plus BLS_ERR_ARG for device outside [0, 64). */
+#define BLS_NOALLOC_MAX_STARS 16384
+#define BLS_NOALLOC_MAX_CELLS 4096
+#define BLS_NOALLOC_SCRATCH_BYTES 655872
+int bls_variability_noalloc(int32_t device, const bls_variability_config *cfg, const bls_batch *batch,
+                            const int32_t *group, const bls_variability_outputs *out, void *cuda_stream);
 
 /* ---- f4: eclipse detection efficiency of a cadence (Fig. 13; used at L426) ----------
  * "The detection efficiency is the probability that at least two eclipses will be observed from an eclipsing

@@ -18,10 +18,12 @@ LIB_PATH = os.path.join(_HERE, "libbls_b200.so")
 
 EXPORTS = ["bls_plan_create", "bls_run", "bls_topk", "bls_search_host", "bls_plan_destroy",
            "bls_plan_query", "bls_strerror", "bls_plan_last_cuda_error", "bls_debug_fold_bins",
-           "bls_variability", "bls_refine", "bls_detection_efficiency", "bls_run_field"]
+           "bls_variability", "bls_refine", "bls_detection_efficiency", "bls_run_field", "bls_variability_noalloc"]
 
 BLS_OK = 0
 BLS_ERR_NULL, BLS_ERR_CONFIG, BLS_ERR_BATCH, BLS_ERR_ARG, BLS_ERR_CUDA, BLS_ERR_UNSUPPORTED = -1, -2, -3, -4, -5, -6
+BLS_ERR_CAPACITY = -7
+NOALLOC_MAX_STARS, NOALLOC_MAX_CELLS = 16384, 4096      # include/bls.h BLS_NOALLOC_MAX_*
 BLS_FLAG_NONE, BLS_FLAG_CANONICAL_PHASE, BLS_FLAG_SINGLE_BUFFER, BLS_FLAG_NO_SMALL_CTAS, BLS_FLAG_WARP_PER_TILE = 0, 1, 2, 4, 8
 
 
@@ -139,6 +141,9 @@ def lib():
         L.bls_variability.restype = C.c_int
         L.bls_variability.argtypes = [C.c_int32, C.POINTER(BlsVariabilityConfig), C.POINTER(BlsBatch), C.c_void_p,
                                       C.POINTER(BlsVariabilityOutputs), C.c_void_p]
+        L.bls_variability_noalloc.restype = C.c_int
+        L.bls_variability_noalloc.argtypes = [C.c_int32, C.POINTER(BlsVariabilityConfig), C.POINTER(BlsBatch), C.c_void_p,
+                                      C.POINTER(BlsVariabilityOutputs), C.c_void_p]
         _lib = L
     return _lib
 
@@ -187,6 +192,45 @@ def variability(offsets, t, mag, sigma, group=None, *, n_groups: int = 1, mag_lo
     if rc != BLS_OK:
         raise BlsError(rc)
     return {k: v[:n] for k, v in out.items()}
+
+
+def variability_noalloc(offsets, t, mag, sigma, group=None, *, out=None, n_groups: int = 1, mag_lo: float = 12.0,
+                        mag_bin: float = 0.1, n_mag_bins: int = 80, clip: float = 3.0, nsig: float = 2.0, max_iter: int = 5,
+                        min_members: int = 5, device: int = 0, stream: Optional[int] = None):
+    """bls_variability_noalloc: the pre-filter of `variability` for callers that may not allocate GPU memory where
+    they call it (all free memory already belongs to their own pool, a latency bound forbids cudaMalloc's stalls, or
+    the host application owns every allocation).  The library call allocates nothing: its working memory is a fixed
+    array inside the library, which limits it to NOALLOC_MAX_STARS stars and NOALLOC_MAX_CELLS cells
+    (BlsError(BLS_ERR_CAPACITY) beyond that) and means calls that overlap on the GPU corrupt each other: issue them
+    on one stream.  Make the first call on a GPU at start-up.
+
+    `out`: the dict a previous call returned (or tensors of the same names and sizes): it is written in place, so
+    a steady-state caller allocates nothing on the Python side either.  Without it the eight output tensors are made
+    here with torch, as `variability` does.  Same arguments and same results as `variability` otherwise."""
+    import torch
+    offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+    n = offsets.size - 1
+    dev = torch.device("cuda", device)
+    names = ("status", "mean_mag", "rms", "cell", "expected", "scatter", "kept", "flag")
+    if out is None:
+        i32 = lambda: torch.zeros(max(n, 1), dtype=torch.int32, device=dev)
+        f64 = lambda: torch.zeros(max(n, 1), dtype=torch.float64, device=dev)
+        out = dict(status=i32(), mean_mag=f64(), rms=f64(), cell=i32(), expected=f64(), scatter=f64(), kept=i32(), flag=i32())
+    else:
+        for k in names:
+            want = torch.float64 if k in ("mean_mag", "rms", "expected", "scatter") else torch.int32
+            assert out[k].is_cuda and out[k].dtype == want and out[k].numel() >= n and out[k].is_contiguous(), k
+    cfg = BlsVariabilityConfig(C.sizeof(BlsVariabilityConfig), int(n_groups), float(mag_lo), float(mag_bin), int(n_mag_bins),
+                               int(max_iter), float(clip), float(nsig), int(min_members), 0)
+    b = BlsBatch(n, offsets.ctypes.data, _ptr(t), _ptr(mag), _ptr(sigma), None)
+    o = BlsVariabilityOutputs(*[_ptr(out[k]) for k in names])
+    if stream is None:
+        stream = torch.cuda.current_stream(dev).cuda_stream
+    rc = lib().bls_variability_noalloc(device, C.byref(cfg), C.byref(b), C.c_void_p(_ptr(group)) if group is not None else None,
+                                       C.byref(o), C.c_void_p(stream))
+    if rc != BLS_OK:
+        raise BlsError(rc)
+    return {k: out[k][:n] for k in names}
 
 
 def debug_fold_bins(f, t, n_bins: int, flags: int = 0, device: int = 0):

@@ -290,6 +290,7 @@ const char *bls_strerror(int status)
         case BLS_ERR_ARG: return "invalid argument";
         case BLS_ERR_CUDA: return "CUDA failure (see bls_plan_last_cuda_error)";
         case BLS_ERR_UNSUPPORTED: return "shape not supported by the kernels";
+        case BLS_ERR_CAPACITY: return "batch exceeds the built-in scratch of bls_variability_noalloc (BLS_NOALLOC_MAX_STARS / BLS_NOALLOC_MAX_CELLS); use bls_variability";
         default: return "unknown status";
     }
 }

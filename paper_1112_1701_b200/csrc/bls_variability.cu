@@ -195,3 +195,103 @@ cudaError_t launch_variability(const float *t, const float *mag, const float *si
 }
 
 }  // namespace bls
+
+// ---- bls_variability_noalloc: the same filter for callers that must not allocate (include/bls.h) ------------
+// Everything bls_variability takes from cudaMallocAsync lives here instead, in one array that is part of the
+// library image: each GPU that loads the library carries its own copy (BLS_NOALLOC_SCRATCH_BYTES) until the
+// process ends.  The slots are those of bls_variability's scratch block at the fixed maximum sizes.
+#include <math.h>
+
+#include <mutex>
+
+namespace {
+
+constexpr size_t na_pad(size_t bytes) { return (bytes + 255) & ~(size_t)255; }
+constexpr size_t kNaStars = BLS_NOALLOC_MAX_STARS, kNaCells = BLS_NOALLOC_MAX_CELLS;
+constexpr size_t kNaOffsets = 0;                                          // int64 [stars + 1]  device copy of batch->offsets
+constexpr size_t kNaStatus = kNaOffsets + na_pad((kNaStars + 1) * 8);     // int32 [stars]      used when out->status is NULL
+constexpr size_t kNaCell = kNaStatus + na_pad(kNaStars * 4);              // int32 [stars]      ... out->cell
+constexpr size_t kNaMembers = kNaCell + na_pad(kNaStars * 4);             // int32 [stars]      stars sorted by (cell, index)
+constexpr size_t kNaCount = kNaMembers + na_pad(kNaStars * 4);            // int32 [cells]      members per cell: MUST START AT ZERO
+constexpr size_t kNaOffset = kNaCount + na_pad(kNaCells * 4);             // int32 [cells + 1]  exclusive scan of the counts
+constexpr size_t kNaCursor = kNaOffset + na_pad((kNaCells + 1) * 4);      // int32 [cells]      write positions of the scatter
+constexpr size_t kNaMean = kNaCursor + na_pad(kNaCells * 4);              // double [stars]     ... out->mean_mag
+constexpr size_t kNaRms = kNaMean + na_pad(kNaStars * 8);                 // double [stars]     ... out->rms
+constexpr size_t kNaKeep = kNaRms + na_pad(kNaStars * 8);                 // uint8 [stars]      clip marks, by member position
+constexpr size_t kNaBytes = kNaKeep + na_pad(kNaStars);
+static_assert(kNaBytes == BLS_NOALLOC_SCRATCH_BYTES, "bls.h states the size of the built-in scratch");
+
+constexpr int kNaMaxDevices = 64;
+std::mutex g_na_mutex;
+unsigned char *g_na_address[kNaMaxDevices];   // g_na_address[d]: where the array lives on GPU d (nullptr = not looked up yet)
+
+}  // namespace
+
+// In HOST code this name is only a handle for the runtime: it is NOT a device address and must never be handed
+// to a kernel or to cudaMemcpyAsync as a pointer.  The address on the current GPU comes from cudaGetSymbolAddress.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNaBytes];
+
+// Where the built-in array lives on `device`, which must be the current device.  The first call per GPU asks the
+// runtime (no allocation; the array came with the library image) and every later call reuses the answer.
+static cudaError_t noalloc_scratch_on(int device, unsigned char **address)
+{
+    std::lock_guard<std::mutex> lock(g_na_mutex);
+    if (!g_na_address[device]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        g_na_address[device] = (unsigned char *)p;
+    }
+    *address = g_na_address[device];
+    return cudaSuccess;
+}
+
+extern "C" {
+#pragma GCC visibility push(default)
+
+int bls_variability_noalloc(int32_t device, const bls_variability_config *cfg, const bls_batch *b, const int32_t *group,
+                            const bls_variability_outputs *out, void *cuda_stream)
+{
+    // the checks of bls_variability, in its order
+    if (!cfg || !b || !out) return BLS_ERR_NULL;
+    if (cfg->struct_size != (int32_t)sizeof(bls_variability_config)) return BLS_ERR_CONFIG;
+    if (cfg->n_groups < 1 || cfg->n_mag_bins < 1 || (int64_t)cfg->n_groups * cfg->n_mag_bins > (1 << 24)) return BLS_ERR_CONFIG;
+    if (!(cfg->mag_bin > 0.0) || !isfinite(cfg->mag_lo) || !(cfg->clip > 0.0) || !isfinite(cfg->nsig)) return BLS_ERR_CONFIG;
+    if (cfg->max_iter < 0 || cfg->max_iter > 100 || cfg->min_members < 0) return BLS_ERR_CONFIG;
+    if (b->n_curves < 0) return BLS_ERR_BATCH;
+    if (!b->offsets) return BLS_ERR_NULL;
+    if (device < 0 || device >= kNaMaxDevices) return BLS_ERR_ARG;
+    const int64_t nc = b->n_curves;
+    const int64_t n_cells = (int64_t)cfg->n_groups * cfg->n_mag_bins;
+    // the fixed capacity, before the offsets are walked and before any CUDA call
+    if (nc > (int64_t)kNaStars || n_cells > (int64_t)kNaCells) return BLS_ERR_CAPACITY;
+    if (b->offsets[0] != 0) return BLS_ERR_BATCH;
+    for (int64_t c = 0; c < nc; ++c)
+        if (b->offsets[c + 1] < b->offsets[c]) return BLS_ERR_BATCH;
+    if (b->offsets[nc] > 0 && (!b->t || !b->mag || !b->sigma)) return BLS_ERR_NULL;
+    if (nc == 0) return BLS_OK;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unsigned char *scr = nullptr;
+    if (noalloc_scratch_on(device, &scr) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    cudaError_t e = cudaMemcpyAsync(scr + kNaOffsets, b->offsets, (size_t)(nc + 1) * 8, cudaMemcpyHostToDevice, st);
+    int32_t *status = out->status ? out->status : (int32_t *)(scr + kNaStatus);
+    int32_t *cell = out->cell ? out->cell : (int32_t *)(scr + kNaCell);
+    double *mean_mag = out->mean_mag ? out->mean_mag : (double *)(scr + kNaMean);
+    double *rms = out->rms ? out->rms : (double *)(scr + kNaRms);
+    // launch_variability zeroes the member counts on `st` (cudaMemsetAsync) before the count kernel: the one slot
+    // that must not carry the previous call's contents.  Every other slot is written before it is read: status,
+    // cell, mean, rms by the per-star kernel; offset and cursor for all cells by the scan; members by the scatter;
+    // keep, over exactly the member positions in use, at the top of the clip kernel.
+    if (e == cudaSuccess)
+        e = bls::launch_variability(b->t, b->mag, b->sigma, (const int64_t *)(scr + kNaOffsets), group, nc, *cfg, status,
+                                    mean_mag, rms, cell, (int32_t *)(scr + kNaCount), (int32_t *)(scr + kNaOffset),
+                                    (int32_t *)(scr + kNaCursor), (int32_t *)(scr + kNaMembers), scr + kNaKeep,
+                                    out->expected, out->scatter, out->kept, out->flag, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    return BLS_OK;
+}
+
+#pragma GCC visibility pop
+}  // extern "C"
