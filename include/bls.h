@@ -86,13 +86,17 @@ typedef struct {
                                        does every phase, full-size CTAs) instead of the warp-specialised,
                                        double-buffered one.                                        */
 #define BLS_FLAG_NO_SMALL_CTAS 4u    /* tuning: never use the small-CTA launch shape (kernel 1 with CTAs of two
-                                       warps) that small shapes get by default.  Never changes results. */
+                                       warps) that small shapes get by default.                     */
 #define BLS_FLAG_WARP_PER_TILE 8u    /* tuning: use the one-warp-per-tile search kernel (kernel 3, warp-private
-                                       bins) where it fits.  Never changes results.                 */
+                                       bins) where it fits.                                        */
+/* What every kernel-selection flag (SINGLE_BUFFER, NO_SMALL_CTAS, WARP_PER_TILE, WARPS, FOLD_WARPS, WS_SHAPE,
+ * MERGE_WARPS) may change: which of several NEAR-TIED boxes of a frequency (fp32 ranking values within 1e-6
+ * relative of each other) is reported, because the kernels walk the boxes in different orders before the exact
+ * integer merge.  Bin contents, SR of the reported box (computed exactly from its integer sums), statuses and
+ * everything else are identical.  CANONICAL_PHASE and FOLD_DEPTH change nothing at all. */
 #define BLS_FLAG_WARPS(n) (((uint32_t)(n) & 0xffu) << 8) /* tuning: warps per CTA that walk the boxes
                                        (kernel 1: 1..10, all its warps; kernel 2: 1..19 search warps;
-                                       0 = the library's choice).  Tuning flags change which of several
-                                       near-tied boxes (|dSR| < 1e-6) is reported, nothing else.     */
+                                       0 = the library's choice).                                  */
 #define BLS_FLAG_FOLD_WARPS(n) (((uint32_t)(n) & 0xffu) << 16) /* tuning: warps per CTA that fold, in
                                        the warp-specialised kernel (0 = the library's choice; box +
                                        fold warps <= 20).                                          */
@@ -101,11 +105,9 @@ typedef struct {
                                        1 = 20 warps at equal registers (what WARPS / FOLD_WARPS address; the fold
                                        warps also merge), 2 = 8 search + 4 merge + 16 fold warps, 3 = 12 + 4 + 12,
                                        registers moved from the other roles to the search warps with setmaxnreg
-                                       (0 = the library's choice).  Changes which of several near-tied boxes is
-                                       reported, nothing else.                                     */
+                                       (0 = the library's choice).                                 */
 #define BLS_FLAG_MERGE_WARPS(n) (((uint32_t)(n) & 7u) << 24) /* tuning: warps per CTA that share the exact
-                                       merge of a tile, 1..7 (0 = the library's choice).  Changes which of
-                                       several near-tied boxes is reported, nothing else.          */
+                                       merge of a tile, 1..7 (0 = the library's choice).           */
 
 #define BLS_FLAG_FOLD_DEPTH(n) (((uint32_t)(n) & 3u) << 27) /* tuning: groups of 4 points a fold warp keeps in
                                        flight, 1 or 2 (0 = the library's choice).  Never changes results. */
@@ -183,8 +185,9 @@ int bls_plan_create(const bls_config *cfg, bls_plan **out_plan);
  * SR = s^2/(r(1-r)) (R1, R10, R11), best box per frequency with canonical ties (R12) -> per-curve peak
  * candidates (R14) kept in the plan for bls_topk / bls_refine.  `out` may be NULL (peaks only); its non-NULL
  * arrays receive the full spectra.  Enqueues on cuda_stream; synchronises it only to grow plan scratch.
- * batch->offsets and batch->t_origin are HOST arrays, read before the call returns (SURVEY 8(b) proposed
- * device pointers; host metadata lets the call validate structure without a device round trip).
+ * batch->offsets and batch->t_origin are HOST arrays, read before the call returns whether they are pageable
+ * or pinned (they are copied into plan-owned staging first; SURVEY 8(b) proposed device pointers; host metadata
+ * lets the call validate structure without a device round trip).
  * Errors: BLS_ERR_NULL, BLS_ERR_BATCH (negative count, offsets[0] != 0, decreasing offsets, a curve longer than
  * 2^25 points), BLS_ERR_UNSUPPORTED, BLS_ERR_CUDA; per-curve data faults go to status[], not to the return. */
 int bls_run(bls_plan *plan, const bls_batch *batch, const bls_outputs *out, void *cuda_stream);

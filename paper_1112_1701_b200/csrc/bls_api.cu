@@ -107,6 +107,7 @@ struct SearchLaunch {
     SearchArgs a;
     size_t smem;
     int64_t items;
+    int tiles_per_item, kernel, ws_shape;   // launch facts: bls_run stores them for BLS_QUERY_*, bls_refine does not
 };
 
 int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, SearchLaunch &L)
@@ -217,9 +218,9 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     }
     int tiles_per_item = (int)((ntiles + items - 1) / items);
     items = (ntiles + tiles_per_item - 1) / tiles_per_item;
-    p->last_tiles_per_item = tiles_per_item;
-    p->last_kernel = kernel;
-    p->last_ws_shape = kernel == 2 ? ws_shape : -1;
+    L.tiles_per_item = tiles_per_item;
+    L.kernel = kernel;
+    L.ws_shape = kernel == 2 ? ws_shape : -1;
 
     a.pts = p->d_pts; a.offsets = p->d_offsets; a.poffsets = p->d_poffsets; a.meta = p->d_meta; a.freqs = p->d_freqs;
     a.nf = (int)nf; a.nb = p->nb; a.kmin = p->kmin; a.kmax = p->kmax;
@@ -263,6 +264,21 @@ int grow_spectrum_scratch(bls_plan *p, int64_t entries, cudaStream_t st)
     p->cap_entries = entries;
     p->bytes_owned += entries * 12;
     return BLS_OK;
+}
+
+// Enqueue a host -> device copy of a caller's HOST array so that the array has been read when this returns, whatever
+// memory it lives in: cudaMemcpyAsync straight from a pinned array reads it only when the stream gets there, so the
+// bytes go through a private pageable block first (a copy out of pageable memory returns once the driver holds the
+// bytes in its own staging buffer), which is freed at once.
+cudaError_t copy_host_array_now(void *dst, const void *src, size_t bytes, cudaStream_t st)
+{
+    if (bytes == 0) return cudaSuccess;
+    void *tmp = malloc(bytes);
+    if (!tmp) return cudaErrorMemoryAllocation;
+    memcpy(tmp, src, bytes);
+    const cudaError_t e = cudaMemcpyAsync(dst, tmp, bytes, cudaMemcpyHostToDevice, st);
+    free(tmp);
+    return e;
 }
 
 void widths_from_q(int nb, double qmin, double qmax, int *kmin, int *kmax)
@@ -430,15 +446,26 @@ int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_ou
 {
     const bool field = field_epochs > 0;
     const int64_t nc = b->n_curves;
+    // Host staging owned by the plan, three arrays of nc + 1 entries: [prepared offsets | the caller's offsets | the
+    // caller's origins].  The caller's HOST arrays are copied here before anything is enqueued, so they are "read
+    // before the call returns" (bls.h) even when they live in pinned memory, where cudaMemcpyAsync straight from the
+    // caller's pointer would read them only when the stream gets there.  This block is ordinary pageable memory: a
+    // cudaMemcpyAsync from it returns once its contents are in the driver's own staging buffer, so the next run may
+    // overwrite it.
     if (nc + 1 > p->cap_hpoff) {
         free(p->h_poffsets);
-        p->h_poffsets = (int64_t *)malloc((size_t)(nc + 1) * sizeof(int64_t));
+        p->h_poffsets = (int64_t *)malloc((size_t)(nc + 1) * 3 * sizeof(int64_t));
         p->cap_hpoff = p->h_poffsets ? nc + 1 : 0;
         if (!p->h_poffsets) return BLS_ERR_CUDA;
     }
+    int64_t *const h_offsets = p->h_poffsets + p->cap_hpoff;
+    double *const h_origin = (double *)(p->h_poffsets + 2 * p->cap_hpoff);
+    if (!field) memcpy(h_offsets, b->offsets, (size_t)(nc + 1) * sizeof(int64_t));
+    if (b->t_origin)
+        for (int64_t c = 0; c < nc; ++c) h_origin[c] = field ? b->t_origin[0] : b->t_origin[c];
     int64_t max_n = 0, nrec = 0;
     for (int64_t c = 0; c < nc; ++c) {
-        const int64_t n = field ? field_epochs : b->offsets[c + 1] - b->offsets[c];
+        const int64_t n = field ? field_epochs : h_offsets[c + 1] - h_offsets[c];
         if (n < 0 || n > 2147483647LL / 64) return BLS_ERR_BATCH;
         if (n > max_n) max_n = n;
         p->h_poffsets[c] = nrec;
@@ -446,7 +473,7 @@ int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_ou
     }
     p->h_poffsets[nc] = nrec;
     max_n = (max_n + 3) & ~(int64_t)3;                      // records per curve, padded
-    const int64_t npts = field ? nc * field_epochs : b->offsets[nc];
+    const int64_t npts = field ? nc * field_epochs : h_offsets[nc];
     if (npts > 0 && (!b->t || !b->mag || !b->sigma)) return BLS_ERR_NULL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     BLS_CUDA(p, cudaSetDevice(p->device));
@@ -482,21 +509,15 @@ int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_ou
     if (chunk > nc) chunk = nc;
     if ((rc = grow_spectrum_scratch(p, chunk * p->nf, st)) != BLS_OK) return rc;
 
-    // ---- metadata to the device (stream ordered; the caller keeps offsets alive until then) ------
+    // ---- metadata to the device, from the plan's staging block -----------------------------------
     if (!field)
-        BLS_CUDA(p, cudaMemcpyAsync(p->d_offsets, b->offsets, (size_t)(nc + 1) * sizeof(int64_t),
+        BLS_CUDA(p, cudaMemcpyAsync(p->d_offsets, h_offsets, (size_t)(nc + 1) * sizeof(int64_t),
                                     cudaMemcpyHostToDevice, st));
     BLS_CUDA(p, cudaMemcpyAsync(p->d_poffsets, p->h_poffsets, (size_t)(nc + 1) * sizeof(int64_t),
                                 cudaMemcpyHostToDevice, st));
     p->last_has_origin = b->t_origin != nullptr;
-    if (b->t_origin && !field)
-        BLS_CUDA(p, cudaMemcpyAsync(p->d_origin, b->t_origin, (size_t)nc * sizeof(double),
-                                    cudaMemcpyHostToDevice, st));
-    if (b->t_origin && field) {                 // one origin for the whole field: replicated through the staging buffer
-        for (int64_t c = 0; c < nc; ++c) memcpy(&p->h_poffsets[c], b->t_origin, sizeof(double));
-        BLS_CUDA(p, cudaMemcpyAsync(p->d_origin, p->h_poffsets, (size_t)nc * sizeof(double), cudaMemcpyHostToDevice, st));
-        BLS_CUDA(p, cudaStreamSynchronize(st));  // the staging buffer is reused by the next run
-    }
+    if (b->t_origin)                            // (a field's one origin was replicated per star above)
+        BLS_CUDA(p, cudaMemcpyAsync(p->d_origin, h_origin, (size_t)nc * sizeof(double), cudaMemcpyHostToDevice, st));
     BLS_CUDA(p, cudaMemsetAsync(p->d_canon, 0, sizeof(unsigned long long), st));
 
     // ---- a0 prep -------------------------------------------------------------------------------
@@ -515,6 +536,9 @@ int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_ou
     a.u_width = out ? out->best_width : nullptr;
     a.u_depth = out ? out->depth : nullptr;
     p->last_max_n = max_n;
+    p->last_tiles_per_item = L.tiles_per_item;
+    p->last_kernel = L.kernel;
+    p->last_ws_shape = L.ws_shape;
 
     // ---- per chunk of curves: search -> peak candidates ------------------------------------------
     p->last_search_ctas = 0;
@@ -612,7 +636,7 @@ int bls_variability(int32_t device, const bls_variability_config *cfg, const bls
     const size_t o_keep = take((size_t)nc);
     unsigned char *scr = nullptr;
     if (cudaMallocAsync((void **)&scr, off, st) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
-    cudaError_t e = cudaMemcpyAsync(scr + o_offsets, b->offsets, (size_t)(nc + 1) * 8, cudaMemcpyHostToDevice, st);
+    cudaError_t e = copy_host_array_now(scr + o_offsets, b->offsets, (size_t)(nc + 1) * 8, st);
     int32_t *status = out->status ? out->status : (int32_t *)(scr + o_status);
     int32_t *cell = out->cell ? out->cell : (int32_t *)(scr + o_cell);
     double *mean_mag = out->mean_mag ? out->mean_mag : (double *)(scr + o_mean);
@@ -647,11 +671,12 @@ int bls_detection_efficiency(int32_t device, const bls_batch *b, int64_t n_freq,
     size_t off = 0;
     auto take = [&off](size_t bytes) { const size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
     const size_t o_off = take((size_t)(nc + 1) * 8), o_f = take((size_t)n_freq * 8);
-    const size_t o_cnt = take((size_t)(nc * n_freq) * 4), o_eff = take((size_t)(nc * n_freq) * 8);
+    // the kernel writes both results; the one the caller does not want goes to scratch (none if both are wanted)
+    const size_t o_cnt = count ? 0 : take((size_t)(nc * n_freq) * 4), o_eff = efficiency ? 0 : take((size_t)(nc * n_freq) * 8);
     unsigned char *scr = nullptr;
     if (cudaMallocAsync((void **)&scr, off, st) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
-    cudaError_t e = cudaMemcpyAsync(scr + o_off, b->offsets, (size_t)(nc + 1) * 8, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(scr + o_f, freqs, (size_t)n_freq * 8, cudaMemcpyHostToDevice, st);
+    cudaError_t e = copy_host_array_now(scr + o_off, b->offsets, (size_t)(nc + 1) * 8, st);
+    if (e == cudaSuccess) e = copy_host_array_now(scr + o_f, freqs, (size_t)n_freq * 8, st);
     if (e == cudaSuccess)
         e = launch_window(b->t, (const int64_t *)(scr + o_off), nc, (int)n_freq, (const double *)(scr + o_f), duration, n_phase,
                           min_events, count ? count : (int32_t *)(scr + o_cnt), efficiency ? efficiency : (double *)(scr + o_eff), st);

@@ -220,6 +220,38 @@ def test_chunked_scratch_gives_identical_results():
     assert np.array_equal(g1["peaks"], g2["peaks"])
 
 
+def test_host_metadata_is_read_before_bls_run_returns_even_from_pinned_memory():
+    """bls.h: batch->offsets and batch->t_origin are HOST arrays "read before the call returns".  From pinned
+    memory a cudaMemcpyAsync straight out of the caller's arrays would read them only when the stream gets there;
+    here the stream is kept busy, the call is made on pinned arrays, and they are overwritten the moment it
+    returns.  The results must be those of an undisturbed run."""
+    import torch
+    import paper_1112_1701_b200 as bls
+    cfg = synth.config("T0")
+    batch, grid = synth.make_batch(cfg), cfg["grid"]
+    freqs = synth.freq_grid(grid)
+    want = run_gpu(batch, grid, top_k=5)
+    dev = torch.device("cuda", 0)
+    d = [torch.from_numpy(x).to(dev) for x in (batch.t, batch.mag, batch.sigma)]
+    nc, nf = batch.n_curves, len(freqs)
+    offs = torch.from_numpy(batch.offsets.astype(np.int64)).pin_memory()
+    orig = torch.from_numpy(np.asarray(batch.t_origin, dtype=np.float64)).pin_memory()
+    assert offs.is_pinned() and orig.is_pinned()
+    with bls.Plan(n_bins=grid.nb, q_min=grid.qmin, q_max=grid.qmax, freqs=freqs, max_top_k=5) as plan:
+        sr = torch.empty((nc, nf), dtype=torch.float32, device=dev)
+        plan.run(batch.offsets, d[0], d[1], d[2], batch.t_origin, sr=sr)      # scratch grows here, not below
+        torch.cuda.synchronize()
+        sr.fill_(-1.0)
+        torch.cuda._sleep(int(1e9))                                             # ~0.5 s of busy stream
+        plan.run(offs.numpy(), d[0], d[1], d[2], orig.numpy(), sr=sr)
+        offs.fill_(0)                                                           # the caller reuses its arrays at once
+        orig.fill_(-1.0)
+        peaks = plan.peaks_to_numpy(plan.topk(5), 5)
+        torch.cuda.synchronize()
+    assert np.array_equal(sr.cpu().numpy(), want["sr"])
+    assert np.array_equal(peaks, want["peaks"])                                 # epochs carry t_origin
+
+
 def test_canonical_phase_flag_gives_identical_results():
     import paper_1112_1701_b200 as bls
     cfg = synth.config("T2")

@@ -150,3 +150,34 @@ def test_refine_argument_errors():
             with pytest.raises(bls.BlsError):
                 plan.refine(**bad)
         assert plan.refine(2, 8, 2).shape == (batch.n_curves, 2)
+
+
+def test_refine_in_several_chunks_is_bitwise_identical_and_leaves_the_run_queries_alone():
+    """bls_refine's fine spectrum reuses the plan's spectrum scratch in chunks of curves; with the default 2 GiB
+    budget one chunk holds every tested batch, so the loop over chunks (chunk-local rows of the fine spectrum,
+    global candidate / output indices) is forced here with a budget of two curves' fine spectra: 6 curves -> 3
+    chunks.  Records must equal the one-chunk run bit for bit.  Also: BLS_QUERY_SEARCH_KERNEL / WS_SHAPE /
+    TILE_FREQS describe the last bls_run, whatever bls_refine launched after it."""
+    import torch
+    import paper_1112_1701_b200 as bls
+    B = bls.binding
+    cfg = synth.config("T0")
+    batch, grid = synth.make_batch(cfg), cfg["grid"]
+    freqs = synth.freq_grid(grid)
+    k, n_fine, n_shift = 3, 16, 2
+    dev = torch.device("cuda", 0)
+    d = [torch.from_numpy(x).to(dev) for x in (batch.t, batch.mag, batch.sigma)]
+    recs, facts = [], []
+    for scratch in (0, 2 * k * n_fine * n_shift * 12):
+        with bls.Plan(n_bins=grid.nb, q_min=grid.qmin, q_max=grid.qmax, freqs=freqs, max_top_k=k, scratch_bytes=scratch) as plan:
+            plan.run(batch.offsets, d[0], d[1], d[2], batch.t_origin)
+            before = [plan.query(q) for q in (B.QUERY_SEARCH_KERNEL, B.QUERY_WS_SHAPE, B.QUERY_TILE_FREQS)]
+            launches = plan.query(B.QUERY_LAST_LAUNCHES)
+            recs.append(plan.refine(k, n_fine, n_shift))
+            after = [plan.query(q) for q in (B.QUERY_SEARCH_KERNEL, B.QUERY_WS_SHAPE, B.QUERY_TILE_FREQS)]
+            assert before == after
+            facts.append(plan.query(B.QUERY_LAST_LAUNCHES) - launches)
+    assert recs[0].tobytes() == recs[1].tobytes()
+    assert (recs[0]["fine_index"] >= 0).sum() >= batch.n_curves            # something was refined
+    # one grid kernel + (search + reduce) per chunk: 1 chunk vs 3 chunks
+    assert facts == [3, 7], facts

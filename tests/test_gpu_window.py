@@ -57,3 +57,30 @@ def test_argument_errors():
         assert ei.value.code == bls.BLS_ERR_ARG
     with pytest.raises(bls.BlsError):
         bls.detection_efficiency(offs, t, [-1.0], 0.1)
+
+
+def test_either_output_may_be_left_out():
+    """count / efficiency NULL = "do not write": the call then keeps that result in its own scratch (and takes no
+    scratch for a result the caller does hold).  What is written must equal the both-outputs call."""
+    import ctypes as C
+    import torch
+    import paper_1112_1701_b200 as bls
+    B = bls.binding
+    cfg = synth.config("C4")
+    curves = [synth.make_curve(cfg, c)[0] for c in range(3)]
+    offs = np.zeros(4, dtype=np.int64)
+    offs[1:] = np.cumsum([len(c) for c in curves])
+    t = torch.from_numpy(np.concatenate(curves).astype(np.float32)).cuda()
+    freqs = np.ascontiguousarray(1.0 / np.linspace(0.3, 2.5, 37))
+    cnt0, eff0 = bls.detection_efficiency(offs, t, freqs, 0.05, 200)
+    torch.cuda.synchronize()
+    b = B.BlsBatch(3, offs.ctypes.data, t.data_ptr(), None, None, None)
+    st = C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    cnt = torch.full((3, 37), -1, dtype=torch.int32, device="cuda")
+    eff = torch.full((3, 37), -1.0, dtype=torch.float64, device="cuda")
+    L = bls.lib()
+    assert L.bls_detection_efficiency(0, C.byref(b), 37, C.c_void_p(freqs.ctypes.data), 0.05, 200, 2, C.c_void_p(cnt.data_ptr()), None, st) == 0
+    assert L.bls_detection_efficiency(0, C.byref(b), 37, C.c_void_p(freqs.ctypes.data), 0.05, 200, 2, None, C.c_void_p(eff.data_ptr()), st) == 0
+    assert L.bls_detection_efficiency(0, C.byref(b), 37, C.c_void_p(freqs.ctypes.data), 0.05, 200, 2, None, None, st) == 0
+    torch.cuda.synchronize()
+    assert torch.equal(cnt, cnt0) and torch.equal(eff, eff0) and int(cnt0.sum()) > 0
