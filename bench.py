@@ -37,7 +37,7 @@ import synth  # noqa: E402
 METRIC = "bls_point_folds_per_sec"
 UNIT = "point-folds/s"
 
-# Roofline constants, measured on B200 by paper_1112_1701_b200/microbench/issue_rates.cu
+# Roofline constants, measured on B200 by microbench/issue_rates.cu
 # (profiles/r02b_microbench.md): lane-operations per clock per SM.
 LSU_LANE_OPS_PER_CLK_SM = 32.0       # shared wavefront pipe: conflict-free ATOMS.ADD 31.97
 XU_LANE_OPS_PER_CLK_SM = 16.0        # MUFU.RSQ 16.00: one per box
@@ -367,7 +367,7 @@ def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_r
         "traffic": (bpp * pairs_per_launch) if bpp else None,
         "per_launch": {"launches_per_step": search_launches / steps, "avg_launch_ms": 1e3 * search_s * steps / max(search_launches, 1),
                        "point_folds": pf_per_step * steps / max(search_launches, 1),
-                       "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum per (curve, frequency) pair of the "
+                       "traffic_is_from_committed_ncu_capture_not_this_run": "dram__bytes_read.sum + dram__bytes_write.sum per (curve, frequency) pair of the "
                                          "ncu --set full capture (%s) x pairs per launch" % facts.get("source")},
         "peak_def": "n_SM*f_max*N/t_min per (curve,frequency) pair, t_min = max(LSU (2N+2(nb+kmax))/32, XU nb*nk/16, "
                     "issue (5N+3.5 nb nk)/128) clk = max(%.0f, %.0f, %.0f); rates measured by microbench/issue_rates.cu "

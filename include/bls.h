@@ -82,36 +82,6 @@ typedef struct {
 #define BLS_FLAG_CANONICAL_PHASE 1u /* compute every bin index with the slow 3-rounding fp64 rule
                                        (R8) instead of the guarded fast path; results identical   */
 
-#define BLS_FLAG_SINGLE_BUFFER 2u    /* tuning: always use the single-buffer search kernel (every warp
-                                       does every phase, full-size CTAs) instead of the warp-specialised,
-                                       double-buffered one.                                        */
-#define BLS_FLAG_NO_SMALL_CTAS 4u    /* tuning: never use the small-CTA launch shape (kernel 1 with CTAs of two
-                                       warps) that small shapes get by default.                     */
-#define BLS_FLAG_WARP_PER_TILE 8u    /* tuning: use the one-warp-per-tile search kernel (kernel 3, warp-private
-                                       bins) where it fits.                                        */
-/* What every kernel-selection flag (SINGLE_BUFFER, NO_SMALL_CTAS, WARP_PER_TILE, WARPS, FOLD_WARPS, WS_SHAPE,
- * MERGE_WARPS) may change: which of several NEAR-TIED boxes of a frequency (fp32 ranking values within 1e-6
- * relative of each other) is reported, because the kernels walk the boxes in different orders before the exact
- * integer merge.  Bin contents, SR of the reported box (computed exactly from its integer sums), statuses and
- * everything else are identical.  CANONICAL_PHASE and FOLD_DEPTH change nothing at all. */
-#define BLS_FLAG_WARPS(n) (((uint32_t)(n) & 0xffu) << 8) /* tuning: warps per CTA that walk the boxes
-                                       (kernel 1: 1..10, all its warps; kernel 2: 1..19 search warps;
-                                       0 = the library's choice).                                  */
-#define BLS_FLAG_FOLD_WARPS(n) (((uint32_t)(n) & 0xffu) << 16) /* tuning: warps per CTA that fold, in
-                                       the warp-specialised kernel (0 = the library's choice; box +
-                                       fold warps <= 20).                                          */
-
-#define BLS_FLAG_WS_SHAPE(n) (((uint32_t)(n) & 7u) << 4) /* tuning: launch shape of the warp-specialised kernel:
-                                       1 = 20 warps at equal registers (what WARPS / FOLD_WARPS address; the fold
-                                       warps also merge), 2 = 8 search + 4 merge + 16 fold warps, 3 = 12 + 4 + 12,
-                                       registers moved from the other roles to the search warps with setmaxnreg
-                                       (0 = the library's choice).                                 */
-#define BLS_FLAG_MERGE_WARPS(n) (((uint32_t)(n) & 7u) << 24) /* tuning: warps per CTA that share the exact
-                                       merge of a tile, 1..7 (0 = the library's choice).           */
-
-#define BLS_FLAG_FOLD_DEPTH(n) (((uint32_t)(n) & 3u) << 27) /* tuning: groups of 4 points a fold warp keeps in
-                                       flight, 1 or 2 (0 = the library's choice).  Never changes results. */
-
 /* Ragged CSR batch of light curves (per star a list of HJD times, calibrated
  * magnitudes and errors).  Curve c owns points [offsets[c], offsets[c+1]). */
 typedef struct {
@@ -153,23 +123,6 @@ typedef struct {
 #define BLS_QUERY_NBINS 3
 #define BLS_QUERY_NFREQ 4
 #define BLS_QUERY_SCRATCH_BYTES 5   /* device bytes currently owned by the plan                    */
-#define BLS_QUERY_LAST_LAUNCHES 6   /* kernels launched by the last bls_run + bls_topk            */
-#define BLS_QUERY_LAST_CANONICAL 7  /* point-folds of the last bls_run that took the canonical
-                                       fp64 bin rule because the fast phase fell in its guard band
-                                       (synchronises the stream of that run)                       */
-#define BLS_QUERY_TILE_FREQS 8      /* frequencies per CTA work item in the search kernel          */
-#define BLS_QUERY_SEARCH_CTAS 9     /* CTAs of the last search launch                              */
-#define BLS_QUERY_LAST_SEARCH_NS 10 /* device time (ns, CUDA events on the run's stream) the search
-                                       kernel launches of the last bls_run took (synchronises)    */
-#define BLS_QUERY_SEARCH_KERNEL 11  /* search kernel of the last run: 1 = single buffer (all warps do every
-                                       phase; also the small-CTA shape of small configurations),
-                                       2 = warp-specialised double buffer, 3 = one warp per tile
-                                       (0 = none yet)                                              */
-#define BLS_QUERY_LAST_SEARCH_LAUNCHES 12 /* search kernel launches of the last bls_run (one per chunk of
-                                       curves): LAST_SEARCH_NS / this = the average launch duration */
-#define BLS_QUERY_WS_SHAPE 13       /* launch shape of the warp-specialised kernel in the last run: 0 = equal registers,
-                                       the fold warps merge; 1 = 8 search + 4 merge + 16 fold warps; 2 = 12 + 4 + 12
-                                       (-1 = another kernel ran)                                  */
 
 /* Validate cfg, copy the grid to the device, derive kmin/kmax (reading R9: outward rounding of
  * [q_min, q_max] to whole bins; "tests a range of durations") and check the shape fits.
@@ -361,6 +314,59 @@ int bls_variability_noalloc(int32_t device, const bls_variability_config *cfg, c
 int bls_detection_efficiency(int32_t device, const bls_batch *batch, int64_t n_freq, const double *freqs,
                              double duration, int32_t n_phase, int32_t min_events, int32_t *count,
                              double *efficiency, void *cuda_stream);
+
+/* ==== UNSTABLE: development switches and launch introspection, for tests, profiling and bench.py ========
+ * Nothing below is part of the supported interface: values, meanings and existence may change with the
+ * kernels.  A caller that only wants periodograms needs none of it (flags = BLS_FLAG_NONE or
+ * BLS_FLAG_CANONICAL_PHASE; queries 1-5). */
+#define BLS_FLAG_SINGLE_BUFFER 2u    /* tuning: always use the single-buffer search kernel (every warp
+                                       does every phase, full-size CTAs) instead of the warp-specialised,
+                                       double-buffered one.                                        */
+#define BLS_FLAG_NO_SMALL_CTAS 4u    /* tuning: never use the small-CTA launch shape (kernel 1 with CTAs of two
+                                       warps) that small shapes get by default.                     */
+#define BLS_FLAG_WARP_PER_TILE 8u    /* tuning: use the one-warp-per-tile search kernel (kernel 3, warp-private
+                                       bins) where it fits.                                        */
+/* What every kernel-selection flag (SINGLE_BUFFER, NO_SMALL_CTAS, WARP_PER_TILE, WARPS, FOLD_WARPS, WS_SHAPE,
+ * MERGE_WARPS) may change: which of several NEAR-TIED boxes of a frequency (fp32 ranking values within 1e-6
+ * relative of each other) is reported, because the kernels walk the boxes in different orders before the exact
+ * integer merge.  Bin contents, SR of the reported box (computed exactly from its integer sums), statuses and
+ * everything else are identical.  CANONICAL_PHASE and FOLD_DEPTH change nothing at all. */
+#define BLS_FLAG_WARPS(n) (((uint32_t)(n) & 0xffu) << 8) /* tuning: warps per CTA that walk the boxes
+                                       (kernel 1: 1..10, all its warps; kernel 2: 1..19 search warps;
+                                       0 = the library's choice).                                  */
+#define BLS_FLAG_FOLD_WARPS(n) (((uint32_t)(n) & 0xffu) << 16) /* tuning: warps per CTA that fold, in
+                                       the warp-specialised kernel (0 = the library's choice; box +
+                                       fold warps <= 20).                                          */
+
+#define BLS_FLAG_WS_SHAPE(n) (((uint32_t)(n) & 7u) << 4) /* tuning: launch shape of the warp-specialised kernel:
+                                       1 = 20 warps at equal registers (what WARPS / FOLD_WARPS address; the fold
+                                       warps also merge), 2 = 8 search + 4 merge + 16 fold warps, 3 = 12 + 4 + 12,
+                                       registers moved from the other roles to the search warps with setmaxnreg
+                                       (0 = the library's choice).                                 */
+#define BLS_FLAG_MERGE_WARPS(n) (((uint32_t)(n) & 7u) << 24) /* tuning: warps per CTA that share the exact
+                                       merge of a tile, 1..7 (0 = the library's choice).           */
+
+#define BLS_FLAG_FOLD_DEPTH(n) (((uint32_t)(n) & 3u) << 27) /* tuning: groups of 4 points a fold warp keeps in
+                                       flight, 1 or 2 (0 = the library's choice).  Never changes results. */
+
+#define BLS_QUERY_LAST_LAUNCHES 6   /* kernels launched by the last bls_run + bls_topk            */
+#define BLS_QUERY_LAST_CANONICAL 7  /* point-folds of the last bls_run that took the canonical
+                                       fp64 bin rule because the fast phase fell in its guard band
+                                       (synchronises the stream of that run)                       */
+#define BLS_QUERY_TILE_FREQS 8      /* frequencies per CTA work item in the search kernel          */
+#define BLS_QUERY_SEARCH_CTAS 9     /* CTAs of the last search launch                              */
+#define BLS_QUERY_LAST_SEARCH_NS 10 /* device time (ns, CUDA events on the run's stream) the search
+                                       kernel launches of the last bls_run took (synchronises)    */
+#define BLS_QUERY_SEARCH_KERNEL 11  /* search kernel of the last run: 1 = single buffer (all warps do every
+                                       phase; also the small-CTA shape of small configurations),
+                                       2 = warp-specialised double buffer, 3 = one warp per tile
+                                       (0 = none yet)                                              */
+#define BLS_QUERY_LAST_SEARCH_LAUNCHES 12 /* search kernel launches of the last bls_run (one per chunk of
+                                       curves): LAST_SEARCH_NS / this = the average launch duration */
+#define BLS_QUERY_WS_SHAPE 13       /* launch shape of the warp-specialised kernel in the last run: 0 = equal registers,
+                                       the fold warps merge; 1 = 8 search + 4 merge + 16 fold warps; 2 = 12 + 4 + 12
+                                       (-1 = another kernel ran)                                  */
+/* ==== end of the unstable block ==================================================================== */
 
 /* NULL is a no-op. */
 int bls_plan_destroy(bls_plan *plan);
