@@ -15,7 +15,7 @@ configuration whose 20 timed steps fit the driver's bench arm.  Prints ONE JSON 
   roofline     the search kernel against the issue-rate roofline stated in DESIGN.md section 7
   cpu_baseline the oracle as it stands on the host cores, bounded sample, and the parity of the timed
                step's peaks against it
-  per_config   C1, C3 (full) and C4 (full): one timed step each (after warm-up), same fields in short
+  per_config   C0, C1, C3 (full) and C4 (full): one timed step each (after warm-up), same fields in short
 With --impl reference the oracle itself is the timed arm (rank 0 only).
 """
 from __future__ import annotations
@@ -404,7 +404,7 @@ def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_r
     return out
 
 
-PER_CONFIG = [("C1", 0), ("C3", 100), ("C4", 20000)]     # (name, curves of the warm-up prefix; 0 = whole batch)
+PER_CONFIG = [("C0", 0), ("C1", 0), ("C3", 100), ("C4", 20000)]     # (name, curves of the warm-up prefix; 0 = whole batch)
 
 
 def short(r):
@@ -413,7 +413,8 @@ def short(r):
     return {"workload": r["config"]["workload"], "steps": r["steps"], "ms_per_step": r["ms_per_step"],
             "point_folds_per_sec": r["value"], "curves_per_sec": r["curves_per_sec"], "kernel": rf.get("kernel"),
             "clk_per_pair": rf.get("clk_per_pair"), "roofline_frac": rf.get("frac"),
-            "frac_method_floor": rf.get("frac_method_floor"), "kernel_share_of_step": rf.get("kernel_share_of_step"),
+            "frac_method_floor": rf.get("frac_method_floor"), "frac_of_fold_stage_peak": rf.get("frac_of_fold_stage_peak"),
+            "kernel_share_of_step": rf.get("kernel_share_of_step"),
             "clocks": r["clocks"], "generation_s": r["config"]["generation_s"], "refine_top_k": r.get("refine")}
 
 
@@ -427,7 +428,7 @@ def main():
     ap.add_argument("--max-curves", type=int, default=0, help="run only a prefix of the configuration")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (C1, C3, C4)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (C0, C1, C3, C4)")
     ap.add_argument("--flags", type=lambda v: int(v, 0), default=0, help="bls_config.flags (tuning only)")
     args = ap.parse_args()
 

@@ -188,6 +188,13 @@ int bls_search_host(bls_plan *plan, const bls_batch *host_batch, int32_t k, bls_
 int bls_debug_fold_bins(int32_t device, const double *f, const double *t, int64_t n, int32_t n_bins,
                         uint32_t flags, int32_t *bins, int64_t *n_canonical);
 
+/* Diagnostic, the same for the SHIFTED bin grids of bls_refine (reading S3): the grid starts at phase
+ * h / (n_shift * n_bins) cycles, 0 <= h < n_shift <= 8, and the fold uses the additive constant and the wider guard
+ * band (2 nb + 8 units) it uses inside bls_refine -- also for h = 0.  bins[i] must equal the oracle's
+ * oracle_bin_shift(f[i], t[i], n_bins, h / (n_shift * n_bins)).  Arguments and errors as above. */
+int bls_debug_fold_bins_shift(int32_t device, const double *f, const double *t, int64_t n, int32_t n_bins, int32_t h,
+                              int32_t n_shift, uint32_t flags, int32_t *bins, int64_t *n_canonical);
+
 /* ---- f1: peak significance and refinement ("high-confidence"
  * candidates; readings S1-S4 of DESIGN.md section 3) ------------------------------------------------
  *   S1  sde = (SR_peak - mean(SR)) / sd(SR) over the curve's whole coarse spectrum (population sd);

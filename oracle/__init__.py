@@ -67,6 +67,8 @@ def lib():
         L.oracle_sde.argtypes = [C.c_int64, _f64p, C.c_int64]
         L.oracle_bin_shift.restype = C.c_int
         L.oracle_bin_shift.argtypes = [C.c_double, C.c_double, C.c_int, C.c_double]
+        L.oracle_bins_shift_many.restype = None
+        L.oracle_bins_shift_many.argtypes = [C.c_int64, _f64p, _f64p, C.c_int, C.c_double, _i32p]
         L.oracle_refine_spectrum.restype = C.c_int
         L.oracle_refine_spectrum.argtypes = [C.c_int64, _f32p, _f32p, _f32p, C.c_double, C.c_double, C.c_int, C.c_int,
                                              C.c_int, C.c_int, C.c_int, _f64p, _f64p, _i32p, _i32p, _f64p]
@@ -143,6 +145,13 @@ def sde(sr, q: int) -> float:
 
 def bin_index_shift(f: float, t: float, nb: int, shift: float) -> int:
     return lib().oracle_bin_shift(float(f), float(t), int(nb), float(shift))
+
+
+def bins_shift_many(f, t, nb: int, shift: float) -> np.ndarray:
+    f = np.ascontiguousarray(f, dtype=np.float64); t = np.ascontiguousarray(t, dtype=np.float64)
+    out = np.zeros(f.size, dtype=np.int32)
+    lib().oracle_bins_shift_many(f.size, f, t, int(nb), float(shift), out)
+    return out
 
 
 def refine_spectrum(t, mag, sigma, f_lo: float, f_hi: float, n_fine: int, n_shift: int, nb: int, kmin: int, kmax: int):

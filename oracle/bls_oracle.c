@@ -259,6 +259,13 @@ int oracle_bin_shift(double f, double t, int nb, double shift)
     return b;
 }
 
+/* oracle_bin_shift over arrays, one shift for all pairs (for the shifted bin-index parity test on very many
+ * (f, t) pairs): a loop around the rule above, nothing else. */
+void oracle_bins_shift_many(int64_t n, const double *f, const double *t, int nb, double shift, int32_t *bins)
+{
+    for (int64_t i = 0; i < n; ++i) bins[i] = oracle_bin_shift(f[i], t[i], nb, shift);
+}
+
 /* S2 + S3: the spectrum of one curve on the fine grid, entry (j, h) at index j*n_shift + h. */
 int oracle_refine_spectrum(int64_t n, const float *t, const float *mag, const float *sigma, double f_lo, double f_hi,
                            int n_fine, int n_shift, int nb, int kmin, int kmax,

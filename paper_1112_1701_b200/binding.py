@@ -18,7 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libbls_b200.so")
 
 EXPORTS = ["bls_plan_create", "bls_run", "bls_topk", "bls_search_host", "bls_plan_destroy",
            "bls_plan_query", "bls_strerror", "bls_plan_last_cuda_error", "bls_debug_fold_bins",
-           "bls_variability", "bls_refine", "bls_detection_efficiency", "bls_run_field", "bls_variability_noalloc"]
+           "bls_variability", "bls_refine", "bls_detection_efficiency", "bls_run_field", "bls_variability_noalloc",
+           "bls_debug_fold_bins_shift"]
 
 BLS_OK = 0
 BLS_ERR_NULL, BLS_ERR_CONFIG, BLS_ERR_BATCH, BLS_ERR_ARG, BLS_ERR_CUDA, BLS_ERR_UNSUPPORTED = -1, -2, -3, -4, -5, -6
@@ -133,6 +134,9 @@ def lib():
         L.bls_debug_fold_bins.restype = C.c_int
         L.bls_debug_fold_bins.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32,
                                           C.c_uint32, C.c_void_p, C.POINTER(C.c_int64)]
+        L.bls_debug_fold_bins_shift.restype = C.c_int
+        L.bls_debug_fold_bins_shift.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_int32,
+                                                C.c_uint32, C.c_void_p, C.POINTER(C.c_int64)]
         L.bls_refine.restype = C.c_int
         L.bls_refine.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         L.bls_detection_efficiency.restype = C.c_int
@@ -241,6 +245,21 @@ def debug_fold_bins(f, t, n_bins: int, flags: int = 0, device: int = 0):
     ncan = C.c_int64()
     rc = lib().bls_debug_fold_bins(device, C.c_void_p(f.data_ptr()), C.c_void_p(t.data_ptr()), f.numel(),
                                    int(n_bins), int(flags), C.c_void_p(bins.data_ptr()), C.byref(ncan))
+    if rc != BLS_OK:
+        raise BlsError(rc)
+    return bins, ncan.value
+
+
+def debug_fold_bins_shift(f, t, n_bins: int, h: int, n_shift: int, flags: int = 0, device: int = 0, bins=None):
+    """bls_debug_fold_bins_shift: as debug_fold_bins on the bin grid shifted by h / (n_shift * n_bins) cycles.
+    `bins`: optional int32 CUDA tensor to write into."""
+    import torch
+    assert f.is_cuda and t.is_cuda and f.dtype == torch.float64 and t.dtype == torch.float64
+    if bins is None:
+        bins = torch.empty(f.numel(), dtype=torch.int32, device=f.device)
+    ncan = C.c_int64()
+    rc = lib().bls_debug_fold_bins_shift(device, C.c_void_p(f.data_ptr()), C.c_void_p(t.data_ptr()), f.numel(), int(n_bins),
+                                         int(h), int(n_shift), int(flags), C.c_void_p(bins.data_ptr()), C.byref(ncan))
     if rc != BLS_OK:
         raise BlsError(rc)
     return bins, ncan.value

@@ -607,6 +607,27 @@ int bls_debug_fold_bins(int32_t device, const double *f, const double *t, int64_
     return BLS_OK;
 }
 
+int bls_debug_fold_bins_shift(int32_t device, const double *f, const double *t, int64_t n, int32_t n_bins, int32_t h,
+                              int32_t n_shift, uint32_t flags, int32_t *bins, int64_t *n_canonical)
+{
+    if (!f || !t || !bins) return BLS_ERR_NULL;
+    if (n < 0 || n_bins < 4 || n_bins > 2048 || n_shift < 1 || n_shift > 8 || h < 0 || h >= n_shift) return BLS_ERR_ARG;
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    unsigned long long *d_cnt = nullptr, h_cnt = 0;
+    if (cudaMalloc(&d_cnt, sizeof(h_cnt)) != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    cudaError_t e = cudaMemset(d_cnt, 0, sizeof(h_cnt));
+    int sm_count = 1;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess)
+        e = launch_debug_bins_shift(f, t, n, n_bins, h, n_shift, (flags & BLS_FLAG_CANONICAL_PHASE) ? 1 : 0, bins, d_cnt, sm_count, nullptr);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(&h_cnt, d_cnt, sizeof(h_cnt), cudaMemcpyDeviceToHost);
+    cudaFree(d_cnt);
+    if (e != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    if (n_canonical) *n_canonical = (int64_t)h_cnt;
+    return BLS_OK;
+}
+
 int bls_variability(int32_t device, const bls_variability_config *cfg, const bls_batch *b, const int32_t *group,
                     const bls_variability_outputs *out, void *cuda_stream)
 {

@@ -165,6 +165,8 @@ int ws_shape_warps(int shape, int *search_warps);   // kernel 2 launch shape -> 
 size_t search_smem_bytes(int nb, int kmax, int warps, int buffers, int64_t n_points_in_smem);
 cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int nb, int force_canon,
                               int32_t *bins, unsigned long long *n_canon, int sm_count, cudaStream_t st);
+cudaError_t launch_debug_bins_shift(const double *f, const double *t, int64_t n, int nb, int h, int n_shift, int force_canon,
+                                    int32_t *bins, unsigned long long *n_canon, int sm_count, cudaStream_t st);
 cudaError_t search_configure(int max_smem_optin);
 cudaError_t launch_prep(const float *t, const float *mag, const float *sigma, const int64_t *offsets,
                         const int64_t *poffsets, int64_t n_curves, int64_t field_epochs, double fmax, PointRec *pts,

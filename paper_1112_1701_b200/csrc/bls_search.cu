@@ -1050,6 +1050,31 @@ cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int n
     return cudaGetLastError();
 }
 
+// The same for the shifted bin grids of bls_refine (reading S3): shift = h / (n_shift * nb) cycles, the additive
+// constant kPhaseMagic - shift and the wider guard band 2 nb + 8, exactly as lane_freq / load_ctx set them up.
+__global__ void debug_bins_shift_kernel(const double *__restrict__ f, const double *__restrict__ t, int64_t n, int nb,
+                                        int h, int n_shift, int force_canon, int32_t *__restrict__ bins,
+                                        unsigned long long *__restrict__ n_canon_out)
+{
+    const uint32_t G = 2u * (uint32_t)nb + 8u;
+    const double shift = __ddiv_rn((double)h, (double)(n_shift * nb));
+    const double magic = kPhaseMagic - shift;
+    unsigned int n_canon = 0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        bins[i] = fold_bin(f[i], t[i], nb, G, force_canon != 0, n_canon, magic, shift);
+    if (n_canon && n_canon_out) atomicAdd(n_canon_out, (unsigned long long)n_canon);
+}
+
+cudaError_t launch_debug_bins_shift(const double *f, const double *t, int64_t n, int nb, int h, int n_shift, int force_canon,
+                                    int32_t *bins, unsigned long long *n_canon, int sm_count, cudaStream_t st)
+{
+    if (n <= 0) return cudaSuccess;
+    int64_t blocks = (n + 255) / 256;
+    if (blocks > (int64_t)sm_count * 16) blocks = (int64_t)sm_count * 16;
+    debug_bins_shift_kernel<<<(unsigned)blocks, 256, 0, st>>>(f, t, n, nb, h, n_shift, force_canon, bins, n_canon);
+    return cudaGetLastError();
+}
+
 cudaError_t search_configure(int max_smem_optin)
 {
     const void *fns[] = {(const void *)search_kernel<true>,    (const void *)search_kernel<false>,
