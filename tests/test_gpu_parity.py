@@ -4,6 +4,8 @@ Element by element at sizes the oracle finishes in seconds (several frequency ti
 tail, ragged curve lengths, both cadences), then the edge cases.  Tolerances: tests/comparator.py
 (north_star: SR within 1e-4 relative; boxes identical except near-ties < 1e-6; peak lists matching).
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -476,6 +478,63 @@ def test_c2_64_curves_stratified_over_length_all_frequencies():
         if tr is not None and tr["depth"] > 0.05:      # a deep eclipse: the top peak is the period or a harmonic of it
             ratio = g["peaks"][c][0]["freq"] * tr["P"]
             assert min(abs(ratio * m - round(ratio * m)) for m in (1, 2, 3, 4)) < 0.02
+
+
+def test_c2_full_spectrum_at_the_timed_launch_geometry():
+    """The 100,000-curve C2 step bench.py times runs in chunks of 3,579 curves (2 GiB of spectrum scratch), each
+    chunk as ONE launch with 3 work items per curve x 521 tiles per item; the 64-curve test above gets 56 items of
+    28 tiles.  Here one call carries a whole chunk (the first 3,579 curves of C2), so the work-item split, the
+    resident-curve reuse across 521 tiles and the chunk-sized grid are the timed ones, and 32 curves stratified
+    over length (every injected one among the picks first) are compared with the oracle at ALL 50,000 frequencies:
+    spectra element by element, peak lists by R14 with proven ties."""
+    import torch
+    import paper_1112_1701_b200 as bls
+    B = bls.binding
+    cfg = synth.config("C2")
+    grid, k = cfg["grid"], cfg["top_k"]
+    n_chunk = (2 << 30) // (grid.nf * 12)
+    assert n_chunk == 3579
+    batch = synth.make_batch(cfg, range(n_chunk), workers=min(8, os.cpu_count() or 1))
+    freqs = synth.freq_grid(grid)
+    dev = torch.device("cuda", 0)
+    nc, nf = batch.n_curves, len(freqs)
+    with bls.Plan(n_bins=grid.nb, q_min=grid.qmin, q_max=grid.qmax, freqs=freqs, max_top_k=k) as plan:
+        sr = torch.full((nc, nf), -1.0, dtype=torch.float32, device=dev)
+        a = torch.full((nc, nf), -1, dtype=torch.int16, device=dev)
+        w = torch.full((nc, nf), -1, dtype=torch.int16, device=dev)
+        dp = torch.full((nc, nf), -1.0, dtype=torch.float32, device=dev)
+        status = torch.full((nc,), -7, dtype=torch.int32, device=dev)
+        plan.run(batch.offsets, torch.from_numpy(batch.t).to(dev), torch.from_numpy(batch.mag).to(dev),
+                 torch.from_numpy(batch.sigma).to(dev), batch.t_origin, sr=sr, best_start=a, best_width=w, depth=dp, status=status)
+        peaks = plan.peaks_to_numpy(plan.topk(k), k)
+        torch.cuda.synchronize()
+        kmin, kmax = plan.kmin, plan.kmax
+        # the geometry of the timed run: one launch, kernel 2, 3 items per curve of 521 tiles
+        assert plan.query(B.QUERY_LAST_SEARCH_LAUNCHES) == 1 and plan.query(B.QUERY_SEARCH_KERNEL) == 2
+        assert plan.query(B.QUERY_TILE_FREQS) == 521 * 32 and plan.query(B.QUERY_SEARCH_CTAS) == 3 * nc
+    assert (status.cpu().numpy() == 0).all()
+    lens = np.diff(batch.offsets)
+    order = np.argsort(lens, kind="stable")
+    picks = []
+    for st in np.array_split(order, 32):                       # one curve per length stratum, an injected one if any
+        inj = [int(c) for c in st if batch.truth[int(c)] is not None]
+        picks.append(inj[0] if inj else int(st[len(st) // 2]))
+    assert len(set(picks)) == 32 and lens[picks].min() < 700 and lens[picks].max() > 3800
+    orcs, _ = oracle.spectrum_batch(batch.offsets, batch.t, batch.mag, batch.sigma, freqs, grid.nb, kmin, kmax, curves=picks)
+    worst = 0.0
+    near = 0
+    for c, orc in zip(picks, orcs):
+        t, mag, sig = batch.curve(c)
+        g_sr = sr[c].cpu().numpy()
+        r = compare_spectrum(t, mag, sig, freqs, grid.nb, kmin, kmax, g_sr, a[c].cpu().numpy().view(np.uint16).astype(np.int32),
+                             w[c].cpu().numpy().view(np.uint16).astype(np.int32), dp[c].cpu().numpy(), orc=orc,
+                             label="C2 chunk curve %d" % c)
+        check_curve_peaks(t, freqs, grid.nb, orc, peaks[c], k, g_sr, "C2 chunk curve %d" % c)
+        worst = max(worst, r["max_rel_err"])
+        near += r["box_near_ties"]
+    assert near <= max(3, 1e-4 * 32 * nf)
+    print("\n[parity C2 at the timed geometry] %d curves in one launch (3 items x 521 tiles per curve); 32 stratified curves x %d "
+          "frequencies against the oracle: max SR rel err %.3g, %d box near-ties" % (nc, nf, worst, near))
 
 
 def test_c3_8_curves_full_grid_all_frequencies():
