@@ -16,6 +16,9 @@
 //   fold_mix        the fold's per-point-fold instruction mix (LDS.128 bcast amortised over 32 lanes,
 //                   DFMA, IMAD.WIDE, 2 x ATOMS.ADD)
 //   box_mix         the search's per-box mix (2 FADD, FFMA, MUFU.RSQ, FMUL, 1/2 FMNMX3)
+//   fold_mix_nb64, fold_field_s3, fold_field_s7, fold_field_stars
+//                   row f2 (field-shared cadence): the fold when the stars of a pointing share their epochs, so that
+//                   one bin index per (epoch, frequency) serves several stars; two designs against today's mix
 //
 // One CTA of 1024 threads per SM; cycles are clock64() deltas between two __syncthreads(), so the
 // numbers do not depend on the SM clock.  Prints one line per test: median and best over SMs.
@@ -33,13 +36,15 @@ constexpr int kThreads = 1024;
 constexpr int kIters = 2048;
 
 enum Test { ATOMS_CF, ATOMS_RAND, LDS128_BCAST, LDS32_CF, MUFU_RSQ, FADD, FADD2, FFMA, FFMA2, FMNMX3, DFMA, IMAD_WIDE,
-            FOLD_MIX, BOX_MIX, BOX_MIX2, ATOMS_CF2, LDS64_BCAST, LDS32_BCAST, LDS64_CF, I2FP, MUFU_I2FP, FMUL2, BOX_PACKED, BOX_PACKED_CVT, BOX_PACKED_THRESH, BOX_PACKED_PAIRDIV, FFMA2_ALU, FFMA2_MUFU, FFMA_ALU, MUFU_ALU, N_TESTS };
+            FOLD_MIX, BOX_MIX, BOX_MIX2, ATOMS_CF2, LDS64_BCAST, LDS32_BCAST, LDS64_CF, I2FP, MUFU_I2FP, FMUL2, BOX_PACKED, BOX_PACKED_CVT, BOX_PACKED_THRESH, BOX_PACKED_PAIRDIV, FFMA2_ALU, FFMA2_MUFU, FFMA_ALU, MUFU_ALU,
+            FOLD_MIX64, FOLD_FIELD_S3, FOLD_FIELD_S7, FOLD_FIELD_STARS, N_TESTS };
 static const char *kNames[N_TESTS] = {"atoms_add_cf", "atoms_add_rand", "lds128_bcast", "lds32_cf", "mufu_rsq", "fadd",
                                       "fadd2", "ffma", "ffma2", "fmnmx3", "dfma", "imad_wide", "fold_mix", "box_mix",
                                       "box_mix_fadd2", "atoms_add_cf_min", "lds64_bcast", "lds32_bcast", "lds64_cf", "i2fp",
-                                      "mufu_plus_i2fp", "fmul2", "box_packed", "box_packed_cvt", "box_nodiv_thresh", "box_nodiv_pair", "ffma2_plus_alu", "ffma2_plus_mufu", "ffma_plus_alu", "mufu_plus_alu"};
+                                      "mufu_plus_i2fp", "fmul2", "box_packed", "box_packed_cvt", "box_nodiv_thresh", "box_nodiv_pair", "ffma2_plus_alu", "ffma2_plus_mufu", "ffma_plus_alu", "mufu_plus_alu",
+                                      "fold_mix_nb64", "fold_field_s3", "fold_field_s7", "fold_field_stars"};
 // lane-operations each thread performs per inner iteration (what the rate is quoted in)
-static const double kOpsPerIter[N_TESTS] = {8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 4, 8, 8, 8, 8, 8, 8, 8, 8, 8, 14, 14, 14, 12, 16, 12, 16, 12};
+static const double kOpsPerIter[N_TESTS] = {8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 8, 4, 8, 8, 8, 8, 8, 8, 8, 8, 8, 14, 14, 14, 12, 16, 12, 16, 12, 4, 12, 28, 4};
 static const char *kUnit[N_TESTS] = {"ATOMS lane-ops", "ATOMS lane-ops", "LDS.128 lane-loads", "LDS.32 lane-loads",
                                      "MUFU lane-ops", "FADD lane-ops", "FADD2 lane-instr (2 adds each)", "FFMA lane-ops",
                                      "FFMA2 lane-instr (2 fmas each)", "FMNMX3 lane-ops (+1/8 FADD)", "DFMA lane-ops",
@@ -51,7 +56,11 @@ static const char *kUnit[N_TESTS] = {"ATOMS lane-ops", "ATOMS lane-ops", "LDS.12
                                      "warp-instr lanes (8 FFMA2 + 8 LOP3 per iteration: does a packed instruction hold the issue port for 2 clocks?)",
                                      "warp-instr lanes (8 FFMA2 + 4 MUFU.RSQ per iteration)",
                                      "warp-instr lanes (8 FFMA + 8 LOP3 per iteration)",
-                                     "warp-instr lanes (4 MUFU.RSQ + 8 LOP3 per iteration)"};
+                                     "warp-instr lanes (4 MUFU.RSQ + 8 LOP3 per iteration)",
+                                     "point-folds (fold_mix at nb = 64: the baseline of the three field lines)",
+                                     "point-folds (f2, lanes = frequencies, 3 stars per epoch read: bin index once per (epoch, frequency), 2 LDS.128 + 6 ATOMS per 3 stars)",
+                                     "point-folds (f2, lanes = frequencies, 7 stars per epoch read: 4 LDS.128 + 14 ATOMS per 7 stars)",
+                                     "point-folds (f2 as VERDICT r2 #6 words it, lanes = stars: warp-uniform phase from an LDS.64 broadcast of t, per-lane LDS.64 of (qw, qy), 2 ATOMS)"};
 
 __device__ __forceinline__ float rsq(float x) { float y; asm volatile("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ unsigned long long add2(unsigned long long a, unsigned long long b)
@@ -76,7 +85,7 @@ __global__ void __launch_bounds__(kThreads, 1) bench(long long *cycles, float *s
     float f0 = 1.0f + tid * 1e-3f, f1 = 1.5f, f2 = 0.25f, f3 = 0.75f, f4 = 1.25f, f5 = 2.f, f6 = 3.f, f7 = 0.5f;
     unsigned long long p0 = 0x3f8000003f800000ull, p1 = p0 + tid, p2 = p0 + 7, p3 = p0 + 11, p4 = p0, p5 = p1, p6 = p2, p7 = p3;
     double d0 = 1.0 + tid, d1 = 2.0, d2 = 3.0, d3 = 4.0, d4 = 5.0, d5 = 6.0, d6 = 7.0, d7 = 8.0;
-    const double fr = 0.3712345 + 1e-6 * lane, dc = 1e-3 * (1 + lane);
+    const double fr = 0.3712345 + 1e-6 * lane, dc = 1e-3 * (1 + lane), frw = 0.3712345 + 1e-3 * warp;
     float fc = 1e-3f * (1 + lane);
     const float fm = 0.999f + 1e-6f * lane;
     const unsigned long long pc = 0x3a83126f3a83126full + lane, pm = 0x3f7fbe773f7fbe77ull + lane;
@@ -147,7 +156,50 @@ __global__ void __launch_bounds__(kThreads, 1) bench(long long *cycles, float *s
         } else if (T == IMAD_WIDE) {
 #pragma unroll
             for (int u = 0; u < 8; ++u) { q[u] = (unsigned long long)(uint32_t)(q[u] >> 32) * (uint32_t)nb + q[u]; }
-        } else if (T == FOLD_MIX) {
+        } else if (T == FOLD_FIELD_S3 || T == FOLD_FIELD_S7) {
+            // Row f2 with lanes = frequencies: S stars of a field share their epochs, so one phase / bin index per
+            // (epoch, frequency) serves S stars, each with its own [64 bins][W | Y][32 lanes] buffer (16 KB apart: an
+            // immediate offset).  Epoch record: (t fp64, qw0, qy0), then (qw, qy) pairs of the other stars, 16 B each.
+            // 4 epochs per iteration.
+            constexpr int S = T == FOLD_FIELD_S3 ? 3 : 7;
+            constexpr int REC = (S + 1) / 2;            // LDS.128 per epoch
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint4 *rec = reinterpret_cast<const uint4 *>(pts + ((((it * 4 + u) * 8 + warp) * REC) & 1020) * 4);
+                const uint4 v = rec[0];
+                const double t = __hiloint2double((int)(v.y & 0xfffffu) | 0x40000000, (int)v.x);
+                const double y = fma(fr, t, 1572864.0);
+                const unsigned long long pr = (unsigned long long)(uint32_t)__double2loint(y) * 64u;
+                uint32_t *b = &sm[(int)(pr >> 32) * 64 + lane];
+                atomicAdd(b, v.z);
+                atomicAdd(b + 32, v.w + (uint32_t)pr);
+#pragma unroll
+                for (int r = 1; r < REC; ++r) {
+                    const uint4 w = rec[r];
+                    atomicAdd(b + (2 * r - 1) * 4096, w.x);
+                    atomicAdd(b + (2 * r - 1) * 4096 + 32, w.y);
+                    atomicAdd(b + (2 * r) * 4096, w.z);
+                    atomicAdd(b + (2 * r) * 4096 + 32, w.w);
+                }
+            }
+        } else if (T == FOLD_FIELD_STARS) {
+            // Row f2 with lanes = stars: the warp folds ONE frequency for 32 stars.  Per epoch: t from an LDS.64
+            // broadcast, the phase and bin index computed identically by every lane (warp-uniform), the star's
+            // (qw, qy) from a conflict-free per-lane LDS.64 of the [epoch][32 stars] tile, 2 ATOMS into the warp's own
+            // columns bins[bin][W | Y][star].  4 epochs per iteration; the tile is the 64-epoch "points" area.
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int e = ((it * 4 + u) * 8 + warp) & 63;
+                const uint2 tt = *reinterpret_cast<const uint2 *>(sm + (e & 31) * 2);
+                const double t = __hiloint2double((int)(tt.y & 0xfffffu) | 0x40000000, (int)tt.x);
+                const double y = fma(frw, t, 1572864.0);
+                const unsigned long long pr = (unsigned long long)(uint32_t)__double2loint(y) * 64u;
+                const uint2 v = *reinterpret_cast<const uint2 *>(pts + e * 64 + lane * 2);
+                uint32_t *b = &sm[(int)(pr >> 32) * 64 + lane];
+                atomicAdd(b, v.x);
+                atomicAdd(b + 32, v.y + (uint32_t)pr);
+            }
+        } else if (T == FOLD_MIX || T == FOLD_MIX64) {
             // 4 points per iteration: LDS.128 broadcast, DFMA with the magic constant, IMAD.WIDE, 2 ATOMS.ADD
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
@@ -362,5 +414,10 @@ int main()
     run<FFMA_ALU>(n_sm, nb, d_cyc, d_sink);
     run<MUFU_ALU>(n_sm, nb, d_cyc, d_sink);
     run<BOX_PACKED_PAIRDIV>(n_sm, nb, d_cyc, d_sink);
+    // row f2 at the paper's shape (140-300 epochs per star want few bins: nb = 64 as in C4); smem = S buffers of 64 bins
+    run<FOLD_MIX64>(n_sm, 64, d_cyc, d_sink);
+    run<FOLD_FIELD_S3>(n_sm, 3 * 64, d_cyc, d_sink);
+    run<FOLD_FIELD_S7>(n_sm, 7 * 64, d_cyc, d_sink);
+    run<FOLD_FIELD_STARS>(n_sm, 64, d_cyc, d_sink);
     return 0;
 }
