@@ -151,8 +151,10 @@ int bls_run(bls_plan *plan, const bls_batch *batch, const bls_outputs *out, void
  * field is one epoch list and a dense [stars][epochs] matrix of magnitudes and errors.  An entry whose mag or
  * sigma is not finite, or whose sigma <= 0, is an epoch ABSENT for that star (flagged measurement): it simply
  * does not take part; it is not a data fault.  The result for each star is by definition that of bls_run on the
- * star's present epochs.  DESIGN.md section 6.5 says why the bin indices are NOT shared between stars on this
- * hardware (a table lookup costs more shared-memory issue slots than recomputing the phase). */
+ * star's present epochs.  Where three bin buffers and the field's epochs fit shared memory at least twice per SM
+ * (e.g. 64 bins and 140-300 epochs, the paper's cadence; 200 bins do not), the fold computes each epoch's phase
+ * and bin index once per (epoch, frequency) for three stars at a time (1.7x the per-star
+ * fold as an instruction mix); other shapes run the per-star kernels of bls_run on the field layout. */
 typedef struct {
     int64_t n_stars;
     int64_t n_epochs;        /* >= 1                                                                  */
@@ -353,6 +355,10 @@ int bls_detection_efficiency(int32_t device, const bls_batch *batch, int64_t n_f
 #define BLS_FLAG_MERGE_WARPS(n) (((uint32_t)(n) & 7u) << 24) /* tuning: warps per CTA that share the exact
                                        merge of a tile, 1..7 (0 = the library's choice).           */
 
+#define BLS_FLAG_NO_FIELD_KERNEL (1u << 29) /* tuning: bls_run_field never uses the field kernel (kernel 4: three stars
+                                       per CTA share each epoch's bin index) and runs the per-star kernels of bls_run.
+                                       Like the other kernel-selection flags: near-tied boxes only.          */
+
 #define BLS_FLAG_FOLD_DEPTH(n) (((uint32_t)(n) & 3u) << 27) /* tuning: groups of 4 points a fold warp keeps in
                                        flight, 1 or 2 (0 = the library's choice).  Never changes results. */
 
@@ -366,8 +372,8 @@ int bls_detection_efficiency(int32_t device, const bls_batch *batch, int64_t n_f
                                        kernel launches of the last bls_run took (synchronises)    */
 #define BLS_QUERY_SEARCH_KERNEL 11  /* search kernel of the last run: 1 = single buffer (all warps do every
                                        phase; also the small-CTA shape of small configurations),
-                                       2 = warp-specialised double buffer, 3 = one warp per tile
-                                       (0 = none yet)                                              */
+                                       2 = warp-specialised double buffer, 3 = one warp per tile,
+                                       4 = field kernel of bls_run_field (0 = none yet)            */
 #define BLS_QUERY_LAST_SEARCH_LAUNCHES 12 /* search kernel launches of the last bls_run (one per chunk of
                                        curves): LAST_SEARCH_NS / this = the average launch duration */
 #define BLS_QUERY_WS_SHAPE 13       /* launch shape of the warp-specialised kernel in the last run: 0 = equal registers,

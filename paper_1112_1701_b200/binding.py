@@ -26,6 +26,7 @@ BLS_ERR_NULL, BLS_ERR_CONFIG, BLS_ERR_BATCH, BLS_ERR_ARG, BLS_ERR_CUDA, BLS_ERR_
 BLS_ERR_CAPACITY = -7
 NOALLOC_MAX_STARS, NOALLOC_MAX_CELLS = 16384, 4096      # include/bls.h BLS_NOALLOC_MAX_*
 BLS_FLAG_NONE, BLS_FLAG_CANONICAL_PHASE, BLS_FLAG_SINGLE_BUFFER, BLS_FLAG_NO_SMALL_CTAS, BLS_FLAG_WARP_PER_TILE = 0, 1, 2, 4, 8
+BLS_FLAG_NO_FIELD_KERNEL = 1 << 29
 
 
 def BLS_FLAG_WARPS(n):

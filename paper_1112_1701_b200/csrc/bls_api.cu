@@ -244,6 +244,7 @@ int search_launch_setup(bls_plan *p, int64_t nf, int64_t max_n, int64_t chunk, S
     a.u_sr = nullptr; a.u_start = nullptr; a.u_width = nullptr; a.u_depth = nullptr;
     a.f_lo = nullptr; a.f_step = nullptr; a.refine_k = 0; a.n_fine = 0; a.n_shift = 0;
     a.canon_count = p->d_canon;
+    a.field_curves = 0;
 
     smem_out = smem;
     L.items = items;
@@ -529,12 +530,38 @@ int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_ou
     SearchLaunch L;
     if ((rc = search_launch_setup(p, p->nf, max_n, chunk, L)) != BLS_OK) return rc;
     SearchArgs &a = L.a;
-    const size_t smem = L.smem;
-    const int64_t items = L.items;
     a.u_sr = out ? out->sr : nullptr;
     a.u_start = out ? out->best_start : nullptr;
     a.u_width = out ? out->best_width : nullptr;
     a.u_depth = out ? out->depth : nullptr;
+    int64_t units = chunk;                                       // CTAs of a launch = units x items
+    if (field && !(p->flags & (BLS_FLAG_NO_FIELD_KERNEL | BLS_FLAG_SINGLE_BUFFER | BLS_FLAG_WARP_PER_TILE |
+                               BLS_FLAG_WS_SHAPE(7) | BLS_FLAG_FOLD_WARPS(0xff)))) {
+        // f2: the field kernel (kernel 4) where its kFieldStars bin buffers and the field's records fit an SM at least
+        // twice; same work-item sizing as search_launch_setup, over groups of stars instead of stars
+        const int warps_flag = (int)((p->flags >> 8) & 0xffu);
+        const int fw = (warps_flag >= 1 && warps_flag <= kMaxSearchWarps) ? warps_flag : kFieldWarps;
+        const size_t fsmem = field_smem_bytes(p->nb, p->kmax, fw, max_n);
+        if (2 * (fsmem + 1024) <= (size_t)p->max_smem_sm && fsmem <= (size_t)p->max_smem_optin) {
+            int ctas_per_sm = (int)((size_t)p->max_smem_sm / (fsmem + 1024));
+            const int reg_ctas = 65536 / (96 * fw * 32);
+            if (ctas_per_sm > reg_ctas) ctas_per_sm = reg_ctas;
+            if (ctas_per_sm > 32) ctas_per_sm = 32;
+            units = (chunk + kFieldStars - 1) / kFieldStars;
+            const int ntiles = (int)((p->nf + kTileFreqs - 1) / kTileFreqs);
+            int64_t it = ((int64_t)p->sm_count * ctas_per_sm * 24 + units - 1) / units;
+            if (it < 1) it = 1;
+            if (it > ntiles) it = ntiles;
+            const int tpi = (int)((ntiles + it - 1) / it);
+            L.items = (ntiles + tpi - 1) / tpi;
+            L.smem = fsmem;
+            L.tiles_per_item = tpi; L.kernel = 4; L.ws_shape = -1;
+            a.kernel = 4; a.threads = fw * 32; a.pts_in_smem = 1; a.tiles_per_item = tpi; a.items_per_curve = (int)L.items;
+            a.nrows = search_rows_for(p->nb, p->kmax, 0);
+            const int merge_flag = (int)((p->flags >> 24) & 7u);
+            a.merge_warps = merge_flag >= 1 ? merge_flag : (fw < 4 ? fw : 4);
+        }
+    }
     p->last_max_n = max_n;
     p->last_tiles_per_item = L.tiles_per_item;
     p->last_kernel = L.kernel;
@@ -546,19 +573,20 @@ int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_ou
     for (int64_t base = 0; base < nc; base += chunk) {
         const int64_t cc = (nc - base < chunk) ? nc - base : chunk;
         a.curve_base = base;
+        a.field_curves = cc;
         while (p->ev.size() < p->ev_used + 2) {
             cudaEvent_t e;
             BLS_CUDA(p, cudaEventCreate(&e));
             try { p->ev.push_back(e); } catch (...) { cudaEventDestroy(e); return BLS_ERR_CUDA; }
         }
         BLS_CUDA(p, cudaEventRecord(p->ev[p->ev_used], st));
-        BLS_CUDA(p, launch_search(a, cc, smem, st));
+        BLS_CUDA(p, launch_search(a, cc, L.smem, st));
         BLS_CUDA(p, cudaEventRecord(p->ev[p->ev_used + 1], st));
         p->ev_used += 2;
         BLS_CUDA(p, launch_peaks(p->d_sr, p->d_ak, p->d_depth, p->d_meta, base, cc, (int)p->nf,
                                  p->max_top_k, p->d_cand, p->d_sr_stats, st));
         p->last_launches += 2;
-        p->last_search_ctas += cc * items;
+        p->last_search_ctas += (L.kernel == 4 ? (cc + kFieldStars - 1) / kFieldStars : cc) * L.items;
     }
     p->last_n_curves = nc;
     return BLS_OK;

@@ -52,6 +52,8 @@ constexpr int kMergeWarps = 8;        // upper bound of the warps that share the
 constexpr int kSmallWarps = 2;        // small shapes: kernel 1 with CTAs of this many warps ...
 constexpr int kSmallCtasMin = 8;      // ... when at least this many fit an SM
 constexpr int kWtWarps = 5;           // warp-per-tile kernel: warps per CTA (two CTAs per SM)
+constexpr int kFieldStars = 3;        // field kernel (kernel 4): stars of a field per CTA that share each epoch's bin index
+constexpr int kFieldWarps = 4;        // ... and its CTA size in warps (BLS_FLAG_WARPS overrides)
 constexpr int kPrepThreads = 256;
 constexpr int kPeakThreads = 256;
 
@@ -74,7 +76,8 @@ struct SearchArgs {
     int search_warps;           // kernel 2: this many search warps (then the fold warps)
     int ws_shape;               // kernel 2: 0 = equal registers, run-time split; 1, 2 = three roles, registers moved with setmaxnreg (WsShape)
     int merge_warps;            // warps that share the exact merge of a tile (1..kMergeWarps; they split the widths)
-    int kernel;                 // 1 single buffer, 2 warp-specialised double buffer, 3 one warp per tile
+    int kernel;                 // 1 single buffer, 2 warp-specialised double buffer, 3 one warp per tile, 4 field (kFieldStars stars per CTA)
+    int64_t field_curves;       // kernel 4: stars in this launch (the last group may hold fewer than kFieldStars)
     int force_canonical;        // BLS_FLAG_CANONICAL_PHASE
     float *sr;                  // chunk scratch, [chunk_curves][nf]
     uint32_t *ak;
@@ -163,6 +166,7 @@ __device__ __forceinline__ double block_max_d(double v, double *sh) {
 int search_rows_for(int nb, int kmax, int slots);
 int ws_shape_warps(int shape, int *search_warps);   // kernel 2 launch shape -> warps per CTA, search warps (0 = run-time)
 size_t search_smem_bytes(int nb, int kmax, int warps, int buffers, int64_t n_points_in_smem);
+size_t field_smem_bytes(int nb, int kmax, int warps, int64_t n_pad);   // kernel 4: kFieldStars bin buffers + field records
 cudaError_t launch_debug_bins(const double *f, const double *t, int64_t n, int nb, int force_canon,
                               int32_t *bins, unsigned long long *n_canon, int sm_count, cudaStream_t st);
 cudaError_t launch_debug_bins_shift(const double *f, const double *t, int64_t n, int nb, int h, int n_shift, int force_canon,

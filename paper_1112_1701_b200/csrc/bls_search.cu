@@ -1027,6 +1027,200 @@ search_wt_kernel(const SearchArgs a)
     count_canonical(a, n_canon, lane);
 }
 
+// ---- kernel 4 (row f2, field-shared cadence): kFieldStars stars of a field per CTA ---------------------
+// All stars of a pointing share their epochs, so the phase and the bin index of an epoch at a
+// trial frequency are the same for every star: this kernel computes them ONCE per (epoch, frequency) and adds the
+// epoch's (qw, qy) of S stars into S bin buffers.  Measured as an instruction mix (profiles/r03_microbench.md):
+// 9.6 point-folds per clock per SM at S = 3 against 5.7 for the per-star fold -- the DFMA, the slow IMAD.WIDE
+// (18 lane-ops per clock per SM) and the row address are shared by S stars, and the stars' integers come two to
+// an LDS.128.  Everything after the fold (extension rows, box search, exact merge, outputs) is kernel 1's, once per
+// star on that star's buffer, so results are those of the per-star kernels (bins are exact integers).
+//   shared memory: bins [S][nrows][256 B] | cand_t, cand_c, post_v, post_k [nw][32] | field records | S CurveMeta
+//   field record of epoch e, (S + 1) / 2 uint4: (t lo, t hi, qw0, qy0), (qw1, qy1, qw2, qy2), ...
+// The prepared records of a field are per star (prep_kernel<true>): a star's record of an epoch it has no
+// measurement for carries no weight and a placeholder time.  Staging takes the epoch's time from the first star of
+// the group whose record carries weight (all such records hold the same fp32 epoch time); if none does, the epoch
+// adds zero to whatever bin it lands in.
+template <int S>
+__device__ __forceinline__ void field_add(uint32_t addr, uint32_t buf_bytes, uint32_t rec_sa, const uint4 &v0, bool negate)
+{
+    constexpr int REC = (S + 1) / 2;
+    const uint32_t sg = negate ? 0xffffffffu : 0u, one = negate ? 1u : 0u;       // two's complement: -x = (x ^ ~0) + 1
+    red_add(addr, (v0.z ^ sg) + one);
+    red_add(addr + 128, (v0.w ^ sg) + one);
+#pragma unroll
+    for (int r = 1; r < REC; ++r) {
+        const uint4 w = lds128(rec_sa + r * 16);
+        const uint32_t a1 = addr + (uint32_t)(2 * r - 1) * buf_bytes, a2 = a1 + buf_bytes;
+        red_add(a1, (w.x ^ sg) + one);
+        red_add(a1 + 128, (w.y ^ sg) + one);
+        red_add(a2, (w.z ^ sg) + one);
+        red_add(a2 + 128, (w.w ^ sg) + one);
+    }
+}
+
+template <int S>
+__device__ __forceinline__ void fold_field_tile(int nb, uint32_t G, bool force_canon, const LaneFreq &lf, uint32_t bins_s,
+                                                uint32_t buf_bytes, uint32_t frec_sa, int n_pad, const CurveMeta *metas,
+                                                int lane, int gw, int gnw, unsigned int &n_canon)
+{
+    constexpr int REC = (S + 1) / 2;
+    const uint32_t colw = bins_s + lane * 4;
+    const int ngroups = n_pad >> 2;
+    if (gw == 0) {                                   // the zero-time epoch of each star (bin 0)
+#pragma unroll
+        for (int s = 0; s < S; ++s) {
+            const uint32_t w0 = metas[s].w0;
+            const int32_t y0 = metas[s].y0;
+            if (w0 | (uint32_t)y0) {
+                red_add(colw + s * buf_bytes, w0);
+                red_add(colw + s * buf_bytes + 128, (uint32_t)y0);
+            }
+        }
+    }
+    if (force_canon) {
+        for (int g = gw; g < ngroups; g += gnw)
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t ra = frec_sa + (uint32_t)(g * 4 + u) * (REC * 16);
+                const uint4 v0 = lds128(ra);
+                const int bin = canonical_bin(lf.f, __hiloint2double((int)v0.y, (int)v0.x), nb, 0.0);
+                n_canon += S;
+                field_add<S>(colw + bin * kRowBytes, buf_bytes, ra, v0, false);
+            }
+        return;
+    }
+    uint32_t lomin = 0xffffffffu;
+    for (int g = gw; g < ngroups; g += gnw) {        // 4 epochs in flight, S stars each
+        uint4 v0[4];
+        unsigned long long pr[4];
+        const uint32_t ra = frec_sa + (uint32_t)(g * 4) * (REC * 16);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) v0[u] = lds128(ra + u * (REC * 16));
+#pragma unroll
+        for (int u = 0; u < 4; ++u) pr[u] = fast_bin_pos(lf.f, __hiloint2double((int)v0[u].y, (int)v0[u].x), nb, G, lf.magic);
+#pragma unroll
+        for (int u = 0; u < 4; u += 2) lomin = min(lomin, min((uint32_t)pr[u], (uint32_t)pr[u + 1]));
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            field_add<S>(row_addr(colw, (uint32_t)(pr[u] >> 32)), buf_bytes, ra + u * (REC * 16), v0[u], false);
+    }
+    const bool mine = lomin < 2u * G;
+    if (__any_sync(0xffffffffu, mine)) {             // repair (rare), as in fold_tile: move the epoch's S contributions
+        for (int g = gw; g < ngroups; g += gnw)
+            for (int u = 0; u < 4; ++u) {
+                const uint32_t ra = frec_sa + (uint32_t)(g * 4 + u) * (REC * 16);
+                const uint4 v0 = lds128(ra);
+                const double t = __hiloint2double((int)v0.y, (int)v0.x);
+                const unsigned long long pr = fast_bin_pos(lf.f, t, nb, G, lf.magic);
+                if (mine && (uint32_t)pr < 2u * G) {
+                    const int fb = (int)(pr >> 32), cb = canonical_bin(lf.f, t, nb, 0.0);
+                    n_canon += S;
+                    if (cb != fb) {
+                        field_add<S>(colw + fb * kRowBytes, buf_bytes, ra, v0, true);
+                        field_add<S>(colw + cb * kRowBytes, buf_bytes, ra, v0, false);
+                    }
+                }
+            }
+    }
+}
+
+size_t field_smem_bytes(int nb, int kmax, int warps, int64_t n_pad)
+{
+    return (size_t)kFieldStars * search_rows_for(nb, kmax, 0) * kRowBytes + (size_t)4 * warps * kTileFreqs * 4 +
+           (size_t)n_pad * ((kFieldStars + 1) / 2) * 16 + (size_t)kFieldStars * sizeof(CurveMeta);
+}
+
+template <int S>
+__global__ void __launch_bounds__(kMaxSearchWarps * 32, 2)
+search_field_kernel(const SearchArgs a)
+{
+    constexpr int REC = (S + 1) / 2;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nthr = blockDim.x, nw = nthr >> 5;
+    const int64_t local0 = (int64_t)(blockIdx.x / a.items_per_curve) * S;     // first star of the group, within the launch
+    const int item = blockIdx.x % a.items_per_curve;
+    const int ns = (int)min((int64_t)S, a.field_curves - local0);            // the last group of a launch may be short
+    const int64_t cv0 = a.curve_base + local0;
+    const int64_t rec0 = a.poffsets[cv0];
+    const int n_pad = (int)(a.poffsets[cv0 + 1] - rec0);                      // the same for every star of a field
+    const int ntiles = (a.nf + kTileFreqs - 1) / kTileFreqs;
+    const int tile0 = item * a.tiles_per_item, tile1 = min(tile0 + a.tiles_per_item, ntiles);
+    const uint32_t buf_bytes = (uint32_t)a.nrows * kRowBytes;
+    float *cand_t = reinterpret_cast<float *>(smem_raw + (size_t)S * buf_bytes);
+    uint32_t *cand_c = reinterpret_cast<uint32_t *>(cand_t + nw * 32);
+    float *post_v = reinterpret_cast<float *>(cand_c + nw * 32);
+    uint32_t *post_k = reinterpret_cast<uint32_t *>(post_v + nw * 32);
+    uint4 *frec = reinterpret_cast<uint4 *>(post_k + nw * 32);
+    CurveMeta *metas = reinterpret_cast<CurveMeta *>(frec + (size_t)n_pad * REC);
+
+    if (tid < S) {
+        CurveMeta m;
+        if (tid < ns) m = a.meta[cv0 + tid];
+        else {
+            m.ncw = 0.f; m.cy = 0.f; m.status = BLS_CURVE_TOO_FEW; m.force_canonical = 0; m.swt = 0u; m.w0 = 0u; m.y0 = 0;
+            m.pad_ = 0; m.sr_scale = 0.0; m.dp_scale = 0.0; m.wx2 = 0.0;
+        }
+        metas[tid] = m;
+    }
+    for (int e = tid; e < n_pad; e += nthr) {        // a1 Load: the group's records -> field records
+        uint4 r[S];
+#pragma unroll
+        for (int s = 0; s < S; ++s)
+            r[s] = s < ns ? __ldg(reinterpret_cast<const uint4 *>(a.pts + rec0 + (int64_t)s * n_pad + e)) : make_uint4(0u, 0u, 0u, 0u);
+        uint32_t tl = r[0].x, th = r[0].y;
+        bool weighted = (r[0].z | r[0].w) != 0u, timed = (tl | th) != 0u;
+#pragma unroll
+        for (int s = 1; s < S; ++s) {
+            const bool ws = (r[s].z | r[s].w) != 0u, ts = (r[s].x | r[s].y) != 0u;
+            if ((ws && !weighted) || (ts && !timed && !weighted)) { tl = r[s].x; th = r[s].y; }
+            weighted |= ws; timed |= ts;
+        }
+        frec[e * REC] = make_uint4(tl, th, r[0].z, r[0].w);
+#pragma unroll
+        for (int q = 1; q < REC; ++q) frec[e * REC + q] = make_uint4(r[2 * q - 1].z, r[2 * q - 1].w, r[2 * q].z, r[2 * q].w);
+    }
+    __syncthreads();
+    bool any_ok = false, force_canon = a.force_canonical != 0;
+    for (int s = 0; s < ns; ++s) {
+        if (metas[s].status != BLS_CURVE_OK)
+            zero_fill_outputs(out_rows(a, local0 + s, cv0 + s), tile0 * kTileFreqs, min(tile1 * kTileFreqs, a.nf), a.kmin, tid, nthr);
+        else any_ok = true;
+        force_canon |= metas[s].force_canonical != 0;
+    }
+    if (!any_ok) return;
+    const uint32_t bins_s = smem_u32(smem_raw), frec_sa = smem_u32(frec);
+    const uint32_t G = (uint32_t)a.nb + 8u;
+    unsigned int n_canon = 0;
+
+    LaneFreq lf_next = lane_freq(a, cv0, tile0 * kTileFreqs + lane);
+    for (int tile = tile0; tile < tile1; ++tile) {
+        const int q0 = tile * kTileFreqs;
+        const LaneFreq lf = lf_next;
+#pragma unroll
+        for (int s = 0; s < S; ++s) zero_bins(bins_s + s * buf_bytes, a.nb, tid, nthr);
+        __syncthreads();
+        fold_field_tile<S>(a.nb, G, force_canon, lf, bins_s, buf_bytes, frec_sa, n_pad, metas, lane, warp, nw, n_canon);
+        if (tile + 1 < tile1) lf_next = lane_freq(a, cv0, q0 + kTileFreqs + lane);
+        __syncthreads();
+        for (int s = 0; s < ns; ++s) {
+            if (metas[s].status != BLS_CURVE_OK) continue;                     // CTA-uniform
+            TileCtx c;
+            load_ctx(c, a, metas[s], a.nrows);
+            c.n_pad = n_pad;
+            const uint32_t buf = bins_s + s * buf_bytes;
+            extend_rows(c, buf, tid, nthr);
+            __syncthreads();
+            search_warp<kSmax>(buf, c, lane, warp, nw, cand_t, cand_c);
+            __syncthreads();
+            merge_tile(c, buf, cand_t, cand_c, post_v, post_k, nw, min(nw, a.merge_warps), warp, lane, q0 + lane, a.nf,
+                       out_rows(a, local0 + s, cv0 + s), [] { __syncthreads(); });
+            __syncthreads();
+        }
+    }
+    count_canonical(a, n_canon, lane);
+}
+
 // Diagnostic: the bin index the fold assigns to each (f, t) pair -- the same fold_bin() the search
 // kernel inlines.  Lets tests compare bin indices with the oracle on very many pairs.
 __global__ void debug_bins_kernel(const double *__restrict__ f, const double *__restrict__ t, int64_t n,
@@ -1081,7 +1275,8 @@ cudaError_t search_configure(int max_smem_optin)
                          (const void *)search_ws_kernel<true, 0>, (const void *)search_ws_kernel<false, 0>,
                          (const void *)search_ws_kernel<true, 1>, (const void *)search_ws_kernel<false, 1>,
                          (const void *)search_ws_kernel<true, 2>, (const void *)search_ws_kernel<false, 2>,
-                         (const void *)search_wt_kernel<true>, (const void *)search_wt_kernel<false>};
+                         (const void *)search_wt_kernel<true>, (const void *)search_wt_kernel<false>,
+                         (const void *)search_field_kernel<kFieldStars>};
     for (const void *f : fns) {
         cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem_optin);
         if (e != cudaSuccess) return e;
@@ -1091,7 +1286,8 @@ cudaError_t search_configure(int max_smem_optin)
 
 cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem, cudaStream_t st)
 {
-    const int64_t grid = chunk_curves * (int64_t)a.items_per_curve;
+    const int64_t units = a.kernel == 4 ? (chunk_curves + kFieldStars - 1) / kFieldStars : chunk_curves;   // kernel 4: groups of stars
+    const int64_t grid = units * (int64_t)a.items_per_curve;
     if (grid <= 0) return cudaSuccess;
     if (grid > 2147483647LL) return cudaErrorInvalidConfiguration;
     const unsigned g = (unsigned)grid;
@@ -1100,7 +1296,8 @@ cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem
         if (a.pts_in_smem) K<true><<<g, a.threads, smem, st>>>(a);     \
         else K<false><<<g, a.threads, smem, st>>>(a);                  \
     } while (0)
-    if (a.kernel == 3) BLS_LAUNCH(search_wt_kernel);
+    if (a.kernel == 4) search_field_kernel<kFieldStars><<<g, a.threads, smem, st>>>(a);
+    else if (a.kernel == 3) BLS_LAUNCH(search_wt_kernel);
     else if (a.kernel == 2) {
 #define BLS_LAUNCH_WS(SH)                                                           \
     do {                                                                            \

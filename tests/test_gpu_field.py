@@ -105,3 +105,78 @@ def test_field_faults():
         plan.run_field(t, mag, sig, status=status)
         assert status.cpu().tolist() == [0, 0, 0]
         assert plan.peaks_to_numpy(plan.topk(2), 2).shape == (3, 2)
+
+
+def _run_field(t, mag, sig, grid, freqs, k, flags=0, scratch_bytes=0, origin=2455000.5):
+    import torch
+    import paper_1112_1701_b200 as bls
+    B = bls.binding
+    dev = torch.device("cuda", 0)
+    n_stars = mag.shape[0]
+    with bls.Plan(n_bins=grid.nb, q_min=grid.qmin, q_max=grid.qmax, freqs=freqs, max_top_k=k, flags=flags,
+                  scratch_bytes=scratch_bytes) as plan:
+        sr = torch.full((n_stars, grid.nf), -1.0, dtype=torch.float32, device=dev)
+        a = torch.full((n_stars, grid.nf), -1, dtype=torch.int16, device=dev)
+        kk = torch.full((n_stars, grid.nf), -1, dtype=torch.int16, device=dev)
+        dp = torch.full((n_stars, grid.nf), -1.0, dtype=torch.float32, device=dev)
+        status = torch.full((n_stars,), -7, dtype=torch.int32, device=dev)
+        plan.run_field(torch.from_numpy(t).to(dev), torch.from_numpy(mag).to(dev), torch.from_numpy(sig).to(dev), origin,
+                       sr=sr, best_start=a, best_width=kk, depth=dp, status=status)
+        peaks = plan.peaks_to_numpy(plan.topk(k), k)
+        torch.cuda.synchronize()
+        return dict(sr=sr.cpu().numpy(), dp=dp.cpu().numpy(), st=status.cpu().numpy(), peaks=peaks,
+                    a=a.cpu().numpy().view(np.uint16).astype(np.int32), k=kk.cpu().numpy().view(np.uint16).astype(np.int32),
+                    kmin=plan.kmin, kmax=plan.kmax, kernel=plan.query(B.QUERY_SEARCH_KERNEL),
+                    launches=plan.query(B.QUERY_LAST_SEARCH_LAUNCHES), n_canon=plan.query(B.QUERY_LAST_CANONICAL))
+
+
+@pytest.mark.parametrize("n_epochs", [140, 300])
+def test_field_kernel_at_the_papers_cadence_matches_the_oracle(n_epochs):
+    """The field kernel (kernel 4: three stars per CTA share each epoch's phase and bin index) at the paper's shape:
+    140 and 300 epochs per star, 64 bins.  31 stars = 10 groups of three and a last group of
+    ONE; 2 % of the entries absent; star 5 has a single present epoch (TOO_FEW) inside a group of healthy stars; the
+    cadence's first epoch is t = 0 (the zero-time path).  Every healthy star against the fp64 oracle on its present
+    epochs at every frequency, spectra element by element and peak lists by R14; then the same field through the
+    per-star kernels (BLS_FLAG_NO_FIELD_KERNEL), through the canonical phase rule, and in chunks that cut groups."""
+    import paper_1112_1701_b200 as bls
+    n_stars, k = 31, 5
+    t, mag, sig = _field(n_stars, n_epochs, seed=100 + n_epochs)
+    assert t[0] == 0.0
+    grid = synth.Grid(2500, 0.1, 5.0, 64, 0.01, 0.15)
+    freqs = synth.freq_grid(grid)
+    g = _run_field(t, mag, sig, grid, freqs, k)
+    assert g["kernel"] == 4 and g["launches"] == 1
+    assert g["st"][5] == 1 and (g["sr"][5] == 0).all() and (g["peaks"][5]["freq_index"] == -1).all()
+    present = np.isfinite(mag) & np.isfinite(sig) & (sig > 0)
+    worst, near = 0.0, 0
+    for s in range(n_stars):
+        if s == 5:
+            continue
+        ok = present[s]
+        assert g["st"][s] == 0
+        ts, ms, ss = t[ok], mag[s][ok], sig[s][ok]
+        r = compare_spectrum(ts, ms, ss, freqs, grid.nb, g["kmin"], g["kmax"], g["sr"][s], g["a"][s], g["k"][s], g["dp"][s],
+                             label="field kernel star %d" % s)
+        check_curve_peaks(ts, freqs, grid.nb, r["oracle"], g["peaks"][s], k, g["sr"][s], "field kernel star %d" % s)
+        worst = max(worst, r["max_rel_err"])
+        near += r["box_near_ties"]
+    assert near <= max(3, 1e-4 * n_stars * grid.nf)
+    # the per-star kernels on the same field: same integer bins, so the same spectra except at near-tied boxes
+    h = _run_field(t, mag, sig, grid, freqs, k, flags=bls.BLS_FLAG_NO_FIELD_KERNEL)
+    assert h["kernel"] != 4 and np.array_equal(h["st"], g["st"])
+    np.testing.assert_allclose(g["sr"], h["sr"], rtol=2e-6, atol=0)
+    assert (g["sr"] == h["sr"]).mean() > 0.999 and (g["a"] == h["a"]).mean() > 0.999
+    # canonical phase rule for every point-fold: identical bins, identical everything
+    c = _run_field(t, mag, sig, grid, freqs, k, flags=bls.BLS_FLAG_CANONICAL_PHASE)
+    assert c["kernel"] == 4 and c["n_canon"] >= (n_epochs - 1) * grid.nf * 30
+    for key in ("sr", "a", "k", "dp", "st"):
+        assert np.array_equal(c[key], g[key]), key
+    assert np.array_equal(c["peaks"], g["peaks"])
+    # chunks of 7 stars: groups of 3 + 3 + 1 per launch, group borders differ from the one-launch run
+    m = _run_field(t, mag, sig, grid, freqs, k, scratch_bytes=7 * grid.nf * 12)
+    assert m["kernel"] == 4 and m["launches"] == 5
+    for key in ("sr", "a", "k", "dp", "st"):
+        assert np.array_equal(m[key], g[key]), key
+    assert np.array_equal(m["peaks"], g["peaks"])
+    print("\n[parity f2 field kernel] %d stars x %d shared epochs, %d frequencies, 64 bins: max SR rel err vs the oracle %.3g, "
+          "%d box near-ties; per-star kernels, canonical rule and chunked launches agree" % (n_stars, n_epochs, grid.nf, worst, near))
