@@ -536,11 +536,10 @@ int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_ou
     a.u_depth = out ? out->depth : nullptr;
     int64_t units = chunk;                                       // CTAs of a launch = units x items
     if (field && !(p->flags & (BLS_FLAG_NO_FIELD_KERNEL | BLS_FLAG_SINGLE_BUFFER | BLS_FLAG_WARP_PER_TILE |
-                               BLS_FLAG_WS_SHAPE(7) | BLS_FLAG_FOLD_WARPS(0xff)))) {
+                               BLS_FLAG_WS_SHAPE(7) | BLS_FLAG_FOLD_WARPS(0xff) | BLS_FLAG_WARPS(0xff) | BLS_FLAG_MERGE_WARPS(7)))) {
         // f2: the field kernel (kernel 4) where its kFieldStars bin buffers and the field's records fit an SM at least
         // twice; same work-item sizing as search_launch_setup, over groups of stars instead of stars
-        const int warps_flag = (int)((p->flags >> 8) & 0xffu);
-        const int fw = (warps_flag >= 1 && warps_flag <= kMaxSearchWarps) ? warps_flag : kFieldWarps;
+        const int fw = kFieldWarps;                              // one pair of warps per star
         const size_t fsmem = field_smem_bytes(p->nb, p->kmax, fw, max_n);
         if (2 * (fsmem + 1024) <= (size_t)p->max_smem_sm && fsmem <= (size_t)p->max_smem_optin) {
             int ctas_per_sm = (int)((size_t)p->max_smem_sm / (fsmem + 1024));
@@ -558,8 +557,7 @@ int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_ou
             L.tiles_per_item = tpi; L.kernel = 4; L.ws_shape = -1;
             a.kernel = 4; a.threads = fw * 32; a.pts_in_smem = 1; a.tiles_per_item = tpi; a.items_per_curve = (int)L.items;
             a.nrows = search_rows_for(p->nb, p->kmax, 0);
-            const int merge_flag = (int)((p->flags >> 24) & 7u);
-            a.merge_warps = merge_flag >= 1 ? merge_flag : (fw < 4 ? fw : 4);
+            a.merge_warps = 2;
         }
     }
     p->last_max_n = max_n;

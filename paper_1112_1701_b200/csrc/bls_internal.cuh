@@ -53,7 +53,7 @@ constexpr int kSmallWarps = 2;        // small shapes: kernel 1 with CTAs of thi
 constexpr int kSmallCtasMin = 8;      // ... when at least this many fit an SM
 constexpr int kWtWarps = 5;           // warp-per-tile kernel: warps per CTA (two CTAs per SM)
 constexpr int kFieldStars = 3;        // field kernel (kernel 4): stars of a field per CTA that share each epoch's bin index
-constexpr int kFieldWarps = 4;        // ... and its CTA size in warps (BLS_FLAG_WARPS overrides)
+constexpr int kFieldWarps = 2 * kFieldStars;   // ... and its CTA: all warps fold, then one pair of warps per star searches and merges
 constexpr int kPrepThreads = 256;
 constexpr int kPeakThreads = 256;
 

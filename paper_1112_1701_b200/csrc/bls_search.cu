@@ -1193,30 +1193,38 @@ search_field_kernel(const SearchArgs a)
     const uint32_t G = (uint32_t)a.nb + 8u;
     unsigned int n_canon = 0;
 
+    // After the shared fold the CTA splits into S pairs of warps, one pair per star, each with its own named barrier:
+    // pair s extends, searches and merges star s's buffer exactly as a two-warp CTA of kernel 1 would, then zeroes
+    // that buffer for the next tile.  Two CTA barriers per tile: bins zeroed -> fold, fold -> pairs.
+    const int s_mine = warp >> 1, pw = warp & 1, ptid = tid & 63;
+    const bool mine_ok = metas[s_mine].status == BLS_CURVE_OK;                 // uniform over the pair
+    const uint32_t buf = bins_s + s_mine * buf_bytes;
+    float *pc_t = cand_t + s_mine * 64, *pp_v = post_v + s_mine * 64;
+    uint32_t *pc_c = cand_c + s_mine * 64, *pp_k = post_k + s_mine * 64;
+    const int bar = 1 + s_mine;
+    TileCtx c;
+    load_ctx(c, a, metas[s_mine], a.nrows);
+    c.n_pad = n_pad;
+    const OutPtrs outp = out_rows(a, local0 + min(s_mine, ns - 1), cv0 + min(s_mine, ns - 1));
+    zero_bins(buf, a.nb, ptid, 64);
+    __syncthreads();
     LaneFreq lf_next = lane_freq(a, cv0, tile0 * kTileFreqs + lane);
     for (int tile = tile0; tile < tile1; ++tile) {
         const int q0 = tile * kTileFreqs;
         const LaneFreq lf = lf_next;
-#pragma unroll
-        for (int s = 0; s < S; ++s) zero_bins(bins_s + s * buf_bytes, a.nb, tid, nthr);
-        __syncthreads();
         fold_field_tile<S>(a.nb, G, force_canon, lf, bins_s, buf_bytes, frec_sa, n_pad, metas, lane, warp, nw, n_canon);
         if (tile + 1 < tile1) lf_next = lane_freq(a, cv0, q0 + kTileFreqs + lane);
         __syncthreads();
-        for (int s = 0; s < ns; ++s) {
-            if (metas[s].status != BLS_CURVE_OK) continue;                     // CTA-uniform
-            TileCtx c;
-            load_ctx(c, a, metas[s], a.nrows);
-            c.n_pad = n_pad;
-            const uint32_t buf = bins_s + s * buf_bytes;
-            extend_rows(c, buf, tid, nthr);
-            __syncthreads();
-            search_warp<kSmax>(buf, c, lane, warp, nw, cand_t, cand_c);
-            __syncthreads();
-            merge_tile(c, buf, cand_t, cand_c, post_v, post_k, nw, min(nw, a.merge_warps), warp, lane, q0 + lane, a.nf,
-                       out_rows(a, local0 + s, cv0 + s), [] { __syncthreads(); });
-            __syncthreads();
+        if (mine_ok) {
+            extend_rows(c, buf, ptid, 64);
+            named_sync(bar, 64);
+            search_warp<kSmax>(buf, c, lane, pw, 2, pc_t, pc_c);
+            named_sync(bar, 64);
+            merge_tile(c, buf, pc_t, pc_c, pp_v, pp_k, 2, 2, pw, lane, q0 + lane, a.nf, outp, [bar] { named_sync(bar, 64); });
+            named_sync(bar, 64);
+            zero_bins(buf, a.nb, ptid, 64);
         }
+        __syncthreads();
     }
     count_canonical(a, n_canon, lane);
 }
