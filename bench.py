@@ -15,7 +15,8 @@ configuration whose 20 timed steps fit the driver's bench arm.  Prints ONE JSON 
   roofline     the search kernel against the issue-rate roofline stated in DESIGN.md section 7
   cpu_baseline the oracle as it stands on the host cores, bounded sample, and the parity of the timed
                step's peaks against it
-  per_config   C0, C1, C3 (full) and C4 (full): one timed step each (after warm-up), same fields in short
+  per_config   C0, C1, C3 (full) and C4 (full): one timed step each (after warm-up), same fields in short;
+               F2: bls_run_field at the paper's cadence, field kernel against the per-star kernels
 With --impl reference the oracle itself is the timed arm (rank 0 only).
 """
 from __future__ import annotations
@@ -404,6 +405,44 @@ def time_config(name, cfg, steps, warmup, *, rank=0, world=1, dist=None, local_r
     return out
 
 
+def time_field(local_rank=0, n_stars=30000, nf=5000, nb=64, steps=3):
+    """per_config["F2"]: bls_run_field on one synthetic pointing at the paper's cadence (140 and 300 shared epochs,
+    2 % absent, 64 bins, widths 1..10), through the field kernel (three stars per CTA share each epoch's bin index)
+    and through the per-star kernels on the same inputs: search-kernel time from the library's own CUDA events."""
+    import torch
+    import paper_1112_1701_b200 as bls
+    from paper_1112_1701_b200 import binding as B
+    dev = torch.device("cuda", local_rank)
+    props = torch.cuda.get_device_properties(dev)
+    clk = props.clock_rate * 1e3                     # max SM clock, Hz (as the roofline block uses)
+    grid = synth.Grid(nf, 0.1, 5.0, nb, 0.01, 0.15)
+    freqs = synth.freq_grid(grid)
+    out = {"workload": "F2: one pointing, %d stars x {140, 300} shared epochs (2 %% absent), %d freqs in [0.1,5]/d, %d bins, "
+                       "q in [0.01,0.15], top-5" % (n_stars, nf, nb), "steps": steps}
+    for n_epochs in (140, 300):
+        t, mag, sig = synth.make_field(n_stars, n_epochs, seed=n_epochs)
+        td, md, sd = (torch.from_numpy(x).to(dev) for x in (t, mag, sig))
+        n_present = int(np.isfinite(mag).sum())
+        row = {}
+        for name, flags in (("field_kernel", 0), ("per_star_kernels", B.BLS_FLAG_NO_FIELD_KERNEL)):
+            with bls.Plan(n_bins=nb, q_min=grid.qmin, q_max=grid.qmax, freqs=freqs, max_top_k=5, device=local_rank, flags=flags) as plan:
+                for _ in range(3):
+                    plan.run_field(td, md, sd, 0.0)
+                    plan.topk(5)
+                ns = []
+                for _ in range(steps):
+                    plan.run_field(td, md, sd, 0.0)
+                    plan.topk(5)
+                    ns.append(plan.query(B.QUERY_LAST_SEARCH_NS))
+                sec = float(np.mean(ns)) * 1e-9
+                row[name] = {"kernel": int(plan.query(B.QUERY_SEARCH_KERNEL)), "search_ms": sec * 1e3,
+                             "clk_per_pair": props.multi_processor_count * clk * sec / (n_stars * nf),
+                             "point_folds_per_sec": n_present * nf / sec, "stars_per_sec": n_stars / sec}
+        row["speedup"] = row["per_star_kernels"]["search_ms"] / row["field_kernel"]["search_ms"]
+        out["E%d" % n_epochs] = row
+    return out
+
+
 PER_CONFIG = [("C0", 0), ("C1", 0), ("C3", 100), ("C4", 20000)]     # (name, curves of the warm-up prefix; 0 = whole batch)
 
 
@@ -479,6 +518,10 @@ def main():
             except Exception as e:  # a secondary line must not sink the headline
                 per_config[name] = {"error": repr(e)[:300]}
         per_config[args.config] = short(r)
+        try:
+            per_config["F2"] = time_field(local_rank)
+        except Exception as e:
+            per_config["F2"] = {"error": repr(e)[:300]}
 
     line = {"metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",

@@ -10,5 +10,6 @@ from .lightcurves import (  # noqa: F401
     freq_grid,
     make_batch,
     make_curve,
+    make_field,
     curve_lengths,
 )

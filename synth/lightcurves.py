@@ -233,3 +233,27 @@ def make_batch(cfg: dict, curve_ids: Optional[Sequence[int]] = None, workers: in
     cat = (lambda j, dt: np.concatenate([p[j] for p in parts]).astype(dt, copy=False))
     return Batch(offsets=offsets, t=cat(1, np.float32), mag=cat(2, np.float32), sigma=cat(3, np.float32),
                  t_origin=cat(4, np.float64), curve_ids=curve_ids, truth=[tr for p in parts for tr in p[5]])
+
+
+def make_field(n_stars: int, n_epochs: int, seed: int = 0, absent_frac: float = 0.02):
+    """One pointing in the field layout of bls_run_field (row f2): every star is measured on the same exposures
+    (about 3,000 M-dwarfs per pointing; L115: 0-2 % of the epochs rejected; L121: 140 epochs in the
+    figure's example, 300-epoch sets).  Returns (t [n_epochs] float32 days from the first epoch, mag and sigma
+    [n_stars, n_epochs] float32 with absent entries marked by NaN magnitudes).  The cadence is the first n_epochs
+    of a C1 curve's PTF-like cadence; per-star noise floors are log-normal around 10 mmag; every third star carries
+    box eclipses (P 0.3-3 d, depth 0.03-0.2 mag, q 0.02-0.08).  Inputs only: none of the BLS arithmetic."""
+    rng = np.random.Generator(np.random.Philox(key=SEED_BASE + 977, counter=[0, int(seed), 0, 0]))
+    t = make_curve(CONFIGS["C1"], 77)[0][:n_epochs].astype(np.float32)
+    assert t.size == n_epochs, "C1 cadences have 1,500 epochs"
+    star = 0.01 * 10.0 ** (0.5 * rng.normal(size=(n_stars, 1)))
+    sig = (star * (1.0 + 0.25 * np.abs(rng.normal(size=(n_stars, n_epochs))))).astype(np.float32)
+    mag = rng.uniform(14.0, 18.0, size=(n_stars, 1)) + rng.normal(size=(n_stars, n_epochs)) * sig
+    inj = np.arange(n_stars) % 3 == 0
+    P = rng.uniform(0.3, 3.0, size=(n_stars, 1))
+    depth = rng.uniform(0.03, 0.2, size=(n_stars, 1))
+    q = rng.uniform(0.02, 0.08, size=(n_stars, 1))
+    T0 = rng.uniform(0.0, 1.0, size=(n_stars, 1)) * P
+    in_box = (((t[None, :].astype(np.float64) - T0) / P) % 1.0) < q
+    mag = np.where(inj[:, None] & in_box, mag + depth, mag).astype(np.float32)
+    mag[rng.uniform(size=mag.shape) < absent_frac] = np.nan
+    return t, mag, sig
