@@ -58,6 +58,8 @@ def lib():
                                        _f64p, _f64p]
         L.oracle_peaks.restype = C.c_int
         L.oracle_peaks.argtypes = [C.c_int64, _f64p, C.c_int, _i64p]
+        L.oracle_peaks_sep.restype = C.c_int
+        L.oracle_peaks_sep.argtypes = [C.c_int64, _f64p, C.c_int, C.c_int64, _i64p]
         L.oracle_bins_many.restype = None
         L.oracle_bins_many.argtypes = [C.c_int64, _f64p, _f64p, C.c_int, _i32p]
         L.oracle_detection_efficiency.restype = None
@@ -135,6 +137,14 @@ def peaks(sr, kpk: int) -> np.ndarray:
     sr = np.ascontiguousarray(sr, dtype=np.float64)
     idx = np.full(kpk, -1, dtype=np.int64)
     lib().oracle_peaks(sr.size, sr, kpk, idx)
+    return idx
+
+
+def peaks_sep(sr, kpk: int, min_sep: int) -> np.ndarray:
+    """Reading R14 with the exact greedy minimum separation (oracle_peaks_sep)."""
+    sr = np.ascontiguousarray(sr, dtype=np.float64)
+    idx = np.full(kpk, -1, dtype=np.int64)
+    lib().oracle_peaks_sep(sr.size, sr, kpk, int(min_sep), idx)
     return idx
 
 

@@ -28,6 +28,9 @@
  *                         with closed-form depth and SR, invariants                   (pinned)
  *   oracle_sr_at        - same brute force, box/complement symmetry                   (pinned)
  *   oracle_peaks        - hand-written spectra with answers written out               (pinned)
+ *   oracle_peaks_sep    - hand-written spectra with answers written out (a rejected peak
+ *                         suppresses nothing; "more than" is strict), min_sep = 0 equals
+ *                         oracle_peaks, brute force over all subsets on small spectra  (pinned)
  *   oracle_sde          - hand-written spectra, closed form                           (pinned)
  *   oracle_bin_shift    - exact rational arithmetic with a bin-grid shift              (pinned)
  *   oracle_detection_efficiency - closed forms on regular cadences (d/P, 2d/P), degenerate cases,
@@ -211,6 +214,44 @@ int oracle_peaks(int64_t nf, const double *sr, int kpk, int64_t *idx)
         idx[pos] = q;
         if (found < kpk) ++found;
     }
+    return found;
+}
+
+/* Reading R14 with a minimum separation (SURVEY.md section 8(c) reading 14, the optional `peak_min_sep`): on a
+ * fine grid the highest local maxima around one signal are its own sidelobes, and a list of candidates (PAPER.md
+ * L151) should not spend every slot on one of them.  Exact greedy rule: walk ALL peaks of O5 in (SR descending,
+ * index ascending) order; accept a peak iff its index is MORE than min_sep grid steps from every peak accepted so
+ * far; stop at kpk.  A rejected peak suppresses nothing.  min_sep = 0 is oracle_peaks.  Returns the number written;
+ * idx[] is padded with -1. */
+int oracle_peaks_sep(int64_t nf, const double *sr, int kpk, int64_t min_sep, int64_t *idx)
+{
+    for (int j = 0; j < kpk; ++j) idx[j] = -1;
+    int64_t *pk = (int64_t *)malloc(sizeof(int64_t) * (size_t)(nf > 0 ? nf : 1));
+    int64_t np = 0;
+    for (int64_t q = 0; q < nf; ++q) {                      /* the peaks of O5, in index order */
+        if (!(sr[q] > 0.0)) continue;
+        if (q > 0 && !(sr[q] > sr[q - 1])) continue;
+        if (q < nf - 1 && !(sr[q] >= sr[q + 1])) continue;
+        pk[np++] = q;
+    }
+    int found = 0;
+    unsigned char *used = (unsigned char *)calloc((size_t)(np > 0 ? np : 1), 1);
+    while (found < kpk) {
+        /* the best peak not yet visited: largest SR, then smallest index (pk[] is in index order) */
+        int64_t b = -1;
+        for (int64_t i = 0; i < np; ++i)
+            if (!used[i] && (b < 0 || sr[pk[i]] > sr[pk[b]])) b = i;
+        if (b < 0) break;
+        used[b] = 1;
+        int far = 1;
+        for (int j = 0; j < found; ++j) {
+            int64_t d = pk[b] - idx[j];
+            if (d < 0) d = -d;
+            if (d <= min_sep) far = 0;
+        }
+        if (far) idx[found++] = pk[b];
+    }
+    free(pk); free(used);
     return found;
 }
 
