@@ -176,6 +176,15 @@ int bls_run_field(bls_plan *plan, const bls_field_batch *field, const bls_output
  * cuda_stream (the stream of that run, or one ordered after it). */
 int bls_topk(bls_plan *plan, int32_t k, bls_peak *peaks, void *cuda_stream);
 
+/* Minimum separation between the peaks of a curve, in steps of the frequency grid (SURVEY.md section 8(c) reading 14;
+ * the candidates of PAPER.md L151).  On a fine grid (C3: 500,000 frequencies) the highest local maxima around one
+ * signal are its own sidelobes and fill every slot of the list.  With steps > 0 the list is built greedily: peaks
+ * (reading R14) are taken in (SR descending, index ascending) order and one is accepted iff its index is MORE than
+ * `steps` away from every peak accepted before it; a rejected peak suppresses nothing.  0 (the default) is plain
+ * R14.  Takes effect at the next bls_run / bls_run_field / bls_search_host (the peak candidates are picked there);
+ * bls_topk and bls_refine then see the separated list.  0 <= steps <= 2^27, else BLS_ERR_ARG. */
+int bls_plan_set_peak_min_sep(bls_plan *plan, int32_t steps);
+
 /* Convenience for callers whose data lives in HOST memory: copies the batch to the device, runs
  * bls_run + bls_topk, copies peaks (HOST, [n_curves*k]) and status (HOST, [n_curves], may be NULL)
  * back, and synchronises.  host_batch uses HOST pointers for t / mag / sigma as well. */

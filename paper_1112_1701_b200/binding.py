@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libbls_b200.so")
 EXPORTS = ["bls_plan_create", "bls_run", "bls_topk", "bls_search_host", "bls_plan_destroy",
            "bls_plan_query", "bls_strerror", "bls_plan_last_cuda_error", "bls_debug_fold_bins",
            "bls_variability", "bls_refine", "bls_detection_efficiency", "bls_run_field", "bls_variability_noalloc",
-           "bls_debug_fold_bins_shift"]
+           "bls_debug_fold_bins_shift", "bls_plan_set_peak_min_sep"]
 
 BLS_OK = 0
 BLS_ERR_NULL, BLS_ERR_CONFIG, BLS_ERR_BATCH, BLS_ERR_ARG, BLS_ERR_CUDA, BLS_ERR_UNSUPPORTED = -1, -2, -3, -4, -5, -6
@@ -138,6 +138,8 @@ def lib():
         L.bls_debug_fold_bins_shift.restype = C.c_int
         L.bls_debug_fold_bins_shift.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_int32,
                                                 C.c_uint32, C.c_void_p, C.POINTER(C.c_int64)]
+        L.bls_plan_set_peak_min_sep.restype = C.c_int
+        L.bls_plan_set_peak_min_sep.argtypes = [C.c_void_p, C.c_int32]
         L.bls_refine.restype = C.c_int
         L.bls_refine.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
         L.bls_detection_efficiency.restype = C.c_int
@@ -401,6 +403,11 @@ class Plan:
             stream = torch.cuda.current_stream(dev).cuda_stream
         self._check(lib().bls_topk(self._h, int(k), C.c_void_p(out.data_ptr()), C.c_void_p(stream)))
         return out[: self._n_curves * k * PEAK_DTYPE.itemsize]
+
+    def set_peak_min_sep(self, steps: int) -> None:
+        """bls_plan_set_peak_min_sep: greedy minimum separation (grid steps) between a curve's reported peaks, from the
+        next run on; 0 = plain top-k local maxima."""
+        self._check(lib().bls_plan_set_peak_min_sep(self._h, int(steps)))
 
     # -- bls_refine --------------------------------------------------------------------------------
     def refine(self, k: int, n_fine: int = 64, n_shift: int = 4, stream: Optional[int] = None) -> np.ndarray:

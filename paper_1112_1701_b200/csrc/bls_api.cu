@@ -20,6 +20,7 @@ struct bls_plan {
     int max_smem_sm = 0;
     int64_t nf = 0;
     int nb = 0, kmin = 0, kmax = 0, max_top_k = 0;
+    int peak_min_sep = 0;           // grid steps between reported peaks (bls_plan_set_peak_min_sep; 0 = plain R14)
     uint32_t flags = 0;
     double fmax = 0.0;
     int64_t scratch_budget = 0;
@@ -582,7 +583,7 @@ int run_impl(bls_plan *p, const bls_batch *b, int64_t field_epochs, const bls_ou
         BLS_CUDA(p, cudaEventRecord(p->ev[p->ev_used + 1], st));
         p->ev_used += 2;
         BLS_CUDA(p, launch_peaks(p->d_sr, p->d_ak, p->d_depth, p->d_meta, base, cc, (int)p->nf,
-                                 p->max_top_k, p->d_cand, p->d_sr_stats, st));
+                                 p->max_top_k, p->peak_min_sep, p->d_cand, p->d_sr_stats, st));
         p->last_launches += 2;
         p->last_search_ctas += (L.kernel == 4 ? (cc + kFieldStars - 1) / kFieldStars : cc) * L.items;
     }
@@ -729,6 +730,14 @@ int bls_detection_efficiency(int32_t device, const bls_batch *b, int64_t n_freq,
                           min_events, count ? count : (int32_t *)(scr + o_cnt), efficiency ? efficiency : (double *)(scr + o_eff), st);
     const cudaError_t e2 = cudaFreeAsync(scr, st);
     if (e != cudaSuccess || e2 != cudaSuccess) { cudaGetLastError(); return BLS_ERR_CUDA; }
+    return BLS_OK;
+}
+
+int bls_plan_set_peak_min_sep(bls_plan *p, int32_t steps)
+{
+    if (!p) return BLS_ERR_NULL;
+    if (steps < 0 || steps > (1 << 27)) return BLS_ERR_ARG;
+    p->peak_min_sep = steps;
     return BLS_OK;
 }
 

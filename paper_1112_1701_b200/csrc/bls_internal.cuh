@@ -184,7 +184,7 @@ cudaError_t launch_window(const float *t, const int64_t *d_offsets, int64_t n_cu
                           double duration, int n_phase, int min_events, int32_t *count, double *eff, cudaStream_t st);
 cudaError_t launch_search(const SearchArgs &a, int64_t chunk_curves, size_t smem, cudaStream_t st);
 cudaError_t launch_peaks(const float *sr, const uint32_t *ak, const float *depth, const CurveMeta *meta,
-                         int64_t curve_base, int64_t chunk_curves, int nf, int max_k, PeakCand *cand,
+                         int64_t curve_base, int64_t chunk_curves, int nf, int max_k, int min_sep, PeakCand *cand,
                          double2 *sr_stats, cudaStream_t st);
 cudaError_t launch_refine_grid(const PeakCand *cand, int max_k, int k, int64_t n_curves, int nf, int n_fine,
                                const double *freqs, double *f_lo, double *f_step, cudaStream_t st);

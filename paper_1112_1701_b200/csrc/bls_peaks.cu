@@ -4,6 +4,10 @@
 // selects max_k peaks in max_k rounds; each round is a block-wide argmax over the candidates that
 // rank strictly after the previous pick.  The spectrum row is nf*4 bytes (<= 2 MB) and stays in
 // L1/L2 across rounds, so HBM sees it once.
+// With a minimum separation (bls_plan_set_peak_min_sep; SURVEY 8(c) reading 14) a candidate must also lie MORE than
+// min_sep grid steps from every peak picked in the earlier rounds: the round's argmax over the peaks that are still
+// allowed is exactly the greedy walk in rank order (a peak passed over because it was too close stays too close,
+// the accepted set only grows, and it suppresses nothing itself).
 #include "bls_internal.cuh"
 
 namespace bls {
@@ -16,9 +20,10 @@ __device__ __forceinline__ unsigned long long rank_key(float sr, int q)
 
 __global__ void __launch_bounds__(kPeakThreads)
 peaks_kernel(const float *__restrict__ sr, const uint32_t *__restrict__ ak, const float *__restrict__ depth,
-             const CurveMeta *__restrict__ meta, int64_t curve_base, int nf, int max_k,
+             const CurveMeta *__restrict__ meta, int64_t curve_base, int nf, int max_k, int min_sep,
              PeakCand *__restrict__ cand, double2 *__restrict__ sr_stats)
 {
+    __shared__ int s_acc[32];                  // indices picked so far (max_top_k <= 32)
     __shared__ unsigned long long sh[kPeakThreads / 32];
     __shared__ double shd[kPeakThreads / 32];
     __shared__ unsigned long long s_prev;
@@ -51,7 +56,12 @@ peaks_kernel(const float *__restrict__ sr, const uint32_t *__restrict__ ak, cons
                 if (q > 0 && !(v > row[q - 1])) continue;
                 if (q < nf - 1 && !(v >= row[q + 1])) continue;
                 const unsigned long long key = rank_key(v, q);
-                if (key < prev && key > best) best = key;
+                if (key < prev && key > best) {
+                    bool far = true;
+                    if (min_sep > 0)
+                        for (int j = 0; j < round; ++j) far = far && abs(q - s_acc[j]) > min_sep;
+                    if (far) best = key;
+                }
             }
         }
 #pragma unroll
@@ -71,6 +81,7 @@ peaks_kernel(const float *__restrict__ sr, const uint32_t *__restrict__ ak, cons
             else {
                 const int q = (int)(0xffffffffu - (uint32_t)(b & 0xffffffffull));
                 pc.freq_index = q;
+                s_acc[round] = q;
                 pc.sr = row[q];
                 pc.depth = depth[cl * (int64_t)nf + q];
                 pc.ak = ak[cl * (int64_t)nf + q];
@@ -220,12 +231,12 @@ cudaError_t launch_refine_reduce(const float *sr, const uint32_t *ak, const floa
 }
 
 cudaError_t launch_peaks(const float *sr, const uint32_t *ak, const float *depth, const CurveMeta *meta,
-                         int64_t curve_base, int64_t chunk_curves, int nf, int max_k, PeakCand *cand,
+                         int64_t curve_base, int64_t chunk_curves, int nf, int max_k, int min_sep, PeakCand *cand,
                          double2 *sr_stats, cudaStream_t st)
 {
     static_assert(kPeakThreads == kPrepThreads, "block_sum's shape");
     if (chunk_curves <= 0) return cudaSuccess;
-    peaks_kernel<<<(unsigned)chunk_curves, kPeakThreads, 0, st>>>(sr, ak, depth, meta, curve_base, nf, max_k, cand, sr_stats);
+    peaks_kernel<<<(unsigned)chunk_curves, kPeakThreads, 0, st>>>(sr, ak, depth, meta, curve_base, nf, max_k, min_sep, cand, sr_stats);
     return cudaGetLastError();
 }
 
